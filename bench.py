@@ -1,0 +1,320 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the fused SK + polarization-alignment flag-and-average pass on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload lofar] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (one rfi_process_chunk = one kernel launch) over one chunk of
+seeded synthetic correlator output that is already resident in HBM.  The default workload is
+BASELINE.json configs[1] (LOFAR-subband-scale fp32, 18.5 GB, far larger than the 126 MB L2, so no cache
+flush is needed between iterations).  One JSON line is printed by rank 0 (see README / DESIGN.md for keys).
+
+N > 1 (launched by torchrun): the path shards by baseline with no data-path collective (every cell is an
+independent stream), so every rank processes its own chunk ("scaling": "weak"); the timed region
+is bracketed by a barrier and the time is the max over ranks.
+
+--impl reference times the fp64 CPU oracle (oracle/), as it stands, on the host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "visibility samples/s (flag+average, fused SK + polarization alignment)"
+UNIT = "samples/s"
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, torch copy_)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def load_ncu_traffic(workload: str, variant: str):
+    """dram bytes per launch of the dominant kernel from the committed ncu --set full capture, or None."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
+            t = json.load(f)
+        return t.get(f"{workload}:{variant}")
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._pump, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_baseline(vis_np, w, thr, target_cpu_seconds=15.0):
+    """Time the fp64 oracle, as it stands, on a bounded sample of the workload (all host cores)."""
+    from oracle import rfi_oracle as orc
+    cores = orc.max_threads()
+    n_cells = vis_np.shape[1]
+    probe = min(n_cells, 64)
+    t0 = time.perf_counter()
+    orc.process(vis_np[:, :probe], w.window_M, w.n_int, thr, n_threads=cores, want_stats=False)
+    dt = max(time.perf_counter() - t0, 1e-4)
+    per_cell_cpu = dt * min(cores, probe) / probe
+    use = int(max(probe, min(n_cells, target_cpu_seconds / per_cell_cpu)))
+    t0 = time.perf_counter()
+    orc.process(vis_np[:, :use], w.window_M, w.n_int, thr, n_threads=cores, want_stats=False)
+    dt = time.perf_counter() - t0
+    samples = use * vis_np.shape[0]
+    return {"value": samples / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{use} of {w.n_cells} cells x all {vis_np.shape[0]} time samples of the same chunk "
+                      f"({samples} samples, {dt:.2f} s wall, OpenMP over cells)"}
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, each step a bounded sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import numpy as np
+    from oracle import rfi_oracle as orc
+    from paper_2412_14775_b200 import synth
+    w = synth.WORKLOADS[args.workload]
+    thr = synth.default_thresholds(w.window_M)
+    cores = orc.max_threads()
+    # bounded sample: few stations of the same recipe, all time samples; sized so K+W steps end within minutes
+    ns = 6
+    ws = w.scaled(n_stations=ns, burst_cell_frac=max(w.burst_cell_frac, 0.02))
+    vis, _ = synth.make_chunk(ws, seed=1234, device="cpu")
+    v = vis.numpy().reshape(ws.n_time, ws.n_cells, 4, 2)
+    steps, warm = max(1, min(args.steps, 5)), max(1, min(args.warmup, 2))
+    for _ in range(warm):
+        orc.process(v, ws.window_M, ws.n_int, thr, n_threads=cores, want_stats=False)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        orc.process(v, ws.window_M, ws.n_int, thr, n_threads=cores, want_stats=False)
+    dt = (time.perf_counter() - t0) / steps
+    samples = ws.n_time * ws.n_cells
+    val = samples / dt
+    sample = (f"{ws.n_cells} of {w.n_cells} cells ({ns} stations incl. autos) x all {ws.n_time} time samples per step; "
+              f"{steps} timed steps after {warm} warm-up")
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+        "warmup": warm, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic (seeded; stands in for LOFAR data)",
+        "config": {"workload": f"{w.name}: BASELINE.json configs[1] recipe, bounded sample", "sample": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import paper_2412_14775_b200 as rfi
+    from paper_2412_14775_b200 import synth
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    w = synth.WORKLOADS[args.workload]
+    thr = synth.default_thresholds(w.window_M) if args.K <= 1 else synth.sweep_thresholds(w.window_M, args.K)
+    vis, truth = synth.make_chunk(w, seed=1234 + rank, device=dev)
+    plan = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M,
+                       rfi.RFI_FP16 if w.fp16 else rfi.RFI_FP32, n_int=w.n_int)
+    plan.set_thresholds(thr)
+    plan.set_variant(args.variant)
+    avg, weight, _ = plan.alloc_outputs(device=dev)
+    out_bytes = avg.numel() * 4 + weight.numel() * 4 + max(plan.K, 1) * plan.n_win * plan.n_baselines * plan.wpb * 4
+    algo_bytes = w.input_bytes + out_bytes
+    samples = w.n_time * w.n_cells
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        plan.process_chunk(vis, avg, weight)
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    if sampler:
+        sampler.start()
+        time.sleep(0.3)
+    launches0 = plan.launch_count
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    t_start = torch.cuda.Event(enable_timing=True); t_end = torch.cuda.Event(enable_timing=True)
+    t_start.record()
+    for a, b in evs:
+        a.record()
+        plan.process_chunk(vis, avg, weight)      # on torch's current stream, where the events are recorded
+        b.record()
+    t_end.record()
+    barrier()
+    total_ms = t_start.elapsed_time(t_end)
+    kernel_ms = [a.elapsed_time(b) for a, b in evs]
+    launches = plan.launch_count - launches0
+    clocks = sampler.stop() if sampler else None
+    if dist is not None:
+        t = torch.tensor([total_ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    value = world * samples / (ms_per_step * 1e-3)
+
+    # a little science on the way out (not timed): detection quality against the injected ground truth
+    flags = rfi.unpack_flags(plan.get_flags(), w.n_chan).reshape(max(plan.K, 1), plan.n_win, plan.n_cells)
+    tr = truth.reshape(plan.n_win, plan.n_cells)
+    fa = float((flags[0] & ~tr).sum() / max((~tr).sum(), 1))
+    md = float((~flags[0] & tr).sum() / max(tr.sum(), 1))
+
+    if rank != 0:
+        if dist is not None:
+            dist.barrier()
+            dist.destroy_process_group()
+        return
+
+    peak, peak_src = load_peaks()
+    k_ms = statistics.mean(kernel_ms)
+    achieved = algo_bytes / (k_ms * 1e-3) / 1e9
+    variant = plan.last_variant
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": load_ncu_traffic(w.name, variant), "peak_source": peak_src,
+                "kernel": f"rfi_{variant}_kernel", "kernel_ms_mean": k_ms, "kernel_ms_min": min(kernel_ms),
+                "algorithmic_bytes_per_launch": algo_bytes,
+                "frac_of_nominal_8TBs": achieved / 8000.0}
+
+    # end to end through the C ABI with HOST buffers (H2D of the inputs and D2H of the results inside the timed region)
+    e2e = None
+    if not args.no_e2e:
+        try:
+            h_vis = torch.empty(vis.shape, dtype=vis.dtype, pin_memory=True)
+            h_vis.copy_(vis)
+            K = max(plan.K, 1)
+            h_avg = torch.empty(avg.shape, dtype=torch.float32, pin_memory=True)
+            h_weight = torch.empty(weight.shape, dtype=torch.int32, pin_memory=True)
+            h_flags = torch.empty(K, plan.n_win, plan.n_baselines, plan.wpb, dtype=torch.int32, pin_memory=True)
+            plan.process_chunk_host_into(h_vis, h_avg, h_weight, h_flags)          # warm-up (allocates staging)
+            n_e2e = max(2, min(args.steps, 3))
+            t0 = time.perf_counter()
+            for _ in range(n_e2e):
+                plan.process_chunk_host_into(h_vis, h_avg, h_weight, h_flags)      # synchronises before returning
+            dt = (time.perf_counter() - t0) / n_e2e
+            same = bool(torch.equal(h_avg, avg.cpu()) and torch.equal(h_weight, weight.cpu()))
+            e2e = {"value": world * samples / dt, "unit": UNIT, "h2d_bytes_per_step": w.input_bytes,
+                   "d2h_bytes_per_step": out_bytes, "ms_per_step": dt * 1e3, "steps": n_e2e,
+                   "h2d_gbs": w.input_bytes / dt / 1e9, "matches_device_path": same,
+                   "api": "rfi_process_chunk_host (pinned host buffers; per-integration H2D overlapped with the kernel)"}
+            del h_vis
+        except Exception as exc:  # e.g. not enough pinnable host memory on the box
+            e2e = {"value": None, "unit": UNIT, "h2d_bytes_per_step": w.input_bytes, "d2h_bytes_per_step": out_bytes,
+                   "error": str(exc)[:200]}
+
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        g = torch.Generator().manual_seed(7)
+        n_s = min(w.n_cells, 4096)
+        idx = torch.randperm(w.n_cells, generator=g)[:n_s].sort().values.to(dev)
+        sub = vis.reshape(w.n_time, w.n_cells, 4, 2)[:, idx].cpu().numpy()
+        cpu = oracle_baseline(sub, w, thr)
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32" if not w.fp16 else "f32 (f16 storage)", "data": "synthetic (seeded; stands in for LOFAR data)",
+        "config": {"workload": f"{w.name}: BASELINE.json configs[{list(synth.WORKLOADS).index(w.name)}]",
+                   "n_stations": w.n_stations, "n_baselines": w.n_baselines, "n_chan": w.n_chan, "n_time": w.n_time,
+                   "window_M": w.window_M, "n_int": w.n_int, "K": max(plan.K, 1), "variant": variant,
+                   "input_bytes": w.input_bytes, "l2": "input (>= 9 GB) is far larger than the 126 MB L2: no flush needed",
+                   "sharding": "by baseline, no collective" if world > 1 else "single GPU"},
+        "gbytes_per_s": world * algo_bytes / (ms_per_step * 1e-3) / 1e9,
+        "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+        "detection": {"false_alarm": fa, "missed_detection": md, "flag_fraction": float(flags[0].float().mean())},
+    }
+    print(json.dumps(line))
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="lofar")
+    ap.add_argument("--variant", default="auto", choices=["auto", "direct", "tma"])
+    ap.add_argument("--K", type=int, default=1, help="threshold sets (K > 1: batched sweep)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,132 @@
+/* rfi.h -- C ABI of librfi.so: the fused spectral-kurtosis + polarization-alignment
+ * flag-and-average pass of arxiv 2412.14775 on one B200 (sm_100a).
+ *
+ * Citations are lines of /root/reference/PAPER.md ("PAPER.md:n") with the section / equation.
+ *
+ * The operation (one call of rfi_process_chunk), per (baseline b, channel c) "cell", per window w of
+ * W = window_M consecutive time samples, per threshold set k:
+ *
+ *   Stokes (Eq.(2))      I = xx+yy, Q = xx-yy, U = xy+yx, V = j(xy-yx)       (all complex)
+ *   SK     (Eq.(3)-(4))  S1 = sum|I_i|, S2 = sum|I_i|^2,
+ *                                        tau_k = (W d_k + 1)/(W - 1) * (W S2/S1^2 - 1)
+ *   DS     (Eq.(6)-(9))  for the real parts and for the imaginary parts of (Q,U,V):
+ *                                        p_i = sqrt(q_i^2+u_i^2+v_i^2), r = |sum_i (q_i,u_i,v_i)/p_i| / W
+ *   flag   (Eq.(5),(10))
+ *                                        f_k = (tau_k < s_low_k) OR (tau_k > s_high_k) OR (r_re > gamma_k) OR (r_im > gamma_k)
+ *                                        evaluated as !(tau>=s_low && tau<=s_high) || !(r_re<=gamma) || !(r_im<=gamma)
+ *                                        so that a non-finite statistic flags the window
+ *   excise + average  per output integration o (n_int samples): weight = number of samples in
+ *                                        unflagged windows; avg = sum of those samples / weight (0 if weight = 0)
+ *
+ * Guards: an all-zero window has tau = -(W d + 1)/(W - 1); a sample with p_i = 0 adds the zero vector
+ * (the epsilon -> 0 limit of the paper's epsilon guards).
+ * Arithmetic: fp32 throughout (accumulation included); RFI_FP16 only changes the storage type of the input.
+ * Finite inputs must satisfy 1e-18 <= |x| <= 1e18 or x == 0 (fp32 squares must neither overflow nor
+ * underflow); outside that range the statistics are unspecified (never a fault).
+ *
+ * Memory layouts (all device pointers unless the name starts with h_; all row-major, last index fastest):
+ *   vis     [n_time][n_baselines][n_chan][4 pols: XX,XY,YX,YY][re,im]      float (RFI_FP32) or IEEE half (RFI_FP16)
+ *           time-slowest "correlator dump order"; 32 B (16 B) per sample; base 16-byte aligned.
+ *   avg     [K][n_out][n_baselines][n_chan][4][re,im]   float,    n_out = n_time / n_int
+ *   weight  [K][n_out][n_baselines][n_chan]             uint32_t  (unflagged sample count)
+ *   stats   [3][n_win][n_baselines][n_chan]             float,    planes tau (with d of set 0), r_re, r_im;
+ *                                                                  n_win = n_time / window_M, w counts from chunk start
+ *   flags   [K][n_win][n_baselines][ceil(n_chan/32)]    uint32_t, bit (c % 32) of word c/32, 1 = flagged;
+ *                                                                  unused high bits of a baseline's last word are 0
+ *
+ * Ownership: the caller owns vis/avg/weight/stats and the stream; the plan owns its device threshold table,
+ * its flag buffer and (for the host path) its staging buffers.  vis is read exactly once and never written.
+ * rfi_process_chunk enqueues work on the stream and returns without synchronising the host.
+ *
+ * Errors: every function returns RFI_OK (0) or a negative code; nothing throws or aborts.
+ */
+#ifndef RFI_H_
+#define RFI_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct rfi_plan rfi_plan;            /* opaque host object */
+
+enum { RFI_FP32 = 0, RFI_FP16 = 1 };         /* storage precision of vis */
+
+enum {
+    RFI_OK      =  0,
+    RFI_EINVAL  = -1,   /* bad argument (shape, alignment, NULL, K < 1, d <= 0, ...) */
+    RFI_ECUDA   = -2,   /* a CUDA call failed; rfi_last_cuda_error() has the text */
+    RFI_ENOMEM  = -3,   /* host or device allocation failed */
+    RFI_ESTATE  = -4,   /* call order: thresholds not set, no chunk processed yet, ... */
+    RFI_ENODEV  = -5    /* no CUDA device / not an sm_100 device */
+};
+
+/* kernel variants (rfi_plan_set_variant); all compute the same function */
+enum {
+    RFI_VARIANT_AUTO   = 0,   /* TMA pipeline when the shape allows it, else direct */
+    RFI_VARIANT_DIRECT = 1,   /* per-thread 256-bit global loads, no shared-memory staging */
+    RFI_VARIANT_TMA    = 2    /* warp-private TMA (cp.async.bulk.tensor) ring in shared memory */
+};
+
+/* One threshold set: d of Eq.(4), s_low/s_high of Eq.(5), gamma of Eq.(10)
+ * (PAPER.md:103).  s_low = -inf, s_high = +inf disables the SK test; gamma = +inf disables the DS test. */
+typedef struct { float d, s_low, s_high, gamma; } rfi_thresholds;
+
+/* Create a plan for chunks of n_time samples of n_baselines x n_chan cells (N(N+1)/2 streams,
+ * each mitigated separately).  Requirements (else RFI_EINVAL): n_stations >= 1; n_baselines == N(N+1)/2 or
+ * N(N-1)/2; n_chan >= 1; window_M >= 2 (Eq.(4) divides by W-1); n_time % window_M == 0;
+ * precision in {RFI_FP32, RFI_FP16}.  The integration length defaults to n_time (one output per chunk).
+ * No window may straddle a chunk or integration boundary (no cross-chunk state).  Does not need a GPU
+ * until the first process call. */
+int rfi_plan_create(rfi_plan **out, int n_stations, int n_baselines, int n_chan,
+                    int n_time, int window_M, int precision);
+
+/* Samples per output integration: n_time % n_int == 0 and n_int % window_M == 0, else RFI_EINVAL. */
+int rfi_plan_set_integration(rfi_plan *plan, int n_int);
+
+/* Copy K >= 1 threshold sets from host memory (d > 0 and not NaN; s_low/s_high/gamma may be +-inf, not NaN).
+ * K == 1 runs the single-set kernel; K > 1 the batched kernel that evaluates all sets in one pass over the
+ * data (the paper tunes its thresholds with a host-side search). */
+int rfi_set_thresholds(rfi_plan *plan, int K, const rfi_thresholds *h_sets);
+
+/* Choose a kernel variant (default RFI_VARIANT_AUTO).  RFI_EINVAL if unknown. */
+int rfi_plan_set_variant(rfi_plan *plan, int variant);
+
+/* Process one chunk resident in device memory.  d_stats may be NULL.  cuda_stream is a cudaStream_t
+ * (NULL = legacy default stream).  Asynchronous.  RFI_ESTATE if thresholds were never set; RFI_EINVAL for
+ * NULL / misaligned (16 B) pointers; RFI_ECUDA if a launch failed. */
+int rfi_process_chunk(rfi_plan *plan, const void *d_vis, void *d_avg, void *d_weight,
+                      void *d_stats, void *cuda_stream);
+
+/* Device pointer to the flag mask of the last processed chunk and its length in 32-bit words
+ * (K * n_win * n_baselines * ceil(n_chan/32)).  Valid until the next process call or destroy; reading it is
+ * ordered after the kernel only on the stream that was passed to rfi_process_chunk. */
+int rfi_get_flags(rfi_plan *plan, const uint32_t **d_flags, size_t *n_words);
+
+/* End-to-end host path: vis in HOST memory (pinned for full speed), results to HOST memory.  Streams the
+ * chunk to the device one output integration at a time on two internal streams so that host->device copies
+ * overlap the kernel, then copies avg / weight / flags (and stats if non-NULL) back and synchronises.
+ * Same results as rfi_process_chunk. */
+int rfi_process_chunk_host(rfi_plan *plan, const void *h_vis, void *h_avg, void *h_weight,
+                           void *h_flags, void *h_stats);
+
+int rfi_plan_destroy(rfi_plan *plan);
+
+/* helpers */
+const char *rfi_strerror(int code);
+const char *rfi_last_cuda_error(void);                 /* text of the last failed CUDA call (this thread) */
+size_t rfi_flags_bytes(const rfi_plan *plan);          /* bytes of the flag mask for the current K */
+size_t rfi_avg_bytes(const rfi_plan *plan);            /* bytes the caller must provide for d_avg */
+size_t rfi_weight_bytes(const rfi_plan *plan);
+size_t rfi_stats_bytes(const rfi_plan *plan);
+size_t rfi_vis_bytes(const rfi_plan *plan);
+uint64_t rfi_plan_launch_count(const rfi_plan *plan);  /* kernels launched by this plan so far */
+int rfi_plan_last_variant(const rfi_plan *plan);       /* variant the last process call used */
+const char *rfi_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RFI_H_ */

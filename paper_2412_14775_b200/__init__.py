@@ -1,0 +1,8 @@
+"""B200-native fused spectral-kurtosis + polarization-alignment flag-and-average pass (arxiv 2412.14775).
+
+`RfiPlan` mirrors the C ABI of include/rfi.h (librfi.so, hand-written sm_100a CUDA); `synth` holds the
+seeded input generators.  There is no CPU implementation in this package.
+"""
+from .binding import (RFI_FP16, RFI_FP32, RfiError, RfiPlan, load_library, library_path,  # noqa: F401
+                      unpack_flags)
+from . import synth  # noqa: F401

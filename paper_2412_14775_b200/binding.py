@@ -1,0 +1,212 @@
+"""Thin ctypes binding of librfi.so (include/rfi.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels behind the C ABI; this module holds no arithmetic of
+the method and there is no CPU fallback: if librfi.so is missing or no B200 is present the calls raise.
+PyTorch is used for device memory and streams only.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence
+
+import torch
+
+from . import build as _build
+
+RFI_FP32, RFI_FP16 = 0, 1
+VARIANT_AUTO, VARIANT_DIRECT, VARIANT_TMA = 0, 1, 2
+_VARIANTS = {"auto": 0, "direct": 1, "tma": 2}
+
+EXPORTS = [
+    "rfi_plan_create", "rfi_plan_set_integration", "rfi_set_thresholds", "rfi_plan_set_variant",
+    "rfi_process_chunk", "rfi_get_flags", "rfi_process_chunk_host", "rfi_plan_destroy",
+    "rfi_strerror", "rfi_last_cuda_error", "rfi_flags_bytes", "rfi_avg_bytes", "rfi_weight_bytes",
+    "rfi_stats_bytes", "rfi_vis_bytes", "rfi_plan_launch_count", "rfi_plan_last_variant", "rfi_version",
+]
+
+
+class RfiThresholds(ctypes.Structure):
+    _fields_ = [("d", ctypes.c_float), ("s_low", ctypes.c_float), ("s_high", ctypes.c_float),
+                ("gamma", ctypes.c_float)]
+
+
+class RfiError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        lib = load_library()
+        msg = lib.rfi_strerror(code).decode()
+        cuda = lib.rfi_last_cuda_error().decode()
+        super().__init__(f"{where}: {msg} ({code})" + (f" [{cuda}]" if code in (-2, -5) and cuda else ""))
+        self.code = code
+
+
+_lib = None
+
+
+def library_path() -> str:
+    return _build.LIB
+
+
+def load_library(build_if_missing: bool = True):
+    """dlopen librfi.so (building it with nvcc first if absent or stale).  Raises if it cannot be had."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = library_path()
+    if build_if_missing and (not os.path.exists(path) or _build.is_stale()):
+        _build.build_library()
+    if not os.path.exists(path):
+        raise RuntimeError(f"{path} is missing: run `python -m paper_2412_14775_b200.build` (there is no CPU fallback)")
+    lib = ctypes.CDLL(path)
+    vp, sz, ci = ctypes.c_void_p, ctypes.c_size_t, ctypes.c_int
+    lib.rfi_plan_create.argtypes = [ctypes.POINTER(vp), ci, ci, ci, ci, ci, ci]
+    lib.rfi_plan_set_integration.argtypes = [vp, ci]
+    lib.rfi_set_thresholds.argtypes = [vp, ci, ctypes.POINTER(RfiThresholds)]
+    lib.rfi_plan_set_variant.argtypes = [vp, ci]
+    lib.rfi_process_chunk.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.rfi_get_flags.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(sz)]
+    lib.rfi_process_chunk_host.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.rfi_plan_destroy.argtypes = [vp]
+    for name in ("rfi_plan_create", "rfi_plan_set_integration", "rfi_set_thresholds", "rfi_plan_set_variant",
+                 "rfi_process_chunk", "rfi_get_flags", "rfi_process_chunk_host", "rfi_plan_destroy",
+                 "rfi_plan_last_variant"):
+        getattr(lib, name).restype = ci
+    lib.rfi_strerror.argtypes = [ci]
+    lib.rfi_strerror.restype = ctypes.c_char_p
+    lib.rfi_last_cuda_error.argtypes = []
+    lib.rfi_last_cuda_error.restype = ctypes.c_char_p
+    lib.rfi_version.argtypes = []
+    lib.rfi_version.restype = ctypes.c_char_p
+    for name in ("rfi_flags_bytes", "rfi_avg_bytes", "rfi_weight_bytes", "rfi_stats_bytes", "rfi_vis_bytes"):
+        getattr(lib, name).argtypes = [vp]
+        getattr(lib, name).restype = sz
+    lib.rfi_plan_launch_count.argtypes = [vp]
+    lib.rfi_plan_launch_count.restype = ctypes.c_uint64
+    lib.rfi_plan_last_variant.argtypes = [vp]
+    _lib = lib
+    return lib
+
+
+def _check(code: int, where: str):
+    if code != 0:
+        raise RfiError(code, where)
+
+
+class RfiPlan:
+    """Python face of `rfi_plan` with the same call names as the C ABI."""
+
+    def __init__(self, n_stations: int, n_baselines: int, n_chan: int, n_time: int, window_M: int,
+                 precision: int = RFI_FP32, n_int: Optional[int] = None):
+        self._lib = load_library()
+        self._h = ctypes.c_void_p()
+        _check(self._lib.rfi_plan_create(ctypes.byref(self._h), n_stations, n_baselines, n_chan, n_time,
+                                         window_M, precision), "rfi_plan_create")
+        self.n_stations, self.n_baselines, self.n_chan = n_stations, n_baselines, n_chan
+        self.n_time, self.window_M, self.precision = n_time, window_M, precision
+        self.n_int = n_time
+        self.K = 0
+        if n_int is not None:
+            self.set_integration(n_int)
+
+    # ---- shape helpers -------------------------------------------------------------------------
+    @property
+    def n_cells(self): return self.n_baselines * self.n_chan
+    @property
+    def n_win(self): return self.n_time // self.window_M
+    @property
+    def n_out(self): return self.n_time // self.n_int
+    @property
+    def wpb(self): return (self.n_chan + 31) // 32
+
+    # ---- C ABI ---------------------------------------------------------------------------------
+    def set_integration(self, n_int: int):
+        _check(self._lib.rfi_plan_set_integration(self._h, n_int), "rfi_plan_set_integration")
+        self.n_int = n_int
+
+    def set_thresholds(self, sets: Sequence[Sequence[float]]):
+        arr = (RfiThresholds * len(sets))(*[RfiThresholds(*map(float, s)) for s in sets])
+        _check(self._lib.rfi_set_thresholds(self._h, len(sets), arr), "rfi_set_thresholds")
+        self.K = len(sets)
+
+    def set_variant(self, variant):
+        v = _VARIANTS[variant] if isinstance(variant, str) else int(variant)
+        _check(self._lib.rfi_plan_set_variant(self._h, v), "rfi_plan_set_variant")
+
+    def alloc_outputs(self, device="cuda", stats: bool = False):
+        K = max(self.K, 1)
+        avg = torch.empty(K, self.n_out, self.n_baselines, self.n_chan, 4, 2, dtype=torch.float32, device=device)
+        weight = torch.empty(K, self.n_out, self.n_baselines, self.n_chan, dtype=torch.int32, device=device)
+        st = torch.empty(3, self.n_win, self.n_baselines, self.n_chan, dtype=torch.float32, device=device) if stats else None
+        return avg, weight, st
+
+    def process_chunk(self, vis: torch.Tensor, avg: torch.Tensor, weight: torch.Tensor,
+                      stats: Optional[torch.Tensor] = None, stream: Optional[torch.cuda.Stream] = None):
+        """rfi_process_chunk on torch device tensors (asynchronous on `stream`, default: torch's current stream)."""
+        for t, name in ((vis, "vis"), (avg, "avg"), (weight, "weight")):
+            if not (t.is_cuda and t.is_contiguous()):
+                raise ValueError(f"{name} must be a contiguous CUDA tensor")
+        if vis.numel() * vis.element_size() != self._lib.rfi_vis_bytes(self._h):
+            raise ValueError("vis has the wrong size for this plan")
+        if avg.numel() * 4 != self._lib.rfi_avg_bytes(self._h) or weight.numel() * 4 != self._lib.rfi_weight_bytes(self._h):
+            raise ValueError("avg/weight have the wrong size for this plan (set thresholds before allocating)")
+        if stats is not None and stats.numel() * 4 != self._lib.rfi_stats_bytes(self._h):
+            raise ValueError("stats has the wrong size for this plan")
+        s = stream if stream is not None else torch.cuda.current_stream(vis.device)
+        _check(self._lib.rfi_process_chunk(self._h, vis.data_ptr(), avg.data_ptr(), weight.data_ptr(),
+                                           stats.data_ptr() if stats is not None else None, s.cuda_stream),
+               "rfi_process_chunk")
+
+    def get_flags(self) -> torch.Tensor:
+        """uint32-as-int32 tensor [K, n_win, n_baselines, wpb] aliasing the plan's device flag buffer."""
+        ptr, n = ctypes.c_void_p(), ctypes.c_size_t()
+        _check(self._lib.rfi_get_flags(self._h, ctypes.byref(ptr), ctypes.byref(n)), "rfi_get_flags")
+        shape = (max(self.K, 1), self.n_win, self.n_baselines, self.wpb)
+        assert n.value == shape[0] * shape[1] * shape[2] * shape[3]
+        iface = {"shape": (n.value,), "typestr": "<i4", "data": (ptr.value, False), "version": 2}
+        holder = type("_FlagView", (), {"__cuda_array_interface__": iface})()
+        return torch.as_tensor(holder, device="cuda").view(shape)
+
+    def process_chunk_host(self, vis: torch.Tensor, want_stats: bool = False):
+        """rfi_process_chunk_host: vis is a (preferably pinned) CPU tensor; returns CPU tensors."""
+        if vis.is_cuda or not vis.is_contiguous():
+            raise ValueError("vis must be a contiguous CPU tensor")
+        K = max(self.K, 1)
+        pin = torch.cuda.is_available()
+        avg = torch.empty(K, self.n_out, self.n_baselines, self.n_chan, 4, 2, dtype=torch.float32, pin_memory=pin)
+        weight = torch.empty(K, self.n_out, self.n_baselines, self.n_chan, dtype=torch.int32, pin_memory=pin)
+        flags = torch.empty(K, self.n_win, self.n_baselines, self.wpb, dtype=torch.int32, pin_memory=pin)
+        stats = torch.empty(3, self.n_win, self.n_baselines, self.n_chan, dtype=torch.float32, pin_memory=pin) if want_stats else None
+        self.process_chunk_host_into(vis, avg, weight, flags, stats)
+        return avg, weight, flags, stats
+
+    def process_chunk_host_into(self, vis, avg, weight, flags, stats=None):
+        _check(self._lib.rfi_process_chunk_host(self._h, vis.data_ptr(), avg.data_ptr(), weight.data_ptr(),
+                                                flags.data_ptr(), stats.data_ptr() if stats is not None else None),
+               "rfi_process_chunk_host")
+
+    @property
+    def launch_count(self) -> int:
+        return int(self._lib.rfi_plan_launch_count(self._h))
+
+    @property
+    def last_variant(self) -> str:
+        v = self._lib.rfi_plan_last_variant(self._h)
+        return {0: "none", 1: "direct", 2: "tma"}.get(v, str(v))
+
+    def destroy(self):
+        if self._h:
+            self._lib.rfi_plan_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def unpack_flags(flags: torch.Tensor, n_chan: int) -> torch.Tensor:
+    """[.., n_baselines, wpb] int32 words -> bool [.., n_baselines, n_chan] (layout of include/rfi.h)."""
+    bits = torch.arange(32, device=flags.device, dtype=torch.int32)
+    b = ((flags.unsqueeze(-1) >> bits) & 1).bool()
+    return b.flatten(-2)[..., :n_chan]

@@ -1,0 +1,538 @@
+// rfi_api.cu -- host side of librfi.so: plan object, argument validation, kernel selection and the
+// C ABI declared in include/rfi.h.  No CPU implementation of the method lives here: without a CUDA
+// device every process call fails with RFI_ENODEV / RFI_ECUDA.
+#include "../../include/rfi.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "rfi_kernels.cuh"
+
+namespace {
+
+thread_local char g_cuda_err[512] = "";
+
+bool cuda_ok(cudaError_t e, const char* what) {
+    if (e == cudaSuccess) return true;
+    snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", what, cudaGetErrorString(e));
+    return false;
+}
+#define RFI_CUDA(call)                                  \
+    do {                                                \
+        if (!cuda_ok((call), #call)) return RFI_ECUDA;  \
+    } while (0)
+
+int env_int(const char* name, int dflt) {
+    const char* s = getenv(name);
+    return (s && *s) ? atoi(s) : dflt;
+}
+
+using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn get_encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiledFn>(p);
+    }
+    return fn;
+}
+
+struct MapEntry {
+    const void* ptr;
+    int rows;
+    int R;
+    CUtensorMap map;
+};
+
+}  // namespace
+
+struct rfi_plan {
+    int n_stations, n_baselines, n_chan, n_time, M, precision, n_int;
+    int K = 0;
+    std::vector<rfi_thresholds> thr;
+    int variant = RFI_VARIANT_AUTO;
+    int last_variant = 0;
+    uint64_t launches = 0;
+    // device state (created lazily)
+    int device = -1;
+    int sm_count = 0;
+    int smem_optin = 0;
+    bool dev_ready = false;
+    uint32_t* d_flags = nullptr;
+    size_t flags_words_cap = 0;
+    rfi::Thr* d_thr = nullptr;
+    int d_thr_cap = 0;
+    bool thr_dirty = true;
+    bool have_result = false;
+    std::vector<MapEntry> maps;
+    // host path
+    void* d_stage[2] = {nullptr, nullptr};
+    cudaStream_t streams[2] = {nullptr, nullptr};
+    cudaEvent_t ev_copied[2] = {nullptr, nullptr};
+    cudaEvent_t ev_done[2] = {nullptr, nullptr};
+    float* d_avg = nullptr;
+    uint32_t* d_weight = nullptr;
+    float* d_stats = nullptr;
+    size_t d_avg_cap = 0, d_weight_cap = 0, d_stats_cap = 0;
+
+    size_t n_cells() const { return (size_t)n_baselines * n_chan; }
+    int wpb() const { return (n_chan + 31) / 32; }
+    int n_win() const { return n_time / M; }
+    int n_out() const { return n_time / n_int; }
+    size_t sample_bytes() const { return precision == RFI_FP16 ? 16 : 32; }
+    size_t flags_words() const { return (size_t)(K > 0 ? K : 1) * n_win() * n_baselines * wpb(); }
+};
+
+namespace {
+
+int ensure_device(rfi_plan* p) {
+    if (p->dev_ready) return RFI_OK;
+    int count = 0;
+    if (cudaGetDeviceCount(&count) != cudaSuccess || count == 0) {
+        cudaGetLastError();
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "no CUDA device");
+        return RFI_ENODEV;
+    }
+    RFI_CUDA(cudaGetDevice(&p->device));
+    cudaDeviceProp prop;
+    RFI_CUDA(cudaGetDeviceProperties(&prop, p->device));
+    if (prop.major != 10) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "device %s is sm_%d%d; this library is built for sm_100a only",
+                 prop.name, prop.major, prop.minor);
+        return RFI_ENODEV;
+    }
+    p->sm_count = prop.multiProcessorCount;
+    p->smem_optin = (int)prop.sharedMemPerBlockOptin;
+    // 1/(n+1) table for the running-mean recurrence
+    static bool table_done[64] = {false};
+    if (p->device < 64 && !table_done[p->device]) {
+        std::vector<float> t(rfi::kInvNTable);
+        for (int i = 0; i < rfi::kInvNTable; ++i) t[i] = 1.0f / (float)(i + 1);
+        RFI_CUDA(cudaMemcpyToSymbol(rfi::c_inv_n, t.data(), sizeof(float) * rfi::kInvNTable));
+        table_done[p->device] = true;
+    }
+    p->dev_ready = true;
+    return RFI_OK;
+}
+
+rfi::Thr to_device_thr(const rfi_thresholds& t, int M) {
+    rfi::Thr r;
+    r.c = (float)(((double)M * (double)t.d + 1.0) / ((double)M - 1.0));
+    r.s_low = t.s_low;
+    r.s_high = t.s_high;
+    r.gamma = t.gamma;
+    return r;
+}
+
+int largest_divisor_le(int M, int cap) {
+    for (int r = cap; r >= 1; --r)
+        if (M % r == 0) return r;
+    return 1;
+}
+
+int get_tensor_map(rfi_plan* p, const void* vis, int rows, int R, const CUtensorMap** out) {
+    for (auto& e : p->maps)
+        if (e.ptr == vis && e.rows == rows && e.R == R) { *out = &e.map; return RFI_OK; }
+    EncodeTiledFn enc = get_encode_fn();
+    if (!enc) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "cuTensorMapEncodeTiled entry point not found");
+        return RFI_ECUDA;
+    }
+    MapEntry e;
+    e.ptr = vis; e.rows = rows; e.R = R;
+    CUresult rc;
+    const size_t ncell = p->n_cells();
+    if (p->precision == RFI_FP32) {
+        // {32 floats = 4 cells, n_cells/4 groups, rows}; box {32, 8, R}; 128-byte swizzle
+        cuuint64_t dims[3] = {32, (cuuint64_t)(ncell / 4), (cuuint64_t)rows};
+        cuuint64_t strides[2] = {128, (cuuint64_t)ncell * 32};
+        cuuint32_t box[3] = {32, 8, (cuuint32_t)R};
+        cuuint32_t estr[3] = {1, 1, 1};
+        rc = enc(&e.map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<void*>(vis), dims, strides, box, estr,
+                 CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                 CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    } else {
+        // {n_cells*4 32-bit words, rows}; box {128 words = 32 cells, R}
+        cuuint64_t dims[2] = {(cuuint64_t)ncell * 4, (cuuint64_t)rows};
+        cuuint64_t strides[1] = {(cuuint64_t)ncell * 16};
+        cuuint32_t box[2] = {128, (cuuint32_t)R};
+        cuuint32_t estr[2] = {1, 1};
+        rc = enc(&e.map, CU_TENSOR_MAP_DATA_TYPE_UINT32, 2, const_cast<void*>(vis), dims, strides, box, estr,
+                 CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                 CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    }
+    if (rc != CUDA_SUCCESS) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "cuTensorMapEncodeTiled failed with CUresult %d", (int)rc);
+        return RFI_ECUDA;
+    }
+    if (p->maps.size() >= 16) p->maps.erase(p->maps.begin());
+    p->maps.push_back(e);
+    *out = &p->maps.back().map;
+    return RFI_OK;
+}
+
+bool tma_allowed(const rfi_plan* p) {
+    if (p->precision == RFI_FP32) return p->n_cells() % 4 == 0;      // 128-byte inner box = 4 cells
+    return true;
+}
+
+template <int R, bool FP16>
+int launch_tma_r(rfi_plan* p, const rfi::KParams& kp, const CUtensorMap* map, cudaStream_t st) {
+    const int row_bytes = FP16 ? 512 : 1024;
+    const int stage_bytes = R * row_bytes;
+    int warps = env_int("RFI_TMA_WARPS", 8);
+    int stages = env_int("RFI_TMA_STAGES", 0);
+    if (warps < 1) warps = 1;
+    if (warps > 16) warps = 16;
+    const int budget = p->smem_optin - 1024 - 256;
+    if (stages <= 0) {
+        stages = budget / (warps * (stage_bytes + 8));
+        if (stages > 6) stages = 6;
+    }
+    while (stages > 1 && warps * stages * (stage_bytes + 8) > budget) --stages;
+    while (warps > 1 && warps * stages * (stage_bytes + 8) > budget) --warps;
+    const size_t smem = (size_t)warps * stages * (stage_bytes + 8) + 1024;
+    const int n_tiles = (int)((p->n_cells() + 31) / 32);
+    const long n_units = (long)n_tiles * kp.n_out_slab;
+    long grid = (n_units + warps - 1) / warps;
+    const int ctas_per_sm = env_int("RFI_TMA_CTAS_PER_SM", 1);
+    if (grid > (long)p->sm_count * ctas_per_sm) grid = (long)p->sm_count * ctas_per_sm;
+    auto kern = rfi::rfi_tma_kernel<R, FP16>;
+    RFI_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    kern<<<(unsigned)grid, warps * 32, smem, st>>>(*map, kp, stages);
+    RFI_CUDA(cudaGetLastError());
+    p->launches++;
+    return RFI_OK;
+}
+
+template <bool FP16>
+int launch_tma(rfi_plan* p, const rfi::KParams& kp, int rows, cudaStream_t st) {
+    const int cap = env_int("RFI_TMA_ROWS", 8);
+    const int R = largest_divisor_le(kp.M, cap < 1 ? 1 : (cap > 8 ? 8 : cap));
+    const CUtensorMap* map = nullptr;
+    int rc = get_tensor_map(p, kp.vis, rows, R, &map);
+    if (rc != RFI_OK) return rc;
+    switch (R) {
+        case 1: return launch_tma_r<1, FP16>(p, kp, map, st);
+        case 2: return launch_tma_r<2, FP16>(p, kp, map, st);
+        case 3: return launch_tma_r<3, FP16>(p, kp, map, st);
+        case 4: return launch_tma_r<4, FP16>(p, kp, map, st);
+        case 5: return launch_tma_r<5, FP16>(p, kp, map, st);
+        case 6: return launch_tma_r<6, FP16>(p, kp, map, st);
+        case 7: return launch_tma_r<7, FP16>(p, kp, map, st);
+        default: return launch_tma_r<8, FP16>(p, kp, map, st);
+    }
+}
+
+template <int R, bool FP16>
+int launch_direct_r(rfi_plan* p, const rfi::KParams& kp, cudaStream_t st) {
+    const int n_tiles = (int)((p->n_cells() + 31) / 32);
+    const long n_units = (long)n_tiles * kp.n_out_slab;
+    const unsigned grid = (unsigned)((n_units + 3) / 4);
+    const bool v8 = (reinterpret_cast<uintptr_t>(kp.vis) % 32 == 0);
+    if (FP16 || v8) rfi::rfi_direct_kernel<R, FP16, true><<<grid, 128, 0, st>>>(kp);
+    else            rfi::rfi_direct_kernel<R, FP16, false><<<grid, 128, 0, st>>>(kp);
+    RFI_CUDA(cudaGetLastError());
+    p->launches++;
+    return RFI_OK;
+}
+
+template <bool FP16>
+int launch_direct(rfi_plan* p, const rfi::KParams& kp, cudaStream_t st) {
+    const int cap = env_int("RFI_DIRECT_ROWS", 4);
+    const int R = largest_divisor_le(kp.M, cap < 1 ? 1 : (cap > 4 ? 4 : cap));
+    switch (R) {
+        case 1: return launch_direct_r<1, FP16>(p, kp, st);
+        case 2: return launch_direct_r<2, FP16>(p, kp, st);
+        case 3: return launch_direct_r<3, FP16>(p, kp, st);
+        default: return launch_direct_r<4, FP16>(p, kp, st);
+    }
+}
+
+int ensure_flags(rfi_plan* p) {
+    const size_t need = p->flags_words();
+    if (need > p->flags_words_cap) {
+        if (p->d_flags) cudaFree(p->d_flags);
+        p->d_flags = nullptr;
+        p->flags_words_cap = 0;
+        if (cudaMalloc(&p->d_flags, need * sizeof(uint32_t)) != cudaSuccess) {
+            cudaGetLastError();
+            return RFI_ENOMEM;
+        }
+        p->flags_words_cap = need;
+    }
+    return RFI_OK;
+}
+
+int upload_thresholds(rfi_plan* p, cudaStream_t st) {
+    if (!p->thr_dirty) return RFI_OK;
+    if (p->K > p->d_thr_cap) {
+        if (p->d_thr) cudaFree(p->d_thr);
+        p->d_thr = nullptr;
+        p->d_thr_cap = 0;
+        if (cudaMalloc(&p->d_thr, sizeof(rfi::Thr) * p->K) != cudaSuccess) {
+            cudaGetLastError();
+            return RFI_ENOMEM;
+        }
+        p->d_thr_cap = p->K;
+    }
+    std::vector<rfi::Thr> h(p->K);
+    for (int k = 0; k < p->K; ++k) h[k] = to_device_thr(p->thr[k], p->M);
+    // pageable source: the copy is staged before the call returns, so `h` may die
+    RFI_CUDA(cudaMemcpyAsync(p->d_thr, h.data(), sizeof(rfi::Thr) * p->K, cudaMemcpyHostToDevice, st));
+    p->thr_dirty = false;
+    return RFI_OK;
+}
+
+// Enqueue the kernel(s) for one slab of `n_out_slab` whole integrations starting at output o_first.
+int enqueue_slab(rfi_plan* p, const void* d_vis_slab, int o_first, int n_out_slab, float* d_avg, uint32_t* d_weight,
+                 float* d_stats, cudaStream_t st) {
+    rfi::KParams kp;
+    memset(&kp, 0, sizeof(kp));
+    kp.vis = d_vis_slab;
+    kp.avg = d_avg;
+    kp.weight = d_weight;
+    kp.stats = d_stats;
+    kp.flags = p->d_flags;
+    kp.thr_table = p->d_thr;
+    kp.thr0 = to_device_thr(p->thr[0], p->M);
+    kp.n_cells = (int)p->n_cells();
+    kp.n_chan = p->n_chan;
+    kp.n_baselines = p->n_baselines;
+    kp.wpb = p->wpb();
+    kp.M = p->M;
+    kp.n_int = p->n_int;
+    kp.wpo = p->n_int / p->M;
+    kp.n_out_slab = n_out_slab;
+    kp.o_first = o_first;
+    kp.n_out_total = p->n_out();
+    kp.n_win_total = p->n_win();
+    kp.K = p->K;
+    kp.flags_atomic = (p->n_chan % 32 != 0 && 32 % p->n_chan != 0) ? 1 : 0;
+
+    if (p->K > 1) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "batched threshold mode (K > 1) is not built yet");
+        return RFI_EINVAL;
+    }
+    int variant = p->variant;
+    if (variant == RFI_VARIANT_AUTO) variant = tma_allowed(p) ? RFI_VARIANT_TMA : RFI_VARIANT_DIRECT;
+    if (variant == RFI_VARIANT_TMA && !tma_allowed(p)) return RFI_EINVAL;
+    p->last_variant = variant;
+    const bool fp16 = p->precision == RFI_FP16;
+    if (variant == RFI_VARIANT_TMA) {
+        const int rows = n_out_slab * p->n_int;
+        return fp16 ? launch_tma<true>(p, kp, rows, st) : launch_tma<false>(p, kp, rows, st);
+    }
+    return fp16 ? launch_direct<true>(p, kp, st) : launch_direct<false>(p, kp, st);
+}
+
+int prepare(rfi_plan* p, cudaStream_t st) {
+    if (!p) return RFI_EINVAL;
+    if (p->K < 1) return RFI_ESTATE;
+    int rc = ensure_device(p);
+    if (rc != RFI_OK) return rc;
+    rc = ensure_flags(p);
+    if (rc != RFI_OK) return rc;
+    rc = upload_thresholds(p, st);
+    if (rc != RFI_OK) return rc;
+    const bool flags_atomic = (p->n_chan % 32 != 0 && 32 % p->n_chan != 0);
+    if (flags_atomic) RFI_CUDA(cudaMemsetAsync(p->d_flags, 0, p->flags_words() * sizeof(uint32_t), st));
+    return RFI_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int rfi_plan_create(rfi_plan** out, int n_stations, int n_baselines, int n_chan, int n_time, int window_M,
+                    int precision) {
+    if (!out) return RFI_EINVAL;
+    *out = nullptr;
+    if (n_stations < 1 || n_chan < 1 || n_time < 1 || window_M < 2) return RFI_EINVAL;
+    const long N = n_stations;
+    if (n_baselines < 1 || ((long)n_baselines != N * (N + 1) / 2 && (long)n_baselines != N * (N - 1) / 2))
+        return RFI_EINVAL;
+    if (n_time % window_M != 0) return RFI_EINVAL;
+    if (precision != RFI_FP32 && precision != RFI_FP16) return RFI_EINVAL;
+    if ((long)n_baselines * n_chan > (1L << 30)) return RFI_EINVAL;
+    rfi_plan* p = new (std::nothrow) rfi_plan();
+    if (!p) return RFI_ENOMEM;
+    p->n_stations = n_stations;
+    p->n_baselines = n_baselines;
+    p->n_chan = n_chan;
+    p->n_time = n_time;
+    p->M = window_M;
+    p->precision = precision;
+    p->n_int = n_time;
+    *out = p;
+    return RFI_OK;
+}
+
+int rfi_plan_set_integration(rfi_plan* p, int n_int) {
+    if (!p || n_int < 1) return RFI_EINVAL;
+    if (p->n_time % n_int != 0 || n_int % p->M != 0) return RFI_EINVAL;
+    p->n_int = n_int;
+    p->have_result = false;
+    return RFI_OK;
+}
+
+int rfi_set_thresholds(rfi_plan* p, int K, const rfi_thresholds* h_sets) {
+    if (!p || K < 1 || !h_sets || K > 4096) return RFI_EINVAL;
+    for (int k = 0; k < K; ++k) {
+        const rfi_thresholds& t = h_sets[k];
+        if (!(t.d > 0.f) || std::isinf(t.d)) return RFI_EINVAL;
+        if (std::isnan(t.s_low) || std::isnan(t.s_high) || std::isnan(t.gamma)) return RFI_EINVAL;
+    }
+    p->thr.assign(h_sets, h_sets + K);
+    p->K = K;
+    p->thr_dirty = true;
+    p->have_result = false;
+    return RFI_OK;
+}
+
+int rfi_plan_set_variant(rfi_plan* p, int variant) {
+    if (!p || variant < RFI_VARIANT_AUTO || variant > RFI_VARIANT_TMA) return RFI_EINVAL;
+    p->variant = variant;
+    return RFI_OK;
+}
+
+int rfi_process_chunk(rfi_plan* p, const void* d_vis, void* d_avg, void* d_weight, void* d_stats, void* cuda_stream) {
+    if (!p) return RFI_EINVAL;
+    if (p->K < 1) return RFI_ESTATE;
+    if (!d_vis || !d_avg || !d_weight) return RFI_EINVAL;
+    if (reinterpret_cast<uintptr_t>(d_vis) % 16 || reinterpret_cast<uintptr_t>(d_avg) % 16 ||
+        reinterpret_cast<uintptr_t>(d_weight) % 4 || reinterpret_cast<uintptr_t>(d_stats) % 4)
+        return RFI_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    int rc = prepare(p, st);
+    if (rc != RFI_OK) return rc;
+    rc = enqueue_slab(p, d_vis, 0, p->n_out(), static_cast<float*>(d_avg), static_cast<uint32_t*>(d_weight),
+                      static_cast<float*>(d_stats), st);
+    if (rc == RFI_OK) p->have_result = true;
+    return rc;
+}
+
+int rfi_get_flags(rfi_plan* p, const uint32_t** d_flags, size_t* n_words) {
+    if (!p || !d_flags || !n_words) return RFI_EINVAL;
+    if (!p->have_result) return RFI_ESTATE;
+    *d_flags = p->d_flags;
+    *n_words = p->flags_words();
+    return RFI_OK;
+}
+
+int rfi_process_chunk_host(rfi_plan* p, const void* h_vis, void* h_avg, void* h_weight, void* h_flags,
+                           void* h_stats) {
+    if (!p) return RFI_EINVAL;
+    if (p->K < 1) return RFI_ESTATE;
+    if (!h_vis || !h_avg || !h_weight || !h_flags) return RFI_EINVAL;
+    int rc = ensure_device(p);
+    if (rc != RFI_OK) return rc;
+    const size_t slab_bytes = (size_t)p->n_int * p->n_cells() * p->sample_bytes();
+    for (int i = 0; i < 2; ++i) {
+        if (!p->streams[i]) RFI_CUDA(cudaStreamCreateWithFlags(&p->streams[i], cudaStreamNonBlocking));
+        if (!p->ev_copied[i]) RFI_CUDA(cudaEventCreateWithFlags(&p->ev_copied[i], cudaEventDisableTiming));
+        if (!p->ev_done[i]) RFI_CUDA(cudaEventCreateWithFlags(&p->ev_done[i], cudaEventDisableTiming));
+        if (!p->d_stage[i]) {
+            if (cudaMalloc(&p->d_stage[i], slab_bytes) != cudaSuccess) { cudaGetLastError(); return RFI_ENOMEM; }
+        }
+    }
+    auto grow = [](auto*& ptr, size_t& cap, size_t need) -> int {
+        if (need <= cap) return RFI_OK;
+        if (ptr) cudaFree(ptr);
+        ptr = nullptr; cap = 0;
+        void* q = nullptr;
+        if (cudaMalloc(&q, need) != cudaSuccess) { cudaGetLastError(); return RFI_ENOMEM; }
+        ptr = static_cast<std::remove_reference_t<decltype(ptr)>>(q);
+        cap = need;
+        return RFI_OK;
+    };
+    if ((rc = grow(p->d_avg, p->d_avg_cap, rfi_avg_bytes(p))) != RFI_OK) return rc;
+    if ((rc = grow(p->d_weight, p->d_weight_cap, rfi_weight_bytes(p))) != RFI_OK) return rc;
+    if (h_stats && (rc = grow(p->d_stats, p->d_stats_cap, rfi_stats_bytes(p))) != RFI_OK) return rc;
+
+    cudaStream_t copy_st = p->streams[0], comp_st = p->streams[1];
+    rc = prepare(p, comp_st);
+    if (rc != RFI_OK) return rc;
+    const int n_out = p->n_out();
+    const uint8_t* src = static_cast<const uint8_t*>(h_vis);
+    for (int o = 0; o < n_out; ++o) {
+        const int b = o & 1;
+        // the staging buffer is free once the kernel that read it (slab o-2) has finished
+        if (o >= 2) RFI_CUDA(cudaStreamWaitEvent(copy_st, p->ev_done[b], 0));
+        RFI_CUDA(cudaMemcpyAsync(p->d_stage[b], src + (size_t)o * slab_bytes, slab_bytes, cudaMemcpyHostToDevice, copy_st));
+        RFI_CUDA(cudaEventRecord(p->ev_copied[b], copy_st));
+        RFI_CUDA(cudaStreamWaitEvent(comp_st, p->ev_copied[b], 0));
+        rc = enqueue_slab(p, p->d_stage[b], o, 1, p->d_avg, p->d_weight, h_stats ? p->d_stats : nullptr, comp_st);
+        if (rc != RFI_OK) return rc;
+        RFI_CUDA(cudaEventRecord(p->ev_done[b], comp_st));
+    }
+    RFI_CUDA(cudaMemcpyAsync(h_avg, p->d_avg, rfi_avg_bytes(p), cudaMemcpyDeviceToHost, comp_st));
+    RFI_CUDA(cudaMemcpyAsync(h_weight, p->d_weight, rfi_weight_bytes(p), cudaMemcpyDeviceToHost, comp_st));
+    RFI_CUDA(cudaMemcpyAsync(h_flags, p->d_flags, rfi_flags_bytes(p), cudaMemcpyDeviceToHost, comp_st));
+    if (h_stats) RFI_CUDA(cudaMemcpyAsync(h_stats, p->d_stats, rfi_stats_bytes(p), cudaMemcpyDeviceToHost, comp_st));
+    RFI_CUDA(cudaStreamSynchronize(comp_st));
+    RFI_CUDA(cudaStreamSynchronize(copy_st));
+    p->have_result = true;
+    return RFI_OK;
+}
+
+int rfi_plan_destroy(rfi_plan* p) {
+    if (!p) return RFI_EINVAL;
+    if (p->dev_ready) {
+        if (p->d_flags) cudaFree(p->d_flags);
+        if (p->d_thr) cudaFree(p->d_thr);
+        if (p->d_avg) cudaFree(p->d_avg);
+        if (p->d_weight) cudaFree(p->d_weight);
+        if (p->d_stats) cudaFree(p->d_stats);
+        for (int i = 0; i < 2; ++i) {
+            if (p->d_stage[i]) cudaFree(p->d_stage[i]);
+            if (p->ev_copied[i]) cudaEventDestroy(p->ev_copied[i]);
+            if (p->ev_done[i]) cudaEventDestroy(p->ev_done[i]);
+            if (p->streams[i]) cudaStreamDestroy(p->streams[i]);
+        }
+        cudaGetLastError();
+    }
+    delete p;
+    return RFI_OK;
+}
+
+const char* rfi_strerror(int code) {
+    switch (code) {
+        case RFI_OK: return "ok";
+        case RFI_EINVAL: return "invalid argument";
+        case RFI_ECUDA: return "CUDA call failed (see rfi_last_cuda_error)";
+        case RFI_ENOMEM: return "out of memory";
+        case RFI_ESTATE: return "call order: thresholds not set or no chunk processed";
+        case RFI_ENODEV: return "no usable sm_100 CUDA device";
+        default: return "unknown error code";
+    }
+}
+
+const char* rfi_last_cuda_error(void) { return g_cuda_err; }
+
+size_t rfi_flags_bytes(const rfi_plan* p) { return p ? p->flags_words() * sizeof(uint32_t) : 0; }
+size_t rfi_avg_bytes(const rfi_plan* p) {
+    return p ? (size_t)(p->K > 0 ? p->K : 1) * p->n_out() * p->n_cells() * 8 * sizeof(float) : 0;
+}
+size_t rfi_weight_bytes(const rfi_plan* p) {
+    return p ? (size_t)(p->K > 0 ? p->K : 1) * p->n_out() * p->n_cells() * sizeof(uint32_t) : 0;
+}
+size_t rfi_stats_bytes(const rfi_plan* p) { return p ? (size_t)3 * p->n_win() * p->n_cells() * sizeof(float) : 0; }
+size_t rfi_vis_bytes(const rfi_plan* p) { return p ? (size_t)p->n_time * p->n_cells() * p->sample_bytes() : 0; }
+uint64_t rfi_plan_launch_count(const rfi_plan* p) { return p ? p->launches : 0; }
+int rfi_plan_last_variant(const rfi_plan* p) { return p ? p->last_variant : 0; }
+const char* rfi_version(void) { return "rfi-b200 0.1 (sm_100a)"; }
+
+}  // extern "C"

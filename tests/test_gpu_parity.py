@@ -1,0 +1,182 @@
+"""GPU parity: the CUDA path through the C ABI against the fp64 oracle, element by element, on the same
+seeded inputs.  Sizes span several 32-cell tiles, ragged tails, both kernel variants and both storage types."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import paper_2412_14775_b200 as rfi
+from paper_2412_14775_b200 import synth
+from tests.parity_util import compare, gpu_outputs_to_numpy
+
+pytestmark = pytest.mark.gpu
+INF = float("inf")
+
+
+def run_gpu(w, vis, thresholds, variant="auto", stats=True):
+    plan = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M,
+                       rfi.RFI_FP16 if w.fp16 else rfi.RFI_FP32, n_int=w.n_int)
+    plan.set_thresholds(thresholds)
+    plan.set_variant(variant)
+    avg, weight, st = plan.alloc_outputs(stats=stats)
+    avg.fill_(float("nan")); weight.fill_(-1)
+    if st is not None:
+        st.fill_(float("nan"))
+    plan.process_chunk(vis.cuda(), avg, weight, st)
+    torch.cuda.synchronize()
+    flags = rfi.unpack_flags(plan.get_flags(), w.n_chan)
+    out = gpu_outputs_to_numpy(plan, avg, weight, st, flags)
+    used = plan.last_variant
+    assert plan.launch_count >= 1
+    plan.destroy()
+    return out, used
+
+
+def check(w, thresholds, variant, seed=1234, tol=None, mutate=None):
+    vis, truth = synth.make_chunk(w, seed=seed, device="cpu")
+    if mutate is not None:
+        mutate(vis)
+    out, used = run_gpu(w, vis, thresholds, variant)
+    if variant != "auto":
+        assert used == variant
+    v = vis.numpy().reshape(w.n_time, w.n_cells, 4, 2)
+    rep = compare(v, w.window_M, w.n_int, thresholds, out, tol=tol or (2e-3 if w.fp16 else 1e-5), fp16=w.fp16)
+    return rep, out, truth
+
+
+@pytest.mark.parametrize("variant", ["direct", "tma"])
+def test_tiny_config(variant):
+    """BASELINE.json configs[0]: 4 stations, 6 baselines, 16 channels, 1024 samples, M=64, 16 outputs."""
+    w = synth.WORKLOADS["tiny"]
+    thr = synth.default_thresholds(w.window_M)
+    rep, out, truth = check(w, thr, variant)
+    assert rep["n_windows"] == 16 * 96
+    # the injected burst (10x noise power, fully polarised) must be caught where it fills most of a window
+    flagged = out["flags"][0]
+    assert flagged[truth.numpy()].mean() > 0.5
+    assert flagged[~truth.numpy()].mean() < 0.1
+
+
+@pytest.mark.parametrize("variant", ["direct", "tma"])
+def test_mini_lofar_several_tiles_autos_gain_bursts(variant):
+    w = synth.WORKLOADS["lofar"].scaled(n_stations=6, n_time=1024, n_int=256, burst_cell_frac=0.1)
+    assert w.n_cells == 21 * 64
+    rep, out, truth = check(w, synth.default_thresholds(16), variant)
+    assert 0.001 < rep["oracle_flag_fraction"] < 0.2
+
+
+@pytest.mark.parametrize("variant", ["direct", "tma"])
+@pytest.mark.parametrize("M,n_int,n_time", [(20, 100, 400), (10, 50, 200), (2, 8, 64), (3, 12, 48), (7, 28, 56),
+                                              (64, 128, 256), (128, 256, 256), (16, 16, 64)])
+def test_window_sizes_and_ragged_channels(variant, M, n_int, n_time):
+    """n_chan = 20: 200 cells = 6.25 tiles, flag words shared between warps (atomic path); the paper's W = 20."""
+    w = synth.Workload("ragged", 5, False, 20, n_time, M, n_int, burst_cell_frac=0.2, channel_gain=True)
+    assert w.n_cells == 200
+    thr = synth.default_thresholds(M) if M >= 8 else [[1.0, 0.02, 1.5, 0.9]]
+    check(w, thr, variant, seed=7 + M)
+
+
+def test_cells_not_multiple_of_four_falls_back_to_direct():
+    w = synth.Workload("odd", 3, False, 13, 128, 16, 64, burst_cell_frac=0.3)
+    assert w.n_cells == 39
+    vis, _ = synth.make_chunk(w, seed=3)
+    out, used = run_gpu(w, vis, synth.default_thresholds(16), "auto")
+    assert used == "direct"
+    compare(vis.numpy().reshape(w.n_time, w.n_cells, 4, 2), 16, 64, synth.default_thresholds(16), out)
+    plan = rfi.RfiPlan(3, 3, 13, 128, 16)
+    plan.set_thresholds(synth.default_thresholds(16)); plan.set_variant("tma")
+    avg, weight, _ = plan.alloc_outputs()
+    with pytest.raises(rfi.RfiError):
+        plan.process_chunk(vis.cuda(), avg, weight)
+    plan.destroy()
+
+
+@pytest.mark.parametrize("n_chan", [1, 8, 16, 32, 48, 96])
+def test_flag_word_layouts(n_chan):
+    w = synth.Workload("words", 4, True, n_chan, 128, 8, 32, burst_cell_frac=0.3)
+    for variant in ("direct", "tma"):
+        if variant == "tma" and w.n_cells % 4:
+            continue
+        check(w, [[1.0, 0.05, 1.0, 0.7]], variant, seed=n_chan)
+
+
+@pytest.mark.parametrize("variant", ["direct", "tma"])
+def test_fp16_storage(variant):
+    """configs[2] in miniature: fp16 storage, fp32 accumulation, CW tones on one channel.  Statistics against the
+    oracle on the SAME fp16-rounded values at 2e-3; flag agreement >= 99.9 %."""
+    w = synth.WORKLOADS["lofar_fp16"].scaled(n_stations=6, n_time=1024, n_int=256, burst_cell_frac=0.1, tone_chan_frac=0.02)
+    rep, out, truth = check(w, synth.default_thresholds(16), variant)
+    assert rep["flag_agreement"] >= 0.999
+    # and the fp32-accumulate path on fp16 data is in fact as tight as the fp32 one
+    vis, _ = synth.make_chunk(w, seed=1234)
+    compare(vis.numpy().reshape(w.n_time, w.n_cells, 4, 2), 16, 256, synth.default_thresholds(16), out, tol=1e-5)
+
+
+@pytest.mark.parametrize("variant", ["direct", "tma"])
+def test_degenerate_inputs(variant):
+    """All-zero cell, NaN / Inf samples, Hermitian (auto) cells, tiny and huge amplitudes, disabled detectors."""
+    w = synth.Workload("degenerate", 4, True, 16, 256, 16, 64, burst_cell_frac=0.2)
+
+    def mutate(vis):
+        v = vis.view(w.n_time, w.n_cells, 4, 2)
+        v[:, 5] = 0.0                      # all-zero cell: tau = -c, r = 0
+        v[40:48, 7] = 0.0                  # zero samples inside a window
+        v[17, 9, 2, 1] = float("nan")
+        v[100, 11, 0, 0] = float("inf")
+        v[:, 20] *= 1e-12                  # scale invariance at the edges of the documented range
+        v[:, 21] *= 1e12
+
+    thr = [[1.0, 0.1, 0.62, 0.52]]
+    rep, out, _ = check(w, thr, variant, mutate=mutate)
+    f = out["flags"][0]
+    assert f[17 // 16, 9] and f[100 // 16, 11]            # non-finite windows are flagged
+    assert np.isfinite(out["avg"]).all()
+    c = (16 * 1.0 + 1) / 15
+    assert np.allclose(out["tau"][:, 5], -c) and (out["r_re"][:, 5] == 0).all()
+    assert f[:, 5].all() and (out["weight"][0][:, 5] == 0).all() and (out["avg"][0][:, 5] == 0).all()
+    # detectors disabled: only the non-finite windows are flagged
+    rep2, out2, _ = check(w, [[1.0, -INF, INF, INF]], variant, mutate=mutate)
+    assert out2["flags"].sum() == 2
+
+
+@pytest.mark.parametrize("variant", ["direct", "tma"])
+def test_exact_ties_are_not_flagged(variant):
+    """r = |16 - 2*4|/16 = 0.5 exactly and tau = 0 exactly: thresholds equal to the statistic do not flag (Eq.(5),(10) strict)."""
+    M = 16
+    w = synth.Workload("ties", 2, True, 16, M, M, M)
+    vis = torch.zeros(M, 3, 16, 4, 2)
+    sign = torch.ones(M); sign[:4] = -1
+    vis[:, :, :, 0, 0] = 2.0 * sign[:, None, None]        # xx = +-2, everything else 0: Stokes direction (1,0,0), |I| = 2
+    for thr, expect in (([1.0, -INF, INF, 0.5], False), ([1.0, -INF, INF, float(np.nextafter(np.float32(0.5), np.float32(0)))], True),
+                        ([1.0, 0.0, INF, INF], False), ([1.0, 1e-30, INF, INF], True), ([1.0, -INF, 0.0, INF], False)):
+        out, _ = run_gpu(w, vis, [thr], variant)
+        assert out["tau"].max() == 0.0 and out["tau"].min() == 0.0
+        assert (out["r_re"] == 0.5).all() and (out["r_im"] == 0.0).all()
+        assert out["flags"].all() == expect and out["flags"].any() == expect
+
+
+def test_host_path_equals_device_path():
+    w = synth.WORKLOADS["lofar"].scaled(n_stations=5, n_time=1024, n_int=256, burst_cell_frac=0.1)
+    vis, _ = synth.make_chunk(w, seed=11)
+    thr = synth.default_thresholds(16)
+    out_dev, _ = run_gpu(w, vis, thr, "auto")
+    plan = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M, n_int=w.n_int)
+    plan.set_thresholds(thr)
+    for _ in range(2):                                   # twice: staging buffers and tensor maps are reused
+        avg, weight, flags, stats = plan.process_chunk_host(vis.pin_memory(), want_stats=True)
+    out_host = gpu_outputs_to_numpy(plan, avg, weight, stats, rfi.unpack_flags(flags, w.n_chan))
+    assert plan.launch_count == 2 * w.n_out
+    plan.destroy()
+    for key in ("avg", "weight", "flags", "tau", "r_re", "r_im"):
+        np.testing.assert_array_equal(out_dev[key], out_host[key])
+
+
+def test_variants_agree_bit_for_bit():
+    w = synth.WORKLOADS["lofar"].scaled(n_stations=7, n_time=512, n_int=256, burst_cell_frac=0.1)
+    vis, _ = synth.make_chunk(w, seed=13)
+    thr = synth.default_thresholds(16)
+    a, _ = run_gpu(w, vis, thr, "direct")
+    b, _ = run_gpu(w, vis, thr, "tma")
+    for key in ("avg", "weight", "flags", "tau", "r_re", "r_im"):
+        np.testing.assert_array_equal(a[key], b[key])
