@@ -105,11 +105,12 @@ def oracle_baseline(vis_np, w, thr, target_cpu_seconds=15.0):
     from oracle import rfi_oracle as orc
     cores = orc.max_threads()
     n_cells = vis_np.shape[1]
-    probe = min(n_cells, 64)
+    probe = min(n_cells, 1024)
+    orc.process(vis_np[:, :probe], w.window_M, w.n_int, thr, n_threads=cores, want_stats=False)   # warm-up: threads, pages
     t0 = time.perf_counter()
     orc.process(vis_np[:, :probe], w.window_M, w.n_int, thr, n_threads=cores, want_stats=False)
     dt = max(time.perf_counter() - t0, 1e-4)
-    per_cell_cpu = dt * min(cores, probe) / probe
+    per_cell_cpu = dt * cores / probe                       # CPU-seconds per cell
     use = int(max(probe, min(n_cells, target_cpu_seconds / per_cell_cpu)))
     t0 = time.perf_counter()
     orc.process(vis_np[:, :use], w.window_M, w.n_int, thr, n_threads=cores, want_stats=False)
@@ -273,7 +274,7 @@ def run_ours(args):
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         g = torch.Generator().manual_seed(7)
-        n_s = min(w.n_cells, 4096)
+        n_s = min(w.n_cells, 16384)
         idx = torch.randperm(w.n_cells, generator=g)[:n_s].sort().values.to(dev)
         sub = vis.reshape(w.n_time, w.n_cells, 4, 2)[:, idx].cpu().numpy()
         cpu = oracle_baseline(sub, w, thr)

@@ -43,25 +43,23 @@ def compare(vis_np, M, n_int, thresholds, gpu, tol=1e-5, fp16=False, oracle_thre
     n_out = res.weight.shape[1]
     wpo = n_int // M
     rep = {"n_windows": int(n_win * n_cells), "K": int(K)}
-    finite = np.isfinite(res.tau[0])
+    def check_stat(name, got, ref, floor):
+        """compare where the oracle's statistic is finite; where it is not, the GPU's must not be finite either"""
+        fin = np.isfinite(ref)
+        assert (~np.isfinite(got[~fin])).all(), f"{name}: oracle is non-finite where the GPU is finite"
+        d = np.abs(got.astype(np.float64) - ref)[fin]
+        bound = tol * np.maximum(np.abs(ref[fin]), floor)
+        rep[name + "_max_abs"] = float(d.max(initial=0))
+        rep[name + "_max_rel"] = float((d / np.maximum(np.abs(ref[fin]), 1e-300)).max(initial=0))
+        rep[name + "_worst_over_bound"] = float((d / bound).max(initial=0))
+        assert (d <= bound).all(), f"{name} mismatch: worst |d|/bound = {rep[name + '_worst_over_bound']:.3g}"
 
     if gpu.get("tau") is not None:
         d0 = thr32[0, 0]
         c0 = (M * d0 + 1) / (M - 1)
-        dt = np.abs(gpu["tau"].astype(np.float64) - res.tau[0])[finite]
-        bound = tol * np.maximum(np.abs(res.tau[0][finite]), 0.01 * c0)
-        rep["tau_max_abs"] = float(dt.max(initial=0))
-        rep["tau_max_rel"] = float((dt / np.maximum(np.abs(res.tau[0][finite]), 1e-300)).max(initial=0))
-        rep["tau_worst_over_bound"] = float((dt / bound).max(initial=0))
-        assert (dt <= bound).all(), f"tau mismatch: worst |d|/bound = {rep['tau_worst_over_bound']:.3g}"
-        for name, ref in (("r_re", res.r_re), ("r_im", res.r_im)):
-            dr = np.abs(gpu[name].astype(np.float64) - ref)[finite]
-            bound = tol * np.maximum(ref[finite], 1 / math.sqrt(M))
-            rep[name + "_max_abs"] = float(dr.max(initial=0))
-            rep[name + "_worst_over_bound"] = float((dr / bound).max(initial=0))
-            assert (dr <= bound).all(), f"{name} mismatch: worst |d|/bound = {rep[name + '_worst_over_bound']:.3g}"
-        # non-finite oracle statistics must be non-finite (or at least flagged) on the GPU as well
-        assert (~np.isfinite(gpu["tau"][~finite])).all() or (~finite).sum() == 0
+        check_stat("tau", gpu["tau"], res.tau[0], 0.01 * c0)
+        check_stat("r_re", gpu["r_re"], res.r_re, 1 / math.sqrt(M))
+        check_stat("r_im", gpu["r_im"], res.r_im, 1 / math.sqrt(M))
 
     n_mismatch, n_exempt, n_unexplained = 0, 0, 0
     avg_worst, avg_rel_worst = 0.0, 0.0
