@@ -65,9 +65,10 @@ enum {
 
 /* kernel variants (rfi_plan_set_variant); all compute the same function */
 enum {
-    RFI_VARIANT_AUTO   = 0,   /* TMA pipeline when the shape allows it, else direct */
-    RFI_VARIANT_DIRECT = 1,   /* per-thread 256-bit global loads, no shared-memory staging */
-    RFI_VARIANT_TMA    = 2    /* warp-private TMA (cp.async.bulk.tensor) ring in shared memory */
+    RFI_VARIANT_AUTO   = 0,   /* the fastest measured variant for the shape (currently: direct) */
+    RFI_VARIANT_DIRECT = 1,   /* per-thread 256-bit (fp32) / 128-bit (fp16) streaming loads, register double buffer */
+    RFI_VARIANT_TMA    = 2,   /* warp-private TMA (cp.async.bulk.tensor) ring in shared memory */
+    RFI_VARIANT_BATCHED = 3   /* reported by rfi_plan_last_variant when K > 1 (not selectable: K decides) */
 };
 
 /* One threshold set: d of Eq.(4), s_low/s_high of Eq.(5), gamma of Eq.(10)
@@ -87,8 +88,9 @@ int rfi_plan_create(rfi_plan **out, int n_stations, int n_baselines, int n_chan,
 int rfi_plan_set_integration(rfi_plan *plan, int n_int);
 
 /* Copy K >= 1 threshold sets from host memory (d > 0 and not NaN; s_low/s_high/gamma may be +-inf, not NaN).
- * K == 1 runs the single-set kernel; K > 1 the batched kernel that evaluates all sets in one pass over the
- * data (the paper tunes its thresholds with a host-side search). */
+ * K == 1 runs the single-set kernel; K > 1 the batched kernel that evaluates up to 64 sets in one pass over the
+ * data (one launch per 64 sets; the paper tunes its thresholds with a host-side search).
+ * The statistics planes (d_stats) always carry tau with the d of set 0. */
 int rfi_set_thresholds(rfi_plan *plan, int K, const rfi_thresholds *h_sets);
 
 /* Choose a kernel variant (default RFI_VARIANT_AUTO).  RFI_EINVAL if unknown. */

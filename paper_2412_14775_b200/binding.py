@@ -191,7 +191,7 @@ class RfiPlan:
     @property
     def last_variant(self) -> str:
         v = self._lib.rfi_plan_last_variant(self._h)
-        return {0: "none", 1: "direct", 2: "tma"}.get(v, str(v))
+        return {0: "none", 1: "direct", 2: "tma", 3: "batched"}.get(v, str(v))
 
     def destroy(self):
         if self._h:

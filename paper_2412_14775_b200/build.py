@@ -1,28 +1,33 @@
 """Build librfi.so (the C-ABI CUDA library) in-tree with nvcc for sm_100a.
 
-nvcc cross-compiles without a GPU.  The .so is git-ignored but travels to the GPU box with the
-repo snapshot.  Usage: `python -m paper_2412_14775_b200.build [--force]`.
+nvcc cross-compiles without a GPU.  The translation units are compiled in parallel and linked into one
+shared object.  The .so is git-ignored but travels to the GPU box with the repo snapshot.
+Usage: `python -m paper_2412_14775_b200.build [--force]`.
 """
 from __future__ import annotations
 
+import glob
 import os
 import shutil
 import subprocess
 import sys
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 ROOT = os.path.dirname(HERE)
 LIB = os.path.join(CSRC, "librfi.so")
-SOURCES = [os.path.join(CSRC, "rfi_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "rfi_kernels.cuh"), os.path.join(ROOT, "include", "rfi.h")]
+OBJ_DIR = os.path.join(CSRC, "build")
+SOURCES = [os.path.join(CSRC, f) for f in
+           ("rfi_api.cu", "rfi_launch_direct.cu", "rfi_launch_tma.cu", "rfi_launch_batched.cu")]
+DEPS = SOURCES + sorted(glob.glob(os.path.join(CSRC, "*.cuh"))) + [
+    os.path.join(CSRC, "rfi_internal.h"), os.path.join(ROOT, "include", "rfi.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-std=c++17", "-lineinfo",
-    "-Xcompiler", "-fPIC", "-shared",
+    "-Xcompiler", "-fPIC",
     "-Xptxas=-v",
-    "-cudart", "static",
 ]
 
 
@@ -43,18 +48,37 @@ def is_stale() -> bool:
 def build_library(force: bool = False, verbose: bool = False) -> str:
     if not force and not is_stale():
         return LIB
+    nvcc = nvcc_path()
+    os.makedirs(OBJ_DIR, exist_ok=True)
+
+    def compile_one(src):
+        obj = os.path.join(OBJ_DIR, os.path.basename(src)[:-3] + f".{os.getpid()}.o")
+        cmd = [nvcc, *NVCC_FLAGS, "-c", "-o", obj, src]
+        return obj, cmd, subprocess.run(cmd, capture_output=True, text=True)
+
+    with ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
+        results = list(ex.map(compile_one, SOURCES))
+    log = []
+    for obj, cmd, res in results:
+        log.append(" ".join(cmd) + "\n" + res.stderr)
+        if verbose or res.returncode != 0:
+            sys.stderr.write(res.stdout + res.stderr)
+        if res.returncode != 0:
+            raise RuntimeError(f"nvcc failed compiling {cmd[-1]}")
     tmp = LIB + f".tmp{os.getpid()}"
-    cmd = [nvcc_path(), *NVCC_FLAGS, "-o", tmp, *SOURCES]
-    res = subprocess.run(cmd, capture_output=True, text=True)
-    if verbose or res.returncode != 0:
-        sys.stderr.write(res.stdout + res.stderr)
+    link = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-cudart", "static", "-o", tmp,
+            *[obj for obj, _, _ in results]]
+    res = subprocess.run(link, capture_output=True, text=True)
     if res.returncode != 0:
-        raise RuntimeError("nvcc failed building librfi.so")
+        sys.stderr.write(res.stdout + res.stderr)
+        raise RuntimeError("nvcc failed linking librfi.so")
     os.replace(tmp, LIB)
+    for obj, _, _ in results:
+        os.remove(obj)
     with open(os.path.join(CSRC, "ptxas_info.txt"), "w") as f:
-        f.write(" ".join(cmd) + "\n" + res.stderr)
+        f.write("\n".join(log) + "\n" + " ".join(link) + "\n")
     return LIB
 
 
 if __name__ == "__main__":
-    print(build_library(force="--force" in sys.argv, verbose=True))
+    print(build_library(force="--force" in sys.argv, verbose="-v" in sys.argv))

@@ -1,35 +1,20 @@
 // rfi_api.cu -- host side of librfi.so: plan object, argument validation, kernel selection and the
 // C ABI declared in include/rfi.h.  No CPU implementation of the method lives here: without a CUDA
 // device every process call fails with RFI_ENODEV / RFI_ECUDA.
-#include "../../include/rfi.h"
+#include "rfi_internal.h"
 
 #include <cmath>
-#include <cstdio>
-#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
 
-#include "rfi_kernels.cuh"
+namespace rfi_host {
+thread_local char g_cuda_err[512] = "";
+}
+
+using namespace rfi_host;
 
 namespace {
-
-thread_local char g_cuda_err[512] = "";
-
-bool cuda_ok(cudaError_t e, const char* what) {
-    if (e == cudaSuccess) return true;
-    snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", what, cudaGetErrorString(e));
-    return false;
-}
-#define RFI_CUDA(call)                                  \
-    do {                                                \
-        if (!cuda_ok((call), #call)) return RFI_ECUDA;  \
-    } while (0)
-
-int env_int(const char* name, int dflt) {
-    const char* s = getenv(name);
-    return (s && *s) ? atoi(s) : dflt;
-}
 
 using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                    const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -72,9 +57,6 @@ struct rfi_plan {
     bool dev_ready = false;
     uint32_t* d_flags = nullptr;
     size_t flags_words_cap = 0;
-    rfi::Thr* d_thr = nullptr;
-    int d_thr_cap = 0;
-    bool thr_dirty = true;
     bool have_result = false;
     std::vector<MapEntry> maps;
     // host path
@@ -115,14 +97,6 @@ int ensure_device(rfi_plan* p) {
     }
     p->sm_count = prop.multiProcessorCount;
     p->smem_optin = (int)prop.sharedMemPerBlockOptin;
-    // 1/(n+1) table for the running-mean recurrence
-    static bool table_done[64] = {false};
-    if (p->device < 64 && !table_done[p->device]) {
-        std::vector<float> t(rfi::kInvNTable);
-        for (int i = 0; i < rfi::kInvNTable; ++i) t[i] = 1.0f / (float)(i + 1);
-        RFI_CUDA(cudaMemcpyToSymbol(rfi::c_inv_n, t.data(), sizeof(float) * rfi::kInvNTable));
-        table_done[p->device] = true;
-    }
     p->dev_ready = true;
     return RFI_OK;
 }
@@ -134,12 +108,6 @@ rfi::Thr to_device_thr(const rfi_thresholds& t, int M) {
     r.s_high = t.s_high;
     r.gamma = t.gamma;
     return r;
-}
-
-int largest_divisor_le(int M, int cap) {
-    for (int r = cap; r >= 1; --r)
-        if (M % r == 0) return r;
-    return 1;
 }
 
 int get_tensor_map(rfi_plan* p, const void* vis, int rows, int R, const CUtensorMap** out) {
@@ -188,79 +156,6 @@ bool tma_allowed(const rfi_plan* p) {
     return true;
 }
 
-template <int R, bool FP16>
-int launch_tma_r(rfi_plan* p, const rfi::KParams& kp, const CUtensorMap* map, cudaStream_t st) {
-    const int row_bytes = FP16 ? 512 : 1024;
-    const int stage_bytes = R * row_bytes;
-    int warps = env_int("RFI_TMA_WARPS", 8);
-    int stages = env_int("RFI_TMA_STAGES", 0);
-    if (warps < 1) warps = 1;
-    if (warps > 16) warps = 16;
-    const int budget = p->smem_optin - 1024 - 256;
-    if (stages <= 0) {
-        stages = budget / (warps * (stage_bytes + 8));
-        if (stages > 6) stages = 6;
-    }
-    while (stages > 1 && warps * stages * (stage_bytes + 8) > budget) --stages;
-    while (warps > 1 && warps * stages * (stage_bytes + 8) > budget) --warps;
-    const size_t smem = (size_t)warps * stages * (stage_bytes + 8) + 1024;
-    const int n_tiles = (int)((p->n_cells() + 31) / 32);
-    const long n_units = (long)n_tiles * kp.n_out_slab;
-    long grid = (n_units + warps - 1) / warps;
-    const int ctas_per_sm = env_int("RFI_TMA_CTAS_PER_SM", 1);
-    if (grid > (long)p->sm_count * ctas_per_sm) grid = (long)p->sm_count * ctas_per_sm;
-    auto kern = rfi::rfi_tma_kernel<R, FP16>;
-    RFI_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    kern<<<(unsigned)grid, warps * 32, smem, st>>>(*map, kp, stages);
-    RFI_CUDA(cudaGetLastError());
-    p->launches++;
-    return RFI_OK;
-}
-
-template <bool FP16>
-int launch_tma(rfi_plan* p, const rfi::KParams& kp, int rows, cudaStream_t st) {
-    const int cap = env_int("RFI_TMA_ROWS", 8);
-    const int R = largest_divisor_le(kp.M, cap < 1 ? 1 : (cap > 8 ? 8 : cap));
-    const CUtensorMap* map = nullptr;
-    int rc = get_tensor_map(p, kp.vis, rows, R, &map);
-    if (rc != RFI_OK) return rc;
-    switch (R) {
-        case 1: return launch_tma_r<1, FP16>(p, kp, map, st);
-        case 2: return launch_tma_r<2, FP16>(p, kp, map, st);
-        case 3: return launch_tma_r<3, FP16>(p, kp, map, st);
-        case 4: return launch_tma_r<4, FP16>(p, kp, map, st);
-        case 5: return launch_tma_r<5, FP16>(p, kp, map, st);
-        case 6: return launch_tma_r<6, FP16>(p, kp, map, st);
-        case 7: return launch_tma_r<7, FP16>(p, kp, map, st);
-        default: return launch_tma_r<8, FP16>(p, kp, map, st);
-    }
-}
-
-template <int R, bool FP16>
-int launch_direct_r(rfi_plan* p, const rfi::KParams& kp, cudaStream_t st) {
-    const int n_tiles = (int)((p->n_cells() + 31) / 32);
-    const long n_units = (long)n_tiles * kp.n_out_slab;
-    const unsigned grid = (unsigned)((n_units + 3) / 4);
-    const bool v8 = (reinterpret_cast<uintptr_t>(kp.vis) % 32 == 0);
-    if (FP16 || v8) rfi::rfi_direct_kernel<R, FP16, true><<<grid, 128, 0, st>>>(kp);
-    else            rfi::rfi_direct_kernel<R, FP16, false><<<grid, 128, 0, st>>>(kp);
-    RFI_CUDA(cudaGetLastError());
-    p->launches++;
-    return RFI_OK;
-}
-
-template <bool FP16>
-int launch_direct(rfi_plan* p, const rfi::KParams& kp, cudaStream_t st) {
-    const int cap = env_int("RFI_DIRECT_ROWS", 4);
-    const int R = largest_divisor_le(kp.M, cap < 1 ? 1 : (cap > 4 ? 4 : cap));
-    switch (R) {
-        case 1: return launch_direct_r<1, FP16>(p, kp, st);
-        case 2: return launch_direct_r<2, FP16>(p, kp, st);
-        case 3: return launch_direct_r<3, FP16>(p, kp, st);
-        default: return launch_direct_r<4, FP16>(p, kp, st);
-    }
-}
-
 int ensure_flags(rfi_plan* p) {
     const size_t need = p->flags_words();
     if (need > p->flags_words_cap) {
@@ -276,26 +171,6 @@ int ensure_flags(rfi_plan* p) {
     return RFI_OK;
 }
 
-int upload_thresholds(rfi_plan* p, cudaStream_t st) {
-    if (!p->thr_dirty) return RFI_OK;
-    if (p->K > p->d_thr_cap) {
-        if (p->d_thr) cudaFree(p->d_thr);
-        p->d_thr = nullptr;
-        p->d_thr_cap = 0;
-        if (cudaMalloc(&p->d_thr, sizeof(rfi::Thr) * p->K) != cudaSuccess) {
-            cudaGetLastError();
-            return RFI_ENOMEM;
-        }
-        p->d_thr_cap = p->K;
-    }
-    std::vector<rfi::Thr> h(p->K);
-    for (int k = 0; k < p->K; ++k) h[k] = to_device_thr(p->thr[k], p->M);
-    // pageable source: the copy is staged before the call returns, so `h` may die
-    RFI_CUDA(cudaMemcpyAsync(p->d_thr, h.data(), sizeof(rfi::Thr) * p->K, cudaMemcpyHostToDevice, st));
-    p->thr_dirty = false;
-    return RFI_OK;
-}
-
 // Enqueue the kernel(s) for one slab of `n_out_slab` whole integrations starting at output o_first.
 int enqueue_slab(rfi_plan* p, const void* d_vis_slab, int o_first, int n_out_slab, float* d_avg, uint32_t* d_weight,
                  float* d_stats, cudaStream_t st) {
@@ -306,7 +181,6 @@ int enqueue_slab(rfi_plan* p, const void* d_vis_slab, int o_first, int n_out_sla
     kp.weight = d_weight;
     kp.stats = d_stats;
     kp.flags = p->d_flags;
-    kp.thr_table = p->d_thr;
     kp.thr0 = to_device_thr(p->thr[0], p->M);
     kp.n_cells = (int)p->n_cells();
     kp.n_chan = p->n_chan;
@@ -320,22 +194,43 @@ int enqueue_slab(rfi_plan* p, const void* d_vis_slab, int o_first, int n_out_sla
     kp.n_out_total = p->n_out();
     kp.n_win_total = p->n_win();
     kp.K = p->K;
+    kp.k_first = 0;
     kp.flags_atomic = (p->n_chan % 32 != 0 && 32 % p->n_chan != 0) ? 1 : 0;
 
+    const bool fp16 = p->precision == RFI_FP16;
     if (p->K > 1) {
-        snprintf(g_cuda_err, sizeof(g_cuda_err), "batched threshold mode (K > 1) is not built yet");
-        return RFI_EINVAL;
+        // batched-threshold mode: all sets in one pass over the data, 64 sets per launch
+        p->last_variant = RFI_VARIANT_BATCHED;
+        for (int k0 = 0; k0 < p->K; k0 += rfi::kMaxBatch) {
+            rfi::BatchThr bt;
+            memset(&bt, 0, sizeof(bt));
+            kp.k_first = k0;
+            kp.K = p->K - k0 < rfi::kMaxBatch ? p->K - k0 : rfi::kMaxBatch;
+            for (int k = 0; k < kp.K; ++k) bt.t[k] = to_device_thr(p->thr[k0 + k], p->M);
+            const int rc = launch_batched(fp16, kp, bt, st);
+            if (rc != RFI_OK) return rc;
+            p->launches++;
+        }
+        return RFI_OK;
     }
     int variant = p->variant;
-    if (variant == RFI_VARIANT_AUTO) variant = tma_allowed(p) ? RFI_VARIANT_TMA : RFI_VARIANT_DIRECT;
+    // measured on B200 (profiles/): the register-staged direct kernel is the faster one for both storage types
+    if (variant == RFI_VARIANT_AUTO) variant = RFI_VARIANT_DIRECT;
     if (variant == RFI_VARIANT_TMA && !tma_allowed(p)) return RFI_EINVAL;
     p->last_variant = variant;
-    const bool fp16 = p->precision == RFI_FP16;
+    int rc;
     if (variant == RFI_VARIANT_TMA) {
         const int rows = n_out_slab * p->n_int;
-        return fp16 ? launch_tma<true>(p, kp, rows, st) : launch_tma<false>(p, kp, rows, st);
+        const int R = tma_rows(p->M);
+        const CUtensorMap* map = nullptr;
+        rc = get_tensor_map(p, kp.vis, rows, R, &map);
+        if (rc != RFI_OK) return rc;
+        rc = launch_tma(fp16, kp, map, R, p->sm_count, p->smem_optin, st);
+    } else {
+        rc = launch_direct(fp16, kp, st);
     }
-    return fp16 ? launch_direct<true>(p, kp, st) : launch_direct<false>(p, kp, st);
+    if (rc == RFI_OK) p->launches++;
+    return rc;
 }
 
 int prepare(rfi_plan* p, cudaStream_t st) {
@@ -344,8 +239,6 @@ int prepare(rfi_plan* p, cudaStream_t st) {
     int rc = ensure_device(p);
     if (rc != RFI_OK) return rc;
     rc = ensure_flags(p);
-    if (rc != RFI_OK) return rc;
-    rc = upload_thresholds(p, st);
     if (rc != RFI_OK) return rc;
     const bool flags_atomic = (p->n_chan % 32 != 0 && 32 % p->n_chan != 0);
     if (flags_atomic) RFI_CUDA(cudaMemsetAsync(p->d_flags, 0, p->flags_words() * sizeof(uint32_t), st));
@@ -397,13 +290,12 @@ int rfi_set_thresholds(rfi_plan* p, int K, const rfi_thresholds* h_sets) {
     }
     p->thr.assign(h_sets, h_sets + K);
     p->K = K;
-    p->thr_dirty = true;
     p->have_result = false;
     return RFI_OK;
 }
 
 int rfi_plan_set_variant(rfi_plan* p, int variant) {
-    if (!p || variant < RFI_VARIANT_AUTO || variant > RFI_VARIANT_TMA) return RFI_EINVAL;
+    if (!p || variant < RFI_VARIANT_AUTO || variant > RFI_VARIANT_TMA) return RFI_EINVAL;   // BATCHED is not selectable
     p->variant = variant;
     return RFI_OK;
 }
@@ -492,7 +384,6 @@ int rfi_plan_destroy(rfi_plan* p) {
     if (!p) return RFI_EINVAL;
     if (p->dev_ready) {
         if (p->d_flags) cudaFree(p->d_flags);
-        if (p->d_thr) cudaFree(p->d_thr);
         if (p->d_avg) cudaFree(p->d_avg);
         if (p->d_weight) cudaFree(p->d_weight);
         if (p->d_stats) cudaFree(p->d_stats);

@@ -1,0 +1,159 @@
+// rfi_common.cuh -- sm_100a device helpers shared by the kernels of the fused flag-and-average pass:
+// PTX wrappers (packed f32x2 arithmetic, streaming loads, mbarrier/TMA), the per-sample moment
+// accumulation, the window tail and the output stores.
+//
+// What is computed is defined in include/rfi.h (equations of PAPER.md cited there).  This file is
+// the product path: it shares nothing with oracle/.
+//
+// Mapping used by every kernel: one thread = one (baseline, channel) cell, a warp = 32 consecutive
+// cells.  With the time-slowest layout a warp's row of one time step is 1 KiB (fp32) / 512 B (fp16)
+// contiguous, so every global access is a whole-line, fully used request.  Statistics never cross
+// lanes; the only warp collective is the ballot that packs the flag bits.
+//
+// Arithmetic is fp32.  Pairs (re, im) are kept in 64-bit registers and processed with the
+// Blackwell packed instructions FADD2 / FMUL2 / FFMA2 (PTX add/mul/fma.rn.f32x2), which halves the
+// issue slots of the Stokes formation (Eq.(2)), the unit-vector sums (Eq.(8)) and the window sums.
+//
+// SK in centred form: Eq.(4)'s  W*S2/S1^2 - 1  equals  sum (z_i - zbar)^2 / (W zbar^2), z_i = |I_i|.
+// The centred second moment is built block-wise (R samples at a time: block mean, block centred
+// moment, then the pairwise merge of Chan et al.), which has none of the cancellation of the raw-moment
+// form in fp32 and no per-sample dependent chain.
+#pragma once
+
+#include <cuda.h>
+#include <cuda_fp16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace rfi {
+
+typedef unsigned long long f2;                    // two packed floats {lo = re, hi = im}
+
+struct Thr {                                      // one threshold set, device form
+    float c;                                      // (W d + 1)/(W - 1), Eq.(4) prefactor
+    float s_low, s_high, gamma;
+};
+
+constexpr int kMaxBatch = 64;                     // threshold sets evaluated by one batched launch
+
+struct KParams {
+    const void* vis;          // slab base: [rows][n_cells] samples
+    float* avg;               // [K][n_out_total][n_cells][8]
+    uint32_t* weight;         // [K][n_out_total][n_cells]
+    float* stats;             // [3][n_win_total][n_cells] or nullptr
+    uint32_t* flags;          // [K][n_win_total][n_baselines*wpb]
+    Thr thr0;                 // set 0 (single-set kernels; stats use its c)
+    int n_cells, n_chan, n_baselines, wpb;
+    int M, n_int, wpo;        // window, samples per output, windows per output
+    int n_out_slab;           // outputs contained in this slab
+    int o_first;              // global index of the slab's first output
+    int n_out_total, n_win_total;
+    int K;                    // sets handled by this launch (batched kernel: <= kMaxBatch)
+    int k_first;              // global index of this launch's first set
+    int flags_atomic;         // 1: flag words may be shared between warps -> atomicOr into a zeroed buffer
+};
+
+struct BatchThr { Thr t[kMaxBatch]; };            // by-value kernel parameter (constant bank), 1 KiB
+
+// ------------------------------------------------------------------------------------------------
+// PTX wrappers
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ f2 pack2(float lo, float hi) {
+    f2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void unpack2(f2 v, float& lo, float& hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ f2 add2(f2 a, f2 b) { f2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ f2 sub2(f2 a, f2 b) { f2 d; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ f2 mul2(f2 a, f2 b) { f2 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) {
+    f2 d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ float sqrt_approx(float x) { float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float rsqrt_approx(float x) { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float rcp_approx(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+
+// One 4-pol sample in registers as it sits in memory: fp32 -> 4 x (re,im) pairs, fp16 -> 4 x half2.
+template <bool FP16> struct Raw;
+template <> struct Raw<false> { f2 p[4]; };
+template <> struct Raw<true> { uint32_t p[4]; };
+
+// Streaming global loads: read-once data, not allocated in L1 (and evict-first in L2 where PTX allows the
+// qualifier, i.e. on the 256-bit form).
+__device__ __forceinline__ void ldg_stream(const void* ptr, Raw<false>& r) {      // one 256-bit request
+    asm volatile("ld.global.nc.L1::no_allocate.L2::evict_first.v4.b64 {%0,%1,%2,%3}, [%4];"
+                 : "=l"(r.p[0]), "=l"(r.p[1]), "=l"(r.p[2]), "=l"(r.p[3]) : "l"(ptr));
+}
+__device__ __forceinline__ void ldg_stream_16B(const void* ptr, Raw<false>& r) {  // 16-byte-aligned base only
+    asm volatile("ld.global.nc.L1::no_allocate.v2.b64 {%0,%1}, [%2];"
+                 : "=l"(r.p[0]), "=l"(r.p[1]) : "l"(ptr));
+    asm volatile("ld.global.nc.L1::no_allocate.v2.b64 {%0,%1}, [%2+16];"
+                 : "=l"(r.p[2]), "=l"(r.p[3]) : "l"(ptr));
+}
+__device__ __forceinline__ void ldg_stream(const void* ptr, Raw<true>& r) {       // one 128-bit request
+    asm volatile("ld.global.nc.L1::no_allocate.v4.b32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r.p[0]), "=r"(r.p[1]), "=r"(r.p[2]), "=r"(r.p[3]) : "l"(ptr));
+}
+__device__ __forceinline__ void lds_raw(uint32_t a0, uint32_t a1, Raw<false>& r) {
+    asm volatile("ld.shared.v2.b64 {%0,%1}, [%2];" : "=l"(r.p[0]), "=l"(r.p[1]) : "r"(a0));
+    asm volatile("ld.shared.v2.b64 {%0,%1}, [%2];" : "=l"(r.p[2]), "=l"(r.p[3]) : "r"(a1));
+}
+__device__ __forceinline__ void lds_raw(uint32_t a0, uint32_t, Raw<true>& r) {
+    asm volatile("ld.shared.v4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(r.p[0]), "=r"(r.p[1]), "=r"(r.p[2]), "=r"(r.p[3]) : "r"(a0));
+}
+
+// Widen one sample to four fp32 (re,im) pairs: xx, xy, yx, yy (row-major Eq.(1)).
+__device__ __forceinline__ void widen(const Raw<false>& r, f2 (&x)[4]) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) x[i] = r.p[i];
+}
+__device__ __forceinline__ void widen(const Raw<true>& r, f2 (&x)[4]) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&r.p[i]));   // exact
+        x[i] = pack2(f.x, f.y);
+    }
+}
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+    } while (!done);
+}
+__device__ __forceinline__ uint64_t l2_evict_first_policy() {
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, int c0, int c1, int c2,
+                                            uint32_t bar, uint64_t pol) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint"
+        " [%0], [%1, {%2, %3, %4}], [%5], %6;" ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(bar), "l"(pol)
+        : "memory");
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int c0, int c1,
+                                            uint32_t bar, uint64_t pol) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint"
+        " [%0], [%1, {%2, %3}], [%4], %5;" ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar), "l"(pol)
+        : "memory");
+}
+
+}  // namespace rfi

@@ -77,7 +77,7 @@ def test_window_sizes_and_ragged_channels(variant, M, n_int, n_time):
     check(w, thr, variant, seed=7 + M)
 
 
-def test_cells_not_multiple_of_four_falls_back_to_direct():
+def test_cells_not_multiple_of_four_cannot_use_tma():
     w = synth.Workload("odd", 3, False, 13, 128, 16, 64, burst_cell_frac=0.3)
     assert w.n_cells == 39
     vis, _ = synth.make_chunk(w, seed=3)
@@ -172,7 +172,10 @@ def test_host_path_equals_device_path():
         np.testing.assert_array_equal(out_dev[key], out_host[key])
 
 
-def test_variants_agree_bit_for_bit():
+def test_variants_agree_bit_for_bit(monkeypatch):
+    """Same block length R (rows merged at a time) -> the two load paths feed identical arithmetic."""
+    monkeypatch.setenv("RFI_DIRECT_ROWS", "4")
+    monkeypatch.setenv("RFI_TMA_ROWS", "4")
     w = synth.WORKLOADS["lofar"].scaled(n_stations=7, n_time=512, n_int=256, burst_cell_frac=0.1)
     vis, _ = synth.make_chunk(w, seed=13)
     thr = synth.default_thresholds(16)
@@ -180,3 +183,48 @@ def test_variants_agree_bit_for_bit():
     b, _ = run_gpu(w, vis, thr, "tma")
     for key in ("avg", "weight", "flags", "tau", "r_re", "r_im"):
         np.testing.assert_array_equal(a[key], b[key])
+
+
+# ------------------------------------------------------------------------------------------------------
+# batched-threshold mode (K > 1): BASELINE.json configs[4] in miniature
+# ------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("K", [2, 16, 17, 64, 70])
+def test_batched_sets_match_oracle_and_single_set_runs(K):
+    """K sets in one pass: parity with the oracle per set, and bit-for-bit equal to K single-set runs."""
+    w = synth.WORKLOADS["sweep"].scaled(n_stations=5, n_time=1536, n_int=768, burst_cell_frac=0.1)
+    thr = synth.sweep_thresholds(w.window_M, K, seed=K)
+    rep, out, truth = check(w, thr, "auto")
+    assert rep["K"] == K
+    fracs = out["flags"].reshape(K, -1).mean(1)
+    assert fracs.min() < fracs.max()                      # the sets really differ
+    vis, _ = synth.make_chunk(w, seed=1234)
+    for k in sorted({0, 1, K // 2, K - 1}):
+        single, used = run_gpu(w, vis, [thr[k]], "direct", stats=False)
+        assert used == "direct"
+        np.testing.assert_array_equal(single["flags"][0], out["flags"][k])
+        np.testing.assert_array_equal(single["weight"][0], out["weight"][k])
+        np.testing.assert_array_equal(single["avg"][0], out["avg"][k])
+
+
+@pytest.mark.parametrize("M,n_int,n_time,n_chan", [(20, 100, 400, 20), (3, 12, 48, 13), (64, 1024, 2048, 16), (8, 8, 64, 96)])
+def test_batched_ragged_shapes(M, n_int, n_time, n_chan):
+    """windows per output not a multiple of the 16 warps, ragged tiles, shared flag words, one window per output"""
+    w = synth.Workload("ragged_k", 5, False, n_chan, n_time, M, n_int, burst_cell_frac=0.2, channel_gain=True)
+    K = 5
+    thr = synth.sweep_thresholds(M, K, seed=M) if M >= 8 else [[1.0, 0.02 * (k + 1), 1.5, 0.9 - 0.02 * k] for k in range(K)]
+    check(w, thr, "auto", seed=M)
+
+
+def test_batched_fp16_and_host_path():
+    w = synth.WORKLOADS["lofar_fp16"].scaled(n_stations=5, n_time=1024, n_int=256, burst_cell_frac=0.1, tone_chan_frac=0.02)
+    thr = synth.sweep_thresholds(16, 8, seed=3)
+    rep, out, _ = check(w, thr, "auto")
+    vis, _ = synth.make_chunk(w, seed=1234)
+    plan = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M, rfi.RFI_FP16, n_int=w.n_int)
+    plan.set_thresholds(thr)
+    avg, weight, flags, stats = plan.process_chunk_host(vis.pin_memory(), want_stats=True)
+    assert plan.last_variant == "batched"
+    host = gpu_outputs_to_numpy(plan, avg, weight, stats, rfi.unpack_flags(flags, w.n_chan))
+    plan.destroy()
+    for key in ("avg", "weight", "flags", "tau", "r_re", "r_im"):
+        np.testing.assert_array_equal(out[key], host[key])
