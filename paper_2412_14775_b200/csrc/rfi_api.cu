@@ -104,8 +104,9 @@ int ensure_device(rfi_plan* p) {
 rfi::Thr to_device_thr(const rfi_thresholds& t, int M) {
     rfi::Thr r;
     r.c = (float)(((double)M * (double)t.d + 1.0) / ((double)M - 1.0));
-    r.s_low = t.s_low;
-    r.s_high = t.s_high;
+    // Eq.(5) on x = tau / c (c > 0): +-inf stay +-inf, 0 stays 0
+    r.x_low = (float)((double)t.s_low / (double)r.c);
+    r.x_high = (float)((double)t.s_high / (double)r.c);
     r.gamma = t.gamma;
     return r;
 }
@@ -201,13 +202,22 @@ int enqueue_slab(rfi_plan* p, const void* d_vis_slab, int o_first, int n_out_sla
     if (p->K > 1) {
         // batched-threshold mode: all sets in one pass over the data, 64 sets per launch
         p->last_variant = RFI_VARIANT_BATCHED;
+        // same block length as the single-set direct kernel, so K sets equal K single-set runs bit for bit
+        const int R = pick_rows(p->M, fp16);
+        const CUtensorMap* map = nullptr;
+        const bool use_tma = batched_tma_supported(fp16, kp, R) && tma_allowed(p);
+        if (use_tma) {
+            const int rc = get_tensor_map(p, kp.vis, n_out_slab * p->n_int, R, &map);
+            if (rc != RFI_OK) return rc;
+        }
         for (int k0 = 0; k0 < p->K; k0 += rfi::kMaxBatch) {
             rfi::BatchThr bt;
             memset(&bt, 0, sizeof(bt));
             kp.k_first = k0;
             kp.K = p->K - k0 < rfi::kMaxBatch ? p->K - k0 : rfi::kMaxBatch;
             for (int k = 0; k < kp.K; ++k) bt.t[k] = to_device_thr(p->thr[k0 + k], p->M);
-            const int rc = launch_batched(fp16, kp, bt, st);
+            const int rc = use_tma ? launch_batched_tma(fp16, kp, bt, map, R, p->sm_count, p->smem_optin, st)
+                                   : launch_batched(fp16, kp, bt, st);
             if (rc != RFI_OK) return rc;
             p->launches++;
         }

@@ -119,7 +119,7 @@ rfi_batched_kernel(const KParams p, const __grid_constant__ BatchThr bt) {
             for (int i = 0; i < SPW; ++i) {
                 const int k = warp * SPW + i;
                 if (k < p.K) {                                         // warp-uniform
-                    const bool flag = decide(x, r_re, r_im, bt.t[k]);
+                    const bool flag = decide(x, max_nan(r_re, r_im), bt.t[k]);
                     store_flags(p, g, p.k_first + k, w_global, flag);
                     if (!flag) {
 #pragma unroll

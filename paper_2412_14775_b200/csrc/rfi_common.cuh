@@ -30,8 +30,9 @@ namespace rfi {
 typedef unsigned long long f2;                    // two packed floats {lo = re, hi = im}
 
 struct Thr {                                      // one threshold set, device form
-    float c;                                      // (W d + 1)/(W - 1), Eq.(4) prefactor
-    float s_low, s_high, gamma;
+    float c;                                      // (W d + 1)/(W - 1), Eq.(4) prefactor: tau = c * x
+    float x_low, x_high;                          // s_low / c, s_high / c: Eq.(5) decided on x = W S2/S1^2 - 1
+    float gamma;                                  // Eq.(10)
 };
 
 constexpr int kMaxBatch = 64;                     // threshold sets evaluated by one batched launch
@@ -76,6 +77,8 @@ __device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) {
 }
 __device__ __forceinline__ float sqrt_approx(float x) { float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 __device__ __forceinline__ float rsqrt_approx(float x) { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+// max that returns NaN if either operand is NaN (so that a NaN statistic still flags, reading G6)
+__device__ __forceinline__ float max_nan(float a, float b) { float r; asm("max.NaN.f32 %0, %1, %2;" : "=f"(r) : "f"(a), "f"(b)); return r; }
 __device__ __forceinline__ float rcp_approx(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 
 // One 4-pol sample in registers as it sits in memory: fp32 -> 4 x (re,im) pairs, fp16 -> 4 x half2.

@@ -100,10 +100,11 @@ __device__ __forceinline__ void window_stats(const Win& w, float inv_M, float& x
     r_im = sqrt_refined(fmaf(qi, qi, fmaf(ui, ui, vi * vi))) * inv_M;
 }
 
-// Eq.(5), Eq.(10), OR-combined; negated so that NaN flags.
-__device__ __forceinline__ bool decide(float x, float r_re, float r_im, const Thr& t) {
-    const float tau = t.c * x;
-    return !(tau >= t.s_low && tau <= t.s_high) || !(r_re <= t.gamma) || !(r_im <= t.gamma);
+// Eq.(5), Eq.(10), OR-combined; negated so that NaN flags.  tau = c x with c > 0, so
+// tau < s_low <=> x < s_low / c: the thresholds arrive divided by c (one division on the host per set), and
+// r_re > gamma OR r_im > gamma <=> max(r_re, r_im) > gamma (NaN-propagating max).  Every kernel decides here.
+__device__ __forceinline__ bool decide(float x, float r_max, const Thr& t) {
+    return !(x >= t.x_low && x <= t.x_high && r_max <= t.gamma);
 }
 
 // Per-unit lane geometry: which cell, which flag word / bit.
@@ -178,7 +179,7 @@ __device__ __forceinline__ void finish_window(const KParams& p, const LaneGeom& 
                                               int w_global, f2 (&acc)[4], uint32_t& wt) {
     float x, r_re, r_im;
     window_stats(w, inv_M, x, r_re, r_im);
-    const bool flag = decide(x, r_re, r_im, p.thr0);
+    const bool flag = decide(x, max_nan(r_re, r_im), p.thr0);
     store_flags(p, g, p.k_first, w_global, flag);
     store_stats(p, g, w_global, p.thr0.c * x, r_re, r_im);
     if (!flag) {
