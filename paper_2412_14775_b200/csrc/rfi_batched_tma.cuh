@@ -30,24 +30,35 @@ constexpr int kRecBytes = 48;
 
 // One record against one threshold set (Eq.(5), Eq.(10), then the exclusion of PAPER.md:75).
 // keep = (x >= x_low) && (x <= x_high) && (r_max <= gamma): ordered compares, so a NaN statistic is not kept.
-// Returns the warp's flag word (bit l = lane l flagged).  Same decision as decide() in rfi_window.cuh.
+// Same decision as decide() in rfi_window.cuh.  The masked add is acc = fma(sum, keep ? 1 : 0, acc): exactly
+// acc + sum when kept, exactly acc when not (one packed instruction per pair; a predicated packed add costs
+// three).  This needs finite sums: the stream side stores zeros for a window whose sums are not finite -- such
+// a window has NaN statistics and is flagged by every set anyway.
+// Returns the warp's flag word (bit l = lane l flagged); cnt counts kept windows (exact in fp32 below 2^24).
 __device__ __forceinline__ uint32_t contract_one(float x, float r_max, float x_low, float x_high, float gamma,
-                                                 f2 (&a)[4], uint32_t& cnt, const f2 (&s)[4]) {
+                                                 f2 (&a)[4], float& cnt, const f2 (&s)[4]) {
     uint32_t word;
+    float kf;
     asm volatile(
         "{\n\t.reg .pred k;\n\t"
-        "setp.ge.f32 k, %6, %8;\n\t"
-        "setp.le.and.f32 k, %6, %9, k;\n\t"
-        "setp.le.and.f32 k, %7, %10, k;\n\t"
+        "setp.ge.f32 k, %2, %4;\n\t"
+        "setp.le.and.f32 k, %2, %5, k;\n\t"
+        "setp.le.and.f32 k, %3, %6, k;\n\t"
         "vote.sync.ballot.b32 %0, !k, 0xffffffff;\n\t"
-        "@k add.rn.f32x2 %1, %1, %11;\n\t"
-        "@k add.rn.f32x2 %2, %2, %12;\n\t"
-        "@k add.rn.f32x2 %3, %3, %13;\n\t"
-        "@k add.rn.f32x2 %4, %4, %14;\n\t"
-        "@k add.u32 %5, %5, 1;\n\t}"
-        : "=r"(word), "+l"(a[0]), "+l"(a[1]), "+l"(a[2]), "+l"(a[3]), "+r"(cnt)
-        : "f"(x), "f"(r_max), "f"(x_low), "f"(x_high), "f"(gamma), "l"(s[0]), "l"(s[1]), "l"(s[2]), "l"(s[3]));
+        "selp.f32 %1, 0f3F800000, 0f00000000, k;\n\t}"
+        : "=r"(word), "=f"(kf)
+        : "f"(x), "f"(r_max), "f"(x_low), "f"(x_high), "f"(gamma));
+    const f2 kk = pack2(kf, kf);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) a[q] = fma2(s[q], kk, a[q]);
+    cnt += kf;
     return word;
+}
+
+__device__ __forceinline__ bool finite2(f2 v) {
+    float lo, hi;
+    unpack2(v, lo, hi);
+    return fabsf(lo) <= 3.402823466e38f && fabsf(hi) <= 3.402823466e38f;
 }
 
 __device__ __forceinline__ void sts128(uint32_t addr, float a, float b, float c, float d) {
@@ -153,10 +164,10 @@ rfi_batched_tma_kernel(const __grid_constant__ CUtensorMap tmap, const KParams p
         g.word = tile; g.bit = lane; g.group = 0xffffffffu; g.leader = lane == 0;
 
         f2 acc[SPW][4];
-        uint32_t cnt[SPW];
+        float cnt[SPW];
 #pragma unroll
         for (int i = 0; i < SPW; ++i) {
-            cnt[i] = 0;
+            cnt[i] = 0.f;
 #pragma unroll
             for (int q = 0; q < 4; ++q) acc[i][q] = 0ull;
         }
@@ -184,8 +195,9 @@ rfi_batched_tma_kernel(const __grid_constant__ CUtensorMap tmap, const KParams p
                 window_stats(w, inv_M, x, r_re, r_im);
                 const uint32_t ra = rbuf + ((uint32_t)warp * 32u + lane) * kRecBytes;
                 sts128(ra, x, max_nan(r_re, r_im), 0.f, 0.f);
-                sts128_f2(ra + 16, w.s[0], w.s[1]);
-                sts128_f2(ra + 32, w.s[2], w.s[3]);
+                const bool fin = finite2(w.s[0]) && finite2(w.s[1]) && finite2(w.s[2]) && finite2(w.s[3]);
+                sts128_f2(ra + 16, fin ? w.s[0] : 0ull, fin ? w.s[1] : 0ull);
+                sts128_f2(ra + 32, fin ? w.s[2] : 0ull, fin ? w.s[3] : 0ull);
                 if (p.k_first == 0) store_stats(p, g, o_global * p.wpo + wl, p.thr0.c * x, r_re, r_im);
             }
             __syncthreads();
@@ -227,7 +239,7 @@ rfi_batched_tma_kernel(const __grid_constant__ CUtensorMap tmap, const KParams p
 #pragma unroll
         for (int i = 0; i < SPW; ++i) {
             const int k = warp * SPW + i;
-            if (k < p.K) store_output(p, g, p.k_first + k, o_global, acc[i], cnt[i] * (uint32_t)p.M);
+            if (k < p.K) store_output(p, g, p.k_first + k, o_global, acc[i], (uint32_t)cnt[i] * (uint32_t)p.M);
         }
     }
 }
