@@ -4,6 +4,8 @@
 // n_int time samples in blocks of R rows (R divides the window length M).
 #pragma once
 
+#include <type_traits>
+
 #include "rfi_window.cuh"
 
 namespace rfi {
@@ -49,15 +51,7 @@ __global__ void __launch_bounds__(128, 4) rfi_direct_kernel(const KParams p) {
     int blk = 0, b_in_win = 0;
 
     Raw<FP16> A[R], B[R];
-    load_block<R, FP16, ALIGN32>(ptr, row_stride, A);
-    ptr += blk_stride;
-
-    auto step = [&](Raw<FP16> (&cur)[R], Raw<FP16> (&nxt)[R]) {
-        if (blk + 1 < total) {
-            load_block<R, FP16, ALIGN32>(ptr, row_stride, nxt);
-            ptr += blk_stride;
-        }
-        accumulate_block<R, FP16>(w, cur, b_in_win);
+    auto window_end = [&]() {
         ++blk;
         if (++b_in_win == bpw) {
             finish_window(p, g, w, inv_M, w_global, acc, wt);
@@ -66,11 +60,54 @@ __global__ void __launch_bounds__(128, 4) rfi_direct_kernel(const KParams p) {
             w.reset();
         }
     };
-    while (blk + 2 <= total) {
-        step(A, B);
-        step(B, A);
+    if constexpr (FP16) {
+        // Row-granular register ring of 2R rows: a row's registers are refilled (row + 2R) right after the row
+        // is consumed, so between R and 2R-1 rows (128..240 B) per thread are in flight instead of exactly R.
+        // Measured on B200 (profiles/): fp16 1.445 -> 1.321 ms; fp32 loses 1.5 % to spills and keeps the ping-pong.
+        load_block<R, FP16, ALIGN32>(ptr, row_stride, A);
+        if (total > 1) load_block<R, FP16, ALIGN32>(ptr + blk_stride, row_stride, B);
+        ptr += 2 * blk_stride;                        // address of the row that refills A[0]
+        auto step = [&](auto always, Raw<FP16> (&cur)[R]) {
+            const bool refill = decltype(always)::value || blk + 2 < total;
+            float z[R];
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                f2 x[4];
+                widen(cur[r], x);
+                if (refill) ldg_stream(ptr + (size_t)r * row_stride, cur[r]);
+                z[r] = accumulate_sample(w, x);
+            }
+            ptr += blk_stride;
+            merge_block<R>(w, z, b_in_win);
+            window_end();
+        };
+        while (blk + 4 <= total) {                    // both steps refill unconditionally
+            step(std::true_type{}, A);
+            step(std::true_type{}, B);
+        }
+        while (blk + 2 <= total) {
+            step(std::false_type{}, A);
+            step(std::false_type{}, B);
+        }
+        if (blk < total) step(std::false_type{}, A);
+    } else {
+        // Ping-pong: the loads of block i+1 are issued before block i is consumed.
+        load_block<R, FP16, ALIGN32>(ptr, row_stride, A);
+        ptr += blk_stride;
+        auto step = [&](Raw<FP16> (&cur)[R], Raw<FP16> (&nxt)[R]) {
+            if (blk + 1 < total) {
+                load_block<R, FP16, ALIGN32>(ptr, row_stride, nxt);
+                ptr += blk_stride;
+            }
+            accumulate_block<R, FP16>(w, cur, b_in_win);
+            window_end();
+        };
+        while (blk + 2 <= total) {
+            step(A, B);
+            step(B, A);
+        }
+        if (blk < total) step(A, B);
     }
-    if (blk < total) step(A, B);
     store_output(p, g, p.k_first, o_global, acc, wt);
 }
 

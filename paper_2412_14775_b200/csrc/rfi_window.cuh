@@ -52,15 +52,8 @@ __device__ __forceinline__ float accumulate_sample(Win& w, const f2 (&x)[4]) {
 // R samples (one block) of the window; `blk` = index of the block inside the window (0-based).
 // Merge of (n_a = blk*R, mean, m2) with the block's (R, mb, m2b):
 //   delta = mb - mean;  mean += delta/(blk+1);  m2 += m2b + delta^2 * R*blk/(blk+1)
-template <int R, bool FP16>
-__device__ __forceinline__ void accumulate_block(Win& w, const Raw<FP16> (&raw)[R], int blk) {
-    float z[R];
-#pragma unroll
-    for (int r = 0; r < R; ++r) {
-        f2 x[4];
-        widen(raw[r], x);
-        z[r] = accumulate_sample(w, x);
-    }
+template <int R>
+__device__ __forceinline__ void merge_block(Win& w, const float (&z)[R], int blk) {
     float zs = z[0];
 #pragma unroll
     for (int r = 1; r < R; ++r) zs += z[r];
@@ -76,6 +69,18 @@ __device__ __forceinline__ void accumulate_block(Win& w, const Raw<FP16> (&raw)[
     const float delta = mb - w.mean;
     w.mean = fmaf(delta, wgt, w.mean);
     w.m2 += fmaf(delta * delta, (float)R * fb * wgt, m2b);
+}
+
+template <int R, bool FP16>
+__device__ __forceinline__ void accumulate_block(Win& w, const Raw<FP16> (&raw)[R], int blk) {
+    float z[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        f2 x[4];
+        widen(raw[r], x);
+        z[r] = accumulate_sample(w, x);
+    }
+    merge_block<R>(w, z, blk);
 }
 
 // sqrt(s) for s >= 0 from the hardware rsqrt plus one Newton step on the residual s - r^2 (an fma, exact):
