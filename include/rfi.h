@@ -87,6 +87,13 @@ int rfi_plan_create(rfi_plan **out, int n_stations, int n_baselines, int n_chan,
 /* Samples per output integration: n_time % n_int == 0 and n_int % window_M == 0, else RFI_EINVAL. */
 int rfi_plan_set_integration(rfi_plan *plan, int n_int);
 
+/* Multi-GPU sharding (every baseline stream is mitigated separately, so streams partition across
+ * devices with no exchange).  Declares that this plan processes only baselines [b_first, b_first + b_count) of the
+ * n_baselines given at creation: from now on every buffer (vis, avg, weight, stats, flags) holds b_count baselines
+ * in place of n_baselines, in the same layouts.  RFI_EINVAL unless 0 <= b_first, b_count >= 1 and
+ * b_first + b_count <= n_baselines.  Results equal the corresponding slices of an unsharded run bit for bit. */
+int rfi_plan_set_baseline_shard(rfi_plan *plan, int b_first, int b_count);
+
 /* Copy K >= 1 threshold sets from host memory (d > 0 and not NaN; s_low/s_high/gamma may be +-inf, not NaN).
  * K == 1 runs the single-set kernel; K > 1 the batched kernel that evaluates up to 64 sets in one pass over the
  * data (one launch per 64 sets; the paper tunes its thresholds with a host-side search).

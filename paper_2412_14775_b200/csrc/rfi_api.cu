@@ -45,6 +45,7 @@ struct MapEntry {
 
 struct rfi_plan {
     int n_stations, n_baselines, n_chan, n_time, M, precision, n_int;
+    int n_baselines_total = 0, b_first = 0;   // n_baselines is the shard this plan processes (default: all)
     int K = 0;
     std::vector<rfi_thresholds> thr;
     int variant = RFI_VARIANT_AUTO;
@@ -274,6 +275,7 @@ int rfi_plan_create(rfi_plan** out, int n_stations, int n_baselines, int n_chan,
     if (!p) return RFI_ENOMEM;
     p->n_stations = n_stations;
     p->n_baselines = n_baselines;
+    p->n_baselines_total = n_baselines;
     p->n_chan = n_chan;
     p->n_time = n_time;
     p->M = window_M;
@@ -288,6 +290,15 @@ int rfi_plan_set_integration(rfi_plan* p, int n_int) {
     if (p->n_time % n_int != 0 || n_int % p->M != 0) return RFI_EINVAL;
     p->n_int = n_int;
     p->have_result = false;
+    return RFI_OK;
+}
+
+int rfi_plan_set_baseline_shard(rfi_plan* p, int b_first, int b_count) {
+    if (!p || b_first < 0 || b_count < 1 || (long)b_first + b_count > p->n_baselines_total) return RFI_EINVAL;
+    p->b_first = b_first;
+    p->n_baselines = b_count;
+    p->have_result = false;
+    p->maps.clear();
     return RFI_OK;
 }
 

@@ -85,6 +85,18 @@ def test_integration_and_threshold_validation():
     p.destroy()
 
 
+def test_baseline_shard_validation():
+    plan = rfi.RfiPlan(48, 1176, 64, 7680, 16)
+    plan.set_baseline_shard(588, 588)
+    assert plan.n_baselines == 588 and plan.b_first == 588
+    for first, count in ((-1, 4), (0, 0), (1000, 177), (1176, 1)):
+        with pytest.raises(rfi.RfiError) as e:
+            plan.set_baseline_shard(first, count)
+        assert e.value.code == -1
+    plan.set_baseline_shard(0, 1176)
+    plan.destroy()
+
+
 def test_call_order_errors():
     p = rfi.RfiPlan(4, 6, 16, 1024, 64)
     lib = rfi.load_library()

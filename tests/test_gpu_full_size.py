@@ -1,0 +1,77 @@
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times: the whole chunk is
+generated and processed on the device; a seeded sample of cells (all time samples of each) is brought back and
+compared with the fp64 oracle element by element, plus properties that hold at any size."""
+import numpy as np
+import pytest
+import torch
+
+import paper_2412_14775_b200 as rfi
+from paper_2412_14775_b200 import synth
+from tests.parity_util import compare
+
+pytestmark = pytest.mark.gpu
+
+
+def _sample_cells(w, truth, n_clean, n_rfi, seed):
+    g = torch.Generator().manual_seed(seed)
+    has = truth.any(0).cpu()
+    rfi_cells = torch.nonzero(has).flatten()
+    clean = torch.nonzero(~has).flatten()
+    pick = torch.cat([rfi_cells[torch.randperm(rfi_cells.numel(), generator=g)[:n_rfi]],
+                      clean[torch.randperm(clean.numel(), generator=g)[:n_clean]]])
+    return pick.sort().values
+
+
+def _run_full(name, K, n_clean=768, n_rfi=256):
+    w = synth.WORKLOADS[name]
+    need = w.input_bytes * 1.15 + 6e9
+    if torch.cuda.mem_get_info()[0] < need:
+        pytest.skip("not enough free device memory for the full-size chunk")
+    dev = torch.device("cuda")
+    vis, truth = synth.make_chunk(w, seed=1234, device=dev)
+    thr = synth.default_thresholds(w.window_M) if K == 1 else synth.sweep_thresholds(w.window_M, K)
+    plan = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M,
+                       rfi.RFI_FP16 if w.fp16 else rfi.RFI_FP32, n_int=w.n_int)
+    plan.set_thresholds(thr)
+    avg, weight, stats = plan.alloc_outputs(stats=True)
+    plan.process_chunk(vis, avg, weight, stats)                 # auto variant: what bench.py times
+    torch.cuda.synchronize()
+    assert plan.launch_count == 1
+    flags = rfi.unpack_flags(plan.get_flags(), w.n_chan).reshape(K, plan.n_win, plan.n_cells)
+    # properties at full size
+    wt = weight.reshape(K, plan.n_out, plan.n_cells).long()
+    kept = (~flags).reshape(K, plan.n_out, w.n_int // w.window_M, plan.n_cells).sum(2) * w.window_M
+    assert torch.equal(wt, kept)                                 # weight = unflagged sample count
+    assert torch.isfinite(avg).all()
+    s = stats.reshape(3, plan.n_win, plan.n_cells)
+    assert (s[1] >= 0).all() and (s[1] <= 1 + 1e-6).all() and (s[2] >= 0).all() and (s[2] <= 1 + 1e-6).all()
+    # sampled cells against the oracle
+    idx = _sample_cells(w, truth.reshape(plan.n_win, plan.n_cells), n_clean, n_rfi, seed=3).to(dev)
+    sub = vis.reshape(w.n_time, plan.n_cells, 4, 2)[:, idx].cpu().numpy()
+    out = {
+        "avg": avg.reshape(K, plan.n_out, plan.n_cells, 4, 2)[:, :, idx].cpu().numpy().view(np.complex64).reshape(K, plan.n_out, -1, 4),
+        "weight": wt[:, :, idx].cpu().numpy(),
+        "flags": flags[:, :, idx].cpu().numpy(),
+        "tau": s[0][:, idx].cpu().numpy(), "r_re": s[1][:, idx].cpu().numpy(), "r_im": s[2][:, idx].cpu().numpy(),
+    }
+    used = plan.last_variant
+    plan.destroy()
+    del vis, avg, weight, stats
+    torch.cuda.empty_cache()
+    rep = compare(sub, w.window_M, w.n_int, thr, out, tol=2e-3 if w.fp16 else 1e-5, fp16=w.fp16)
+    return rep, used
+
+
+def test_lofar_fp32_full_size():
+    rep, used = _run_full("lofar", 1)
+    assert used == "direct" and rep["flag_mismatch_unexplained"] == 0
+
+
+def test_lofar_fp16_full_size():
+    rep, used = _run_full("lofar_fp16", 1)
+    assert rep["flag_agreement"] >= 0.999
+
+
+def test_sweep_K64_full_size():
+    rep, used = _run_full("sweep", 64, n_clean=192, n_rfi=64)
+    assert used == "batched" and rep["K"] == 64 and rep["flag_mismatch_unexplained"] == 0

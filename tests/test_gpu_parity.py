@@ -172,6 +172,32 @@ def test_host_path_equals_device_path():
         np.testing.assert_array_equal(out_dev[key], out_host[key])
 
 
+@pytest.mark.parametrize("K", [1, 5])
+def test_baseline_shards_equal_slices_of_the_full_run(K):
+    """shard by baseline with no exchange -- two shard plans reproduce the full run bit for bit."""
+    from paper_2412_14775_b200 import sharding
+    w = synth.WORKLOADS["lofar"].scaled(n_stations=6, n_time=512, n_int=256, burst_cell_frac=0.1)
+    vis, _ = synth.make_chunk(w, seed=17)
+    thr = synth.default_thresholds(16) if K == 1 else synth.sweep_thresholds(16, K, seed=2)
+    full, _ = run_gpu(w, vis, thr, "auto")
+    B, C = w.n_baselines, w.n_chan
+    for rank in range(2):
+        b0, bc = sharding.shard_baselines(B, 2, rank)
+        plan = rfi.RfiPlan(w.n_stations, B, C, w.n_time, w.window_M, n_int=w.n_int)
+        plan.set_baseline_shard(b0, bc)
+        plan.set_thresholds(thr)
+        avg, weight, stats = plan.alloc_outputs(stats=True)
+        plan.process_chunk(vis[:, b0:b0 + bc].contiguous().cuda(), avg, weight, stats)
+        torch.cuda.synchronize()
+        out = gpu_outputs_to_numpy(plan, avg, weight, stats, rfi.unpack_flags(plan.get_flags(), C))
+        plan.destroy()
+        sl = slice(b0 * C, (b0 + bc) * C)
+        for key in ("avg", "weight", "flags"):
+            np.testing.assert_array_equal(out[key], full[key][:, :, sl])
+        for key in ("tau", "r_re", "r_im"):
+            np.testing.assert_array_equal(out[key], full[key][:, sl])
+
+
 def test_variants_agree_bit_for_bit(monkeypatch):
     """Same block length R (rows merged at a time) -> the two load paths feed identical arithmetic."""
     monkeypatch.setenv("RFI_DIRECT_ROWS", "4")

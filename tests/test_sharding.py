@@ -1,0 +1,67 @@
+"""Multi-GPU host logic on CPU: world_size-2 gloo processes (shard by baseline, no data-path collective)."""
+import os
+import socket
+
+import numpy as np
+import pytest
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+from paper_2412_14775_b200 import sharding
+
+
+@pytest.mark.parametrize("n,world", [(1176, 1), (1176, 2), (1176, 8), (6, 4), (3, 8), (2926, 7)])
+def test_shard_baselines_is_a_contiguous_balanced_partition(n, world):
+    parts = [sharding.shard_baselines(n, world, r) for r in range(world)]
+    assert parts[0][0] == 0 and sum(c for _, c in parts) == n
+    for (f0, c0), (f1, _) in zip(parts, parts[1:]):
+        assert f1 == f0 + c0
+    counts = [c for _, c in parts]
+    assert max(counts) - min(counts) <= 1
+    with pytest.raises(ValueError):
+        sharding.shard_baselines(n, world, world)
+
+
+def test_confusion_counts_by_hand():
+    flags = torch.tensor([[[1, 0, 1], [0, 0, 1]], [[0, 0, 0], [1, 1, 1]]]).bool()      # [K=2, W=2, cells=3]
+    truth = torch.tensor([[1, 0, 0], [0, 0, 1]]).bool()
+    c = sharding.confusion_counts(flags, truth)
+    assert c.tolist() == [[1, 4, 0, 2], [2, 4, 1, 2]]
+    fa, md = sharding.rates(c)
+    assert fa.tolist() == [0.25, 0.5] and md.tolist() == [0.0, 0.5]
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _worker(rank, world, port, n_baselines, n_chan, n_win, K, out_dir):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        # the same seeded global masks on every rank; each rank keeps its baseline slice only
+        g = torch.Generator().manual_seed(5)
+        flags = torch.rand(K, n_win, n_baselines, n_chan, generator=g) < 0.1
+        truth = torch.rand(n_win, n_baselines, n_chan, generator=g) < 0.05
+        b0, bc = sharding.shard_baselines(n_baselines, world, rank)
+        mine = sharding.confusion_counts(flags[:, :, b0:b0 + bc].flatten(2), truth[:, b0:b0 + bc].flatten(1))
+        total = sharding.sum_over_ranks(mine.clone())
+        full = sharding.confusion_counts(flags.flatten(2), truth.flatten(1))
+        assert torch.equal(total, full), (total, full)
+        # device-time bookkeeping: MAX over ranks
+        t = sharding.max_over_ranks(1.0 + rank)
+        assert t == float(world)
+        dist.barrier()
+        np.save(os.path.join(out_dir, f"ok{rank}.npy"), np.array([b0, bc]))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_world_size_2_gloo_partition_and_reductions(tmp_path):
+    world = 2
+    mp.spawn(_worker, args=(world, _free_port(), 15, 4, 6, 3, str(tmp_path)), nprocs=world, join=True)
+    parts = [np.load(tmp_path / f"ok{r}.npy") for r in range(world)]
+    assert parts[0].tolist() == [0, 8] and parts[1].tolist() == [8, 7]
