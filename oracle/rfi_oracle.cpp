@@ -151,29 +151,36 @@ int oracle_rfi_decide(double tau, double r_re, double r_im,
 // The whole path on one chunk.
 //
 //   vis      [n_time][n_cells][4 pols][re,im], storage 0/1/2 (f32/f16/f64), time slowest.
-//            A "cell" is one (baseline, channel) stream; cells are independent,
-//            so any subset of cells may be passed.
-//   M        window length W (time samples; F = 1, reading G7).   M >= 2.
+//            A "cell" is one (baseline, channel) stream; baselines are independent,
+//            so any subset of cells (whole groups of F adjacent channels) may be passed.
+//   M, F     window footprint: T = M time samples x F frequency samples, W = T x F (
+//            typical W = 20 as 10 x 2 or 5 x 4).  The F channels of a window are
+//            F consecutive cells (n_cells % F == 0).  F = 1 is the per-channel window (reading G7).
+//            The statistics of Eq.(3)-(4) and Eq.(6)-(9) run over all W samples of the footprint;
+//            the flag applies to all of them.  M * F >= 2.
 //   n_int    samples per output integration; n_time % n_int == 0, n_int % M == 0 (reading G8).
 //   thr      [K][4] = d, s_low, s_high, gamma for each threshold set.
-// Outputs (any may be NULL):
+// Outputs (any may be NULL), all per cell (the F cells of a window carry the same statistics and flag):
 //   tau      [K][n_win][n_cells]       n_win = n_time / M, window index w counts from chunk start
 //   r_re,r_im[n_win][n_cells]
 //   flags    [K][n_win][n_cells]       1 = flagged
-//   avg      [K][n_out][n_cells][8]    mean of the unflagged samples, 0 if none
-//   weight   [K][n_out][n_cells]       number of unflagged samples
+//   avg      [K][n_out][n_cells][8]    mean of the unflagged samples of the cell, 0 if none;
+//                                      no averaging across frequency (reading G9)
+//   weight   [K][n_out][n_cells]       number of unflagged samples of the cell
 // Returns 0, or -1 on invalid arguments.
-int oracle_rfi_process(const void* vis, int storage,
-                       int64_t n_time, int64_t n_cells, int M, int64_t n_int,
-                       int K, const double* thr,
-                       double* tau, double* r_re, double* r_im, uint8_t* flags,
-                       double* avg, int64_t* weight, int n_threads) {
-    if (!vis || !thr || M < 2 || n_int <= 0 || n_time <= 0 || n_cells < 0 || K < 1) return -1;
-    if (n_time % n_int != 0 || n_int % M != 0) return -1;
+int oracle_rfi_process_tf(const void* vis, int storage,
+                          int64_t n_time, int64_t n_cells, int M, int F, int64_t n_int,
+                          int K, const double* thr,
+                          double* tau, double* r_re, double* r_im, uint8_t* flags,
+                          double* avg, int64_t* weight, int n_threads) {
+    if (!vis || !thr || M < 1 || F < 1 || M * F < 2 || n_int <= 0 || n_time <= 0 || n_cells < 0 || K < 1) return -1;
+    if (n_time % n_int != 0 || n_int % M != 0 || n_cells % F != 0) return -1;
     if (storage < 0 || storage > 2) return -1;
     const int64_t n_win = n_time / M;
     const int64_t n_out = n_time / n_int;
     const int64_t win_per_out = n_int / M;
+    const int64_t n_groups = n_cells / F;
+    const int W = M * F;
 #ifdef _OPENMP
     if (n_threads > 0) omp_set_num_threads(n_threads);
 #else
@@ -181,53 +188,71 @@ int oracle_rfi_process(const void* vis, int storage,
 #endif
 
 #pragma omp parallel for schedule(static)
-    for (int64_t cell = 0; cell < n_cells; ++cell) {
-        double* win = new double[static_cast<size_t>(M) * 8];
+    for (int64_t grp = 0; grp < n_groups; ++grp) {
+        const int64_t cell0 = grp * F;
+        double* win = new double[static_cast<size_t>(W) * 8];      // sample (i, f) at index i * F + f
+        double* acc = new double[static_cast<size_t>(K) * F * 8];
+        int64_t* cnt = new int64_t[static_cast<size_t>(K) * F];
         for (int64_t o = 0; o < n_out; ++o) {
-            // per-set running sums for this output
-            double* acc = new double[static_cast<size_t>(K) * 8];
-            int64_t* cnt = new int64_t[K];
-            for (int k = 0; k < K; ++k) { cnt[k] = 0; for (int p = 0; p < 8; ++p) acc[k * 8 + p] = 0.0; }
+            // per-set, per-channel running sums for this output
+            for (int64_t j = 0; j < static_cast<int64_t>(K) * F; ++j) { cnt[j] = 0; for (int p = 0; p < 8; ++p) acc[j * 8 + p] = 0.0; }
 
             for (int64_t wl = 0; wl < win_per_out; ++wl) {
                 const int64_t w = o * win_per_out + wl;
                 for (int i = 0; i < M; ++i) {
                     const int64_t t = w * M + i;
-                    for (int p = 0; p < 8; ++p)
-                        win[i * 8 + p] = load_real(vis, storage, (t * n_cells + cell) * 8 + p);
+                    for (int f = 0; f < F; ++f)
+                        for (int p = 0; p < 8; ++p)
+                            win[(i * F + f) * 8 + p] = load_real(vis, storage, (t * n_cells + cell0 + f) * 8 + p);
                 }
                 for (int k = 0; k < K; ++k) {
                     const double d = thr[k * 4 + 0], s_low = thr[k * 4 + 1];
                     const double s_high = thr[k * 4 + 2], gamma = thr[k * 4 + 3];
                     double t_k, rr, ri;
-                    oracle_rfi_window_stats(win, M, d, &t_k, &rr, &ri);
-                    const int f = oracle_rfi_decide(t_k, rr, ri, s_low, s_high, gamma);
-                    if (tau)   tau[(static_cast<int64_t>(k) * n_win + w) * n_cells + cell] = t_k;
-                    if (flags) flags[(static_cast<int64_t>(k) * n_win + w) * n_cells + cell] = static_cast<uint8_t>(f);
-                    if (k == 0) {
-                        if (r_re) r_re[w * n_cells + cell] = rr;
-                        if (r_im) r_im[w * n_cells + cell] = ri;
-                    }
-                    if (!f) {                                   // flagged windows are excluded
-                        for (int i = 0; i < M; ++i)
-                            for (int p = 0; p < 8; ++p) acc[k * 8 + p] += win[i * 8 + p];
-                        cnt[k] += M;
+                    oracle_rfi_window_stats(win, W, d, &t_k, &rr, &ri);
+                    const int fl = oracle_rfi_decide(t_k, rr, ri, s_low, s_high, gamma);
+                    for (int f = 0; f < F; ++f) {
+                        const int64_t cell = cell0 + f;
+                        if (tau)   tau[(static_cast<int64_t>(k) * n_win + w) * n_cells + cell] = t_k;
+                        if (flags) flags[(static_cast<int64_t>(k) * n_win + w) * n_cells + cell] = static_cast<uint8_t>(fl);
+                        if (k == 0) {
+                            if (r_re) r_re[w * n_cells + cell] = rr;
+                            if (r_im) r_im[w * n_cells + cell] = ri;
+                        }
+                        if (!fl) {                              // flagged windows are excluded
+                            for (int i = 0; i < M; ++i)
+                                for (int p = 0; p < 8; ++p) acc[(k * F + f) * 8 + p] += win[(i * F + f) * 8 + p];
+                            cnt[k * F + f] += M;
+                        }
                     }
                 }
             }
-            for (int k = 0; k < K; ++k) {
-                const int64_t oi = (static_cast<int64_t>(k) * n_out + o) * n_cells + cell;
-                if (weight) weight[oi] = cnt[k];
-                if (avg)
-                    for (int p = 0; p < 8; ++p)
-                        avg[oi * 8 + p] = cnt[k] ? acc[k * 8 + p] / static_cast<double>(cnt[k]) : 0.0;
-            }
-            delete[] acc;
-            delete[] cnt;
+            for (int k = 0; k < K; ++k)
+                for (int f = 0; f < F; ++f) {
+                    const int64_t oi = (static_cast<int64_t>(k) * n_out + o) * n_cells + cell0 + f;
+                    const int64_t n = cnt[k * F + f];
+                    if (weight) weight[oi] = n;
+                    if (avg)
+                        for (int p = 0; p < 8; ++p)
+                            avg[oi * 8 + p] = n ? acc[(k * F + f) * 8 + p] / static_cast<double>(n) : 0.0;
+                }
         }
+        delete[] acc;
+        delete[] cnt;
         delete[] win;
     }
     return 0;
+}
+
+// The per-channel window (F = 1, M >= 2): the main path of the build (reading G7).
+int oracle_rfi_process(const void* vis, int storage,
+                       int64_t n_time, int64_t n_cells, int M, int64_t n_int,
+                       int K, const double* thr,
+                       double* tau, double* r_re, double* r_im, uint8_t* flags,
+                       double* avg, int64_t* weight, int n_threads) {
+    if (M < 2) return -1;
+    return oracle_rfi_process_tf(vis, storage, n_time, n_cells, M, 1, n_int, K, thr,
+                                 tau, r_re, r_im, flags, avg, weight, n_threads);
 }
 
 // Bit-packed flag mask in the boundary's layout (include/rfi.h):

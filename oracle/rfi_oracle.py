@@ -50,6 +50,10 @@ def _load():
             ctypes.c_void_p, ctypes.c_int, ctypes.c_int64, ctypes.c_int64, ctypes.c_int, ctypes.c_int64,
             ctypes.c_int, c_dp, c_dp, c_dp, c_dp, ctypes.c_void_p, c_dp, ctypes.c_void_p, ctypes.c_int]
         lib.oracle_rfi_process.restype = ctypes.c_int
+        lib.oracle_rfi_process_tf.argtypes = [
+            ctypes.c_void_p, ctypes.c_int, ctypes.c_int64, ctypes.c_int64, ctypes.c_int, ctypes.c_int, ctypes.c_int64,
+            ctypes.c_int, c_dp, c_dp, c_dp, c_dp, ctypes.c_void_p, c_dp, ctypes.c_void_p, ctypes.c_int]
+        lib.oracle_rfi_process_tf.restype = ctypes.c_int
         lib.oracle_rfi_pack_flags.argtypes = [ctypes.c_void_p, ctypes.c_int64, ctypes.c_int64,
                                               ctypes.c_int64, ctypes.c_void_p]
         lib.oracle_rfi_pack_flags.restype = ctypes.c_int
@@ -98,8 +102,9 @@ class OracleResult:
     weight: np.ndarray   # [K, n_out, n_cells] int64
 
 
-def process(vis, M: int, n_int: int, thresholds, n_threads: int = 0, want_stats: bool = True) -> OracleResult:
-    """Run the whole path.
+def process(vis, M: int, n_int: int, thresholds, n_threads: int = 0, want_stats: bool = True,
+            F: int = 1) -> OracleResult:
+    """Run the whole path.  Window footprint: M time samples x F adjacent cells (W = M*F).
 
     vis: real array [n_time, n_cells, 4, 2] (float16/32/64) or complex [n_time, n_cells, 4].
     thresholds: [K,4] rows of (d, s_low, s_high, gamma).
@@ -122,8 +127,8 @@ def process(vis, M: int, n_int: int, thresholds, n_threads: int = 0, want_stats:
     flags = np.empty((K, n_win, n_cells), np.uint8)
     avg = np.empty((K, n_out, n_cells, 8), np.float64)
     weight = np.empty((K, n_out, n_cells), np.int64)
-    rc = _load().oracle_rfi_process(
-        a.ctypes.data, _STORAGE[a.dtype], n_time, n_cells, int(M), int(n_int), K, _dp(thr),
+    rc = _load().oracle_rfi_process_tf(
+        a.ctypes.data, _STORAGE[a.dtype], n_time, n_cells, int(M), int(F), int(n_int), K, _dp(thr),
         _dp(tau), _dp(r_re), _dp(r_im), flags.ctypes.data, _dp(avg), weight.ctypes.data, int(n_threads))
     if rc != 0:
         raise ValueError("oracle_rfi_process: invalid arguments")

@@ -75,3 +75,10 @@ def test_lofar_fp16_full_size():
 def test_sweep_K64_full_size():
     rep, used = _run_full("sweep", 64, n_clean=192, n_rfi=64)
     assert used == "batched" and rep["K"] == 64 and rep["flag_mismatch_unexplained"] == 0
+
+
+def test_large_array_full_size():
+    """BASELINE.json configs[3] as read in DESIGN.md (C4): 2926 baselines x 256 channels, W=32, one 3072-sample
+    integration per chunk (73.6 GB); bursts, tones and 100-sigma unpolarised spikes."""
+    rep, used = _run_full("large", 1, n_clean=384, n_rfi=384)
+    assert used == "direct" and rep["flag_mismatch_unexplained"] == 0

@@ -486,3 +486,70 @@ def test_invalid_arguments_rejected():
         orc.process(vis, 3, 16, [NO_FLAG])       # n_int % M
     with pytest.raises(ValueError):
         orc.process(vis, 4, 12, [NO_FLAG])       # n_time % n_int
+
+
+# ----------------------------------------------------------------------------------------------
+# T x F window footprints, W = T x F (10 x 2 and 5 x 4 at PAPER.md:182,233,241)
+# ----------------------------------------------------------------------------------------------
+def test_tf_hand_worked_2x2():
+    """2 time x 2 channel footprint with |I| = 1,2 (channel 0) and 3,4 (channel 1): the same four amplitudes as
+    the hand-worked W=4 window -> x = 0.2, tau(d=1) = 1/3; all Q > 0 -> r_re = 1.  Catches: W taken as T."""
+    vis = np.zeros((2, 2, 4), np.complex128)
+    vis[:, 0, 0] = [1, 2]
+    vis[:, 1, 0] = [3, 4]
+    res = orc.process(vis, 2, 2, [NO_FLAG], F=2)
+    assert res.tau[0, 0, 0] == pytest.approx(1 / 3, rel=1e-14) and res.tau[0, 0, 1] == res.tau[0, 0, 0]
+    assert res.r_re[0, 0] == pytest.approx(1.0, rel=1e-14) and res.r_im[0, 1] == 0.0
+
+
+@pytest.mark.parametrize("T,F", [(10, 2), (5, 4), (1, 8), (16, 1), (3, 3)])
+def test_tf_window_equals_time_window_of_the_rearranged_samples(T, F):
+    """The statistics are sums over the W = T*F samples of the footprint, so they must equal those of a
+    per-channel window of length W holding the same samples (the F = 1 path is pinned by the closed forms above).
+    Catches: a channel left out, per-channel instead of joint statistics, W = T in Eq.(4)/(9)."""
+    rng = np.random.default_rng(T * 10 + F)
+    n_win = 3
+    vis = rng.normal(size=(n_win * T, 2 * F, 4)) + 1j * rng.normal(size=(n_win * T, 2 * F, 4))
+    vis[T:2 * T, :F] += 4 * coherency(np.array([0.6, 0.8j]))          # a polarised window in group 0
+    thr = [[0.7, 0.1, 1.1, 0.55]]
+    res = orc.process(vis, T, T, thr, F=F)
+    for grp in range(2):
+        flat = vis[:, grp * F:(grp + 1) * F].reshape(n_win * T * F, 1, 4)   # window w -> rows w*T*F ... (t-major, f inner)
+        ref = orc.process(flat, T * F, T * F, thr)
+        for f in range(F):
+            c = grp * F + f
+            np.testing.assert_allclose(res.tau[0][:, c], ref.tau[0][:, 0], rtol=1e-13, atol=1e-15)
+            np.testing.assert_allclose(res.r_re[:, c], ref.r_re[:, 0], rtol=1e-13, atol=1e-15)
+            np.testing.assert_allclose(res.r_im[:, c], ref.r_im[:, 0], rtol=1e-13, atol=1e-15)
+            np.testing.assert_array_equal(res.flags[0][:, c], ref.flags[0][:, 0])
+    assert res.flags[0][1, :F].all() and not res.flags[0][1, F:].all()
+
+
+def test_tf_exclusion_is_per_footprint_and_average_per_channel():
+    """A burst in ONE channel flags the whole T x F footprint: both channels lose that window's
+    samples, and each channel's average is the plain mean of its own remaining samples (no frequency averaging)."""
+    rng = np.random.default_rng(77)
+    T, F, n_win = 5, 2, 4
+    vis = 0.1 * (rng.normal(size=(n_win * T, F, 4)) + 1j * rng.normal(size=(n_win * T, F, 4)))
+    vis[2 * T:3 * T, 1] += 10 * coherency(np.array([0.6, 0.8j]))
+    # half of the footprint at amplitude ~10, half at ~0.1: x = W S2/S1^2 - 1 ~ 1, tau ~ 11/9; noise windows ~0.3
+    res = orc.process(vis, T, n_win * T, [[1.0, -INF, 1.0, INF]], F=F)
+    assert res.tau[0][2, 0] == pytest.approx(11 / 9, rel=0.15) and res.tau[0][[0, 1, 3], 0].max() < 0.9
+    assert res.flags[0][:, 0].tolist() == [0, 0, 1, 0] and res.flags[0][:, 1].tolist() == [0, 0, 1, 0]
+    keep = np.r_[0:2 * T, 3 * T:4 * T]
+    assert res.weight[0, 0].tolist() == [3 * T, 3 * T]
+    for c in range(F):
+        np.testing.assert_allclose(res.avg[0, 0, c], vis[keep, c].mean(0), rtol=1e-12, atol=1e-15)
+
+
+def test_tf_f1_is_the_per_channel_path_and_bad_shapes_are_rejected():
+    rng = np.random.default_rng(5)
+    vis = rng.normal(size=(32, 6, 4)) + 1j * rng.normal(size=(32, 6, 4))
+    a = orc.process(vis, 8, 16, [[1.0, 0.1, 0.9, 0.5]])
+    b = orc.process(vis, 8, 16, [[1.0, 0.1, 0.9, 0.5]], F=1)
+    for key in ("tau", "r_re", "r_im", "flags", "avg", "weight"):
+        np.testing.assert_array_equal(getattr(a, key), getattr(b, key))
+    with pytest.raises(ValueError):
+        orc.process(vis, 8, 16, [NO_FLAG], F=4)           # 6 cells are not whole groups of 4
+    with pytest.raises(ValueError):
+        orc.process(vis, 1, 16, [NO_FLAG], F=1)           # W = 1: Eq.(4) divides by W - 1
