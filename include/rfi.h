@@ -87,6 +87,15 @@ int rfi_plan_create(rfi_plan **out, int n_stations, int n_baselines, int n_chan,
 /* Samples per output integration: n_time % n_int == 0 and n_int % window_M == 0, else RFI_EINVAL. */
 int rfi_plan_set_integration(rfi_plan *plan, int n_int);
 
+/* Window footprint in frequency ("a data window of size W divided into T time samples and F
+ * frequency samples, W = T x F"; the paper uses 10 x 2 and 5 x 4).  T is the window_M of
+ * rfi_plan_create, F defaults to 1.  With F > 1 a window covers F adjacent channels of one baseline: the
+ * statistics of Eq.(3)-(4) and Eq.(6)-(9) run over all W = T*F samples (W replaces window_M in both equations),
+ * the flag applies to the whole footprint, and every channel is still averaged on its own.  All
+ * buffer layouts are unchanged (the F channels of a footprint carry the same statistics and flag bit).
+ * RFI_EINVAL unless F is a power of two, F <= 32 and n_chan % F == 0. */
+int rfi_plan_set_window_freq(rfi_plan *plan, int F);
+
 /* Multi-GPU sharding (every baseline stream is mitigated separately, so streams partition across
  * devices with no exchange).  Declares that this plan processes only baselines [b_first, b_first + b_count) of the
  * n_baselines given at creation: from now on every buffer (vis, avg, weight, stats, flags) holds b_count baselines

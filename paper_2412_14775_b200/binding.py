@@ -19,7 +19,7 @@ VARIANT_AUTO, VARIANT_DIRECT, VARIANT_TMA = 0, 1, 2
 _VARIANTS = {"auto": 0, "direct": 1, "tma": 2}
 
 EXPORTS = [
-    "rfi_plan_create", "rfi_plan_set_integration", "rfi_plan_set_baseline_shard", "rfi_set_thresholds", "rfi_plan_set_variant",
+    "rfi_plan_create", "rfi_plan_set_integration", "rfi_plan_set_baseline_shard", "rfi_plan_set_window_freq", "rfi_set_thresholds", "rfi_plan_set_variant",
     "rfi_process_chunk", "rfi_get_flags", "rfi_process_chunk_host", "rfi_plan_destroy",
     "rfi_strerror", "rfi_last_cuda_error", "rfi_flags_bytes", "rfi_avg_bytes", "rfi_weight_bytes",
     "rfi_stats_bytes", "rfi_vis_bytes", "rfi_plan_launch_count", "rfi_plan_last_variant", "rfi_version",
@@ -62,13 +62,15 @@ def load_library(build_if_missing: bool = True):
     lib.rfi_plan_create.argtypes = [ctypes.POINTER(vp), ci, ci, ci, ci, ci, ci]
     lib.rfi_plan_set_integration.argtypes = [vp, ci]
     lib.rfi_plan_set_baseline_shard.argtypes = [vp, ci, ci]
+    lib.rfi_plan_set_window_freq.argtypes = [vp, ci]
     lib.rfi_set_thresholds.argtypes = [vp, ci, ctypes.POINTER(RfiThresholds)]
     lib.rfi_plan_set_variant.argtypes = [vp, ci]
     lib.rfi_process_chunk.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.rfi_get_flags.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(sz)]
     lib.rfi_process_chunk_host.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.rfi_plan_destroy.argtypes = [vp]
-    for name in ("rfi_plan_create", "rfi_plan_set_integration", "rfi_plan_set_baseline_shard", "rfi_set_thresholds", "rfi_plan_set_variant",
+    for name in ("rfi_plan_create", "rfi_plan_set_integration", "rfi_plan_set_baseline_shard",
+                 "rfi_plan_set_window_freq", "rfi_set_thresholds", "rfi_plan_set_variant",
                  "rfi_process_chunk", "rfi_get_flags", "rfi_process_chunk_host", "rfi_plan_destroy",
                  "rfi_plan_last_variant"):
         getattr(lib, name).restype = ci
@@ -107,6 +109,7 @@ class RfiPlan:
         self.n_int = n_time
         self.K = 0
         self.b_first = 0
+        self.window_F = 1
         if n_int is not None:
             self.set_integration(n_int)
 
@@ -124,6 +127,11 @@ class RfiPlan:
     def set_integration(self, n_int: int):
         _check(self._lib.rfi_plan_set_integration(self._h, n_int), "rfi_plan_set_integration")
         self.n_int = n_int
+
+    def set_window_freq(self, F: int):
+        """rfi_plan_set_window_freq: T x F footprints, W = window_M * F."""
+        _check(self._lib.rfi_plan_set_window_freq(self._h, F), "rfi_plan_set_window_freq")
+        self.window_F = F
 
     def set_baseline_shard(self, b_first: int, b_count: int):
         """rfi_plan_set_baseline_shard: this plan processes baselines [b_first, b_first + b_count) only."""

@@ -45,6 +45,7 @@ struct MapEntry {
 
 struct rfi_plan {
     int n_stations, n_baselines, n_chan, n_time, M, precision, n_int;
+    int F = 1;                                // window extent in frequency (channels), W = M * F
     int n_baselines_total = 0, b_first = 0;   // n_baselines is the shard this plan processes (default: all)
     int K = 0;
     std::vector<rfi_thresholds> thr;
@@ -102,9 +103,9 @@ int ensure_device(rfi_plan* p) {
     return RFI_OK;
 }
 
-rfi::Thr to_device_thr(const rfi_thresholds& t, int M) {
+rfi::Thr to_device_thr(const rfi_thresholds& t, int W) {
     rfi::Thr r;
-    r.c = (float)(((double)M * (double)t.d + 1.0) / ((double)M - 1.0));
+    r.c = (float)(((double)W * (double)t.d + 1.0) / ((double)W - 1.0));
     // Eq.(5) on x = tau / c (c > 0): +-inf stay +-inf, 0 stays 0
     r.x_low = (float)((double)t.s_low / (double)r.c);
     r.x_high = (float)((double)t.s_high / (double)r.c);
@@ -183,12 +184,14 @@ int enqueue_slab(rfi_plan* p, const void* d_vis_slab, int o_first, int n_out_sla
     kp.weight = d_weight;
     kp.stats = d_stats;
     kp.flags = p->d_flags;
-    kp.thr0 = to_device_thr(p->thr[0], p->M);
+    kp.thr0 = to_device_thr(p->thr[0], p->M * p->F);
     kp.n_cells = (int)p->n_cells();
     kp.n_chan = p->n_chan;
     kp.n_baselines = p->n_baselines;
     kp.wpb = p->wpb();
     kp.M = p->M;
+    kp.F = p->F;
+    kp.inv_W = (float)(1.0 / ((double)p->M * p->F));
     kp.n_int = p->n_int;
     kp.wpo = p->n_int / p->M;
     kp.n_out_slab = n_out_slab;
@@ -216,7 +219,7 @@ int enqueue_slab(rfi_plan* p, const void* d_vis_slab, int o_first, int n_out_sla
             memset(&bt, 0, sizeof(bt));
             kp.k_first = k0;
             kp.K = p->K - k0 < rfi::kMaxBatch ? p->K - k0 : rfi::kMaxBatch;
-            for (int k = 0; k < kp.K; ++k) bt.t[k] = to_device_thr(p->thr[k0 + k], p->M);
+            for (int k = 0; k < kp.K; ++k) bt.t[k] = to_device_thr(p->thr[k0 + k], p->M * p->F);
             const int rc = use_tma ? launch_batched_tma(fp16, kp, bt, map, R, p->sm_count, p->smem_optin, st)
                                    : launch_batched(fp16, kp, bt, st);
             if (rc != RFI_OK) return rc;
@@ -289,6 +292,13 @@ int rfi_plan_set_integration(rfi_plan* p, int n_int) {
     if (!p || n_int < 1) return RFI_EINVAL;
     if (p->n_time % n_int != 0 || n_int % p->M != 0) return RFI_EINVAL;
     p->n_int = n_int;
+    p->have_result = false;
+    return RFI_OK;
+}
+
+int rfi_plan_set_window_freq(rfi_plan* p, int F) {
+    if (!p || F < 1 || F > 32 || (F & (F - 1)) != 0 || p->n_chan % F != 0) return RFI_EINVAL;
+    p->F = F;
     p->have_result = false;
     return RFI_OK;
 }

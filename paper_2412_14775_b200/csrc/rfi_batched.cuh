@@ -38,7 +38,7 @@ rfi_batched_kernel(const KParams p, const __grid_constant__ BatchThr bt) {
     const int tile = unit - o_local * n_tiles;
     const int o_global = p.o_first + o_local;
     const LaneGeom g = lane_geom(p, tile, lane);
-    const float inv_M = 1.0f / (float)p.M;
+    const float inv_M = p.inv_W;                             // 1/W, W = T*F
     const size_t row_stride = (size_t)p.n_cells * SAMPLE_BYTES;
     const size_t blk_stride = row_stride * R;
     const size_t win_jump = blk_stride + (size_t)(NW - 1) * p.M * row_stride;   // last block of a window -> first block of window + NW
@@ -89,6 +89,7 @@ rfi_batched_kernel(const KParams p, const __grid_constant__ BatchThr bt) {
                 if (blk & 1) step(B, A); else step(A, B);
             }
             float x, r_re, r_im;
+            if (p.F > 1) combine_group(w, p.F, p.M);
             window_stats(w, inv_M, x, r_re, r_im);
             float (*my)[32] = rec[buf][warp];
             my[0][lane] = x;

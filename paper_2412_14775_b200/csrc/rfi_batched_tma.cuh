@@ -99,7 +99,7 @@ rfi_batched_tma_kernel(const __grid_constant__ CUtensorMap tmap, const KParams p
     const int n_rounds = (p.wpo + NW - 1) / NW;
     const int my_n = warp < p.wpo ? (p.wpo - 1 - warp) / NW + 1 : 0;     // windows of a unit streamed by this warp
     const int total = my_units * my_n * bpw;                  // stages this warp consumes in its lifetime
-    const float inv_M = 1.0f / (float)p.M;
+    const float inv_M = p.inv_W;                             // 1/W, W = T*F
     const size_t flag_words_per_win = (size_t)p.n_baselines * p.wpb;
 
     if (lane == 0) {
@@ -192,7 +192,8 @@ rfi_batched_tma_kernel(const __grid_constant__ CUtensorMap tmap, const KParams p
                     if (++stage == stages) { stage = 0; parity ^= 1u; }
                 }
                 float x, r_re, r_im;
-                window_stats(w, inv_M, x, r_re, r_im);
+                if (p.F > 1) combine_group(w, p.F, p.M);
+            window_stats(w, inv_M, x, r_re, r_im);
                 const uint32_t ra = rbuf + ((uint32_t)warp * 32u + lane) * kRecBytes;
                 sts128(ra, x, max_nan(r_re, r_im), 0.f, 0.f);
                 const bool fin = finite2(w.s[0]) && finite2(w.s[1]) && finite2(w.s[2]) && finite2(w.s[3]);

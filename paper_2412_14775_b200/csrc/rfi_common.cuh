@@ -45,7 +45,9 @@ struct KParams {
     uint32_t* flags;          // [K][n_win_total][n_baselines*wpb]
     Thr thr0;                 // set 0 (single-set kernels; stats use its c)
     int n_cells, n_chan, n_baselines, wpb;
-    int M, n_int, wpo;        // window, samples per output, windows per output
+    int M, n_int, wpo;        // window length in time (T), samples per output, windows per output
+    int F;                    // window extent in frequency: F adjacent channels (lanes), power of two <= 32
+    float inv_W;              // 1 / (T * F), W of Eq.(4) and Eq.(9)
     int n_out_slab;           // outputs contained in this slab
     int o_first;              // global index of the slab's first output
     int n_out_total, n_win_total;

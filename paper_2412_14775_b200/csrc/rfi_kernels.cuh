@@ -34,7 +34,7 @@ __global__ void __launch_bounds__(128, 4) rfi_direct_kernel(const KParams p) {
     const int o_local = unit / n_tiles;
     const int tile = unit - o_local * n_tiles;
     const LaneGeom g = lane_geom(p, tile, lane);
-    const float inv_M = 1.0f / (float)p.M;
+    const float inv_M = p.inv_W;                             // 1/W, W = T*F
     const size_t row_stride = (size_t)p.n_cells * SAMPLE_BYTES;
     const size_t blk_stride = row_stride * R;
     const uint8_t* ptr = static_cast<const uint8_t*>(p.vis) + (size_t)o_local * p.n_int * row_stride
@@ -145,7 +145,7 @@ __global__ void __launch_bounds__(512, 1) rfi_tma_kernel(const __grid_constant__
     const int bpu = p.n_int / R;                              // blocks (stages) per unit
     const int total = my_units * bpu;
     const int bpw = p.M / R;
-    const float inv_M = 1.0f / (float)p.M;
+    const float inv_M = p.inv_W;                             // 1/W, W = T*F
 
     if (lane == 0) {
         for (int s = 0; s < stages; ++s) mbar_init(bars + 8 * s, 1);

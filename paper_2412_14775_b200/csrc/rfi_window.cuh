@@ -91,6 +91,28 @@ __device__ __forceinline__ float sqrt_refined(float s) {
     return fmaf(fmaf(-r0, r0, s), 0.5f * y0, r0);
 }
 
+// T x F footprints (W = T * F): the F channels of a window are F adjacent lanes (F a power of two,
+// groups lane-aligned because n_chan % F == 0 and F | 32).  Each lane arrives with the moments of its own T
+// samples; a butterfly over the group merges them (equal counts: mean = (a+b)/2, m2 = m2a + m2b + delta^2 n/2)
+// and adds the unit-vector sums.  Every operation is symmetric in the two partners, so all lanes of a group end
+// with bit-identical statistics and hence the same flag.  The per-channel sample sums w.s stay per lane.
+__device__ __forceinline__ f2 shfl_xor_f2(f2 v, int m) {
+    return (f2)__shfl_xor_sync(0xffffffffu, (unsigned long long)v, m);
+}
+__device__ __forceinline__ void combine_group(Win& w, int F, int T) {
+    float n = (float)T;                                       // samples behind each partner's moments
+    for (int m = 1; m < F; m <<= 1, n += n) {
+        const float mean_o = __shfl_xor_sync(0xffffffffu, w.mean, m);
+        const float m2_o = __shfl_xor_sync(0xffffffffu, w.m2, m);
+        const float delta = mean_o - w.mean;
+        w.m2 = fmaf(delta * delta, 0.5f * n, w.m2 + m2_o);
+        w.mean = 0.5f * (w.mean + mean_o);
+        w.q = add2(w.q, shfl_xor_f2(w.q, m));
+        w.u = add2(w.u, shfl_xor_f2(w.u, m));
+        w.v = add2(w.v, shfl_xor_f2(w.v, m));
+    }
+}
+
 // Window tail: Eq.(4) in centred form and Eq.(9).  x = W*S2/S1^2 - 1 = m2/(W mean^2); tau = c * x.
 __device__ __forceinline__ void window_stats(const Win& w, float inv_M, float& x, float& r_re, float& r_im) {
     // all-zero window: S1 = 0 -> x = -1 (the eps -> 0 limit of Table 1 row 7).  (m2/mean)/(W mean) keeps the
@@ -180,10 +202,11 @@ __device__ __forceinline__ void store_output(const KParams& p, const LaneGeom& g
 
 // Single-set window tail shared by the streaming kernels: statistics, decision, flag word, statistics planes,
 // masked accumulation into the output integration.
-__device__ __forceinline__ void finish_window(const KParams& p, const LaneGeom& g, const Win& w, float inv_M,
+__device__ __forceinline__ void finish_window(const KParams& p, const LaneGeom& g, Win& w, float inv_W,
                                               int w_global, f2 (&acc)[4], uint32_t& wt) {
     float x, r_re, r_im;
-    window_stats(w, inv_M, x, r_re, r_im);
+    if (p.F > 1) combine_group(w, p.F, p.M);
+    window_stats(w, inv_W, x, r_re, r_im);
     const bool flag = decide(x, max_nan(r_re, r_im), p.thr0);
     store_flags(p, g, p.k_first, w_global, flag);
     store_stats(p, g, w_global, p.thr0.c * x, r_re, r_im);

@@ -32,6 +32,7 @@ class Workload:
     window_M: int
     n_int: int
     fp16: bool = False
+    window_F: int = 1           # window extent in frequency (channels): footprint T x F, W = window_M * window_F
     channel_gain: bool = False  # per-channel gain U[0.8,1.2]
     # RFI recipe
     burst_cell_frac: float = 0.0    # fraction of cells carrying random low-duty-cycle polarised bursts

@@ -19,7 +19,8 @@ from oracle import rfi_oracle as orc
 
 
 def near_threshold(tau, r_re, r_im, thr, M, tol):
-    """bool mask of windows whose statistic is within `tol` (relative, floored) of one of its thresholds."""
+    """bool mask of windows whose statistic is within `tol` (relative, floored) of one of its thresholds.
+    M is the window size W (= T*F for T x F footprints)."""
     d, s_low, s_high, gamma = thr
     c = (M * d + 1) / (M - 1)
     near = np.zeros(tau.shape, bool)
@@ -32,13 +33,14 @@ def near_threshold(tau, r_re, r_im, thr, M, tol):
     return near
 
 
-def compare(vis_np, M, n_int, thresholds, gpu, tol=1e-5, fp16=False, oracle_threads=0):
+def compare(vis_np, M, n_int, thresholds, gpu, tol=1e-5, fp16=False, oracle_threads=0, F=1):
     """gpu: dict with numpy arrays avg [K,O,cells,4] complex, weight [K,O,cells], flags [K,W,cells] bool,
     optional tau/r_re/r_im [W,cells] (tau for set 0).  Returns a report dict; raises AssertionError on failure."""
     thresholds = np.asarray(thresholds, np.float64).reshape(-1, 4)
     # the kernel receives the thresholds as float32: the oracle must decide on the same numbers
     thr32 = thresholds.astype(np.float32).astype(np.float64)
-    res = orc.process(vis_np, M, n_int, thr32, n_threads=oracle_threads)
+    res = orc.process(vis_np, M, n_int, thr32, n_threads=oracle_threads, F=F)
+    W = M * F                                            # window size of Eq.(4), Eq.(9)
     K, n_win, n_cells = res.flags.shape
     n_out = res.weight.shape[1]
     wpo = n_int // M
@@ -56,16 +58,16 @@ def compare(vis_np, M, n_int, thresholds, gpu, tol=1e-5, fp16=False, oracle_thre
 
     if gpu.get("tau") is not None:
         d0 = thr32[0, 0]
-        c0 = (M * d0 + 1) / (M - 1)
+        c0 = (W * d0 + 1) / (W - 1)
         check_stat("tau", gpu["tau"], res.tau[0], 0.01 * c0)
-        check_stat("r_re", gpu["r_re"], res.r_re, 1 / math.sqrt(M))
-        check_stat("r_im", gpu["r_im"], res.r_im, 1 / math.sqrt(M))
+        check_stat("r_re", gpu["r_re"], res.r_re, 1 / math.sqrt(W))
+        check_stat("r_im", gpu["r_im"], res.r_im, 1 / math.sqrt(W))
 
     n_mismatch, n_exempt, n_unexplained = 0, 0, 0
     avg_worst, avg_rel_worst = 0.0, 0.0
     for k in range(K):
         mism = gpu["flags"][k] != res.flags[k].astype(bool)
-        near = near_threshold(res.tau[k], res.r_re, res.r_im, thr32[k], M, tol if not fp16 else 0.0)
+        near = near_threshold(res.tau[k], res.r_re, res.r_im, thr32[k], W, tol if not fp16 else 0.0)
         n_mismatch += int(mism.sum())
         n_exempt += int((mism & near).sum())
         n_unexplained += int((mism & ~near).sum())

@@ -85,6 +85,17 @@ def test_integration_and_threshold_validation():
     p.destroy()
 
 
+def test_window_freq_validation():
+    plan = rfi.RfiPlan(4, 10, 24, 40, 10)
+    for F in (1, 2, 4, 8):
+        plan.set_window_freq(F)
+    for F in (0, 3, 16, 64, -2):                   # not a power of two / does not divide 24 channels / too wide
+        with pytest.raises(rfi.RfiError) as e:
+            plan.set_window_freq(F)
+        assert e.value.code == -1
+    plan.destroy()
+
+
 def test_baseline_shard_validation():
     plan = rfi.RfiPlan(48, 1176, 64, 7680, 16)
     plan.set_baseline_shard(588, 588)

@@ -17,6 +17,8 @@ INF = float("inf")
 def run_gpu(w, vis, thresholds, variant="auto", stats=True):
     plan = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M,
                        rfi.RFI_FP16 if w.fp16 else rfi.RFI_FP32, n_int=w.n_int)
+    if w.window_F > 1:
+        plan.set_window_freq(w.window_F)
     plan.set_thresholds(thresholds)
     plan.set_variant(variant)
     avg, weight, st = plan.alloc_outputs(stats=stats)
@@ -41,7 +43,8 @@ def check(w, thresholds, variant, seed=1234, tol=None, mutate=None):
     if variant != "auto":
         assert used == variant
     v = vis.numpy().reshape(w.n_time, w.n_cells, 4, 2)
-    rep = compare(v, w.window_M, w.n_int, thresholds, out, tol=tol or (2e-3 if w.fp16 else 1e-5), fp16=w.fp16)
+    rep = compare(v, w.window_M, w.n_int, thresholds, out, tol=tol or (2e-3 if w.fp16 else 1e-5), fp16=w.fp16,
+                  F=w.window_F)
     return rep, out, truth
 
 
@@ -254,3 +257,30 @@ def test_batched_fp16_and_host_path():
     plan.destroy()
     for key in ("avg", "weight", "flags", "tau", "r_re", "r_im"):
         np.testing.assert_array_equal(out[key], host[key])
+
+
+# ------------------------------------------------------------------------------------------------------
+# T x F window footprints (the paper's 10 x 2 and 5 x 4, W = 20)
+# ------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("variant", ["direct", "tma"])
+@pytest.mark.parametrize("T,F,n_chan", [(10, 2, 64), (5, 4, 64), (16, 2, 20), (4, 8, 24), (2, 32, 64), (8, 16, 48)])
+def test_tf_footprints(variant, T, F, n_chan):
+    w = synth.Workload("tf", 5, True, n_chan, T * 24, T, T * 6, window_F=F, burst_cell_frac=0.15, channel_gain=True)
+    W = T * F
+    thr = [[0.8, 0.25 * (W * 0.8 + 1) / (W - 1) * 0.4, (W * 0.8 + 1) / (W - 1) * 0.45, 2.2 / math.sqrt(W)]]
+    if variant == "tma" and w.n_cells % 4:
+        pytest.skip("TMA variant needs n_cells % 4 == 0")
+    rep, out, _ = check(w, thr, variant, seed=T * 100 + F)
+    f = out["flags"][0].reshape(w.n_win, w.n_baselines, n_chan // F, F)
+    assert (f == f[..., :1]).all()                        # one flag per footprint
+    assert 0.0 < f.mean() < 0.9
+
+
+@pytest.mark.parametrize("fp16", [False, True])
+def test_tf_footprints_batched(fp16):
+    w = synth.Workload("tf_k", 5, True, 64, 10 * 32, 10, 10 * 16, fp16=fp16, window_F=2, burst_cell_frac=0.15)
+    thr = synth.sweep_thresholds(20, 9, seed=4)
+    rep, out, _ = check(w, thr, "auto")
+    assert rep["K"] == 9
+    w2 = synth.Workload("tf_k2", 5, False, 12, 5 * 16, 5, 5 * 8, fp16=fp16, window_F=4, burst_cell_frac=0.15)   # ragged: old batched kernel
+    check(w2, synth.sweep_thresholds(20, 5, seed=5), "auto")
