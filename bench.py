@@ -178,10 +178,13 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=dev)
 
     w = synth.WORKLOADS[args.workload]
-    thr = synth.default_thresholds(w.window_M) if args.K <= 1 else synth.sweep_thresholds(w.window_M, args.K)
+    W = w.window_M * w.window_F
+    thr = synth.default_thresholds(W) if args.K <= 1 else synth.sweep_thresholds(W, args.K)
     vis, truth = synth.make_chunk(w, seed=1234 + rank, device=dev)
     plan = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M,
                        rfi.RFI_FP16 if w.fp16 else rfi.RFI_FP32, n_int=w.n_int)
+    if w.window_F > 1:
+        plan.set_window_freq(w.window_F)
     plan.set_thresholds(thr)
     plan.set_variant(args.variant)
     avg, weight, _ = plan.alloc_outputs(device=dev)
@@ -226,6 +229,8 @@ def run_ours(args):
     # a little science on the way out (not timed): detection quality against the injected ground truth
     flags = rfi.unpack_flags(plan.get_flags(), w.n_chan).reshape(max(plan.K, 1), plan.n_win, plan.n_cells)
     tr = truth.reshape(plan.n_win, plan.n_cells)
+    if w.window_F > 1:                 # a footprint is RFI-bearing if any of its F channels is
+        tr = tr.reshape(plan.n_win, -1, w.window_F).any(-1, keepdim=True).expand(-1, -1, w.window_F).reshape(plan.n_win, plan.n_cells)
     fa = float((flags[0] & ~tr).sum() / max((~tr).sum(), 1))
     md = float((~flags[0] & tr).sum() / max(tr.sum(), 1))
 
@@ -286,9 +291,10 @@ def run_ours(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32" if not w.fp16 else "f32 (f16 storage)", "data": "synthetic (seeded; stands in for LOFAR data)",
-        "config": {"workload": f"{w.name}: BASELINE.json configs[{list(synth.WORKLOADS).index(w.name)}]",
+        "config": {"workload": (f"{w.name}: BASELINE.json configs[{synth.BASELINE_CONFIG_INDEX[w.name]}]"
+                                if w.name in synth.BASELINE_CONFIG_INDEX else f"{w.name}: SURVEY 8(f) NEXT-1, not a BASELINE.json config"),
                    "n_stations": w.n_stations, "n_baselines": w.n_baselines, "n_chan": w.n_chan, "n_time": w.n_time,
-                   "window_M": w.window_M, "n_int": w.n_int, "K": max(plan.K, 1), "variant": variant,
+                   "window_M": w.window_M, "window_F": w.window_F, "n_int": w.n_int, "K": max(plan.K, 1), "variant": variant,
                    "input_bytes": w.input_bytes, "l2": "input (>= 9 GB) is far larger than the 126 MB L2: no flush needed",
                    "sharding": "by baseline, no collective" if world > 1 else "single GPU"},
         "gbytes_per_s": world * algo_bytes / (ms_per_step * 1e-3) / 1e9,

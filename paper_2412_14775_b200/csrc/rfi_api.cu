@@ -206,8 +206,9 @@ int enqueue_slab(rfi_plan* p, const void* d_vis_slab, int o_first, int n_out_sla
     if (p->K > 1) {
         // batched-threshold mode: all sets in one pass over the data, 64 sets per launch
         p->last_variant = RFI_VARIANT_BATCHED;
-        // same block length as the single-set direct kernel, so K sets equal K single-set runs bit for bit
-        const int R = pick_rows(p->M, fp16);
+        // same block length as the single-set direct kernel whenever that one uses R <= 4 (fp32) / 8 (fp16): then
+        // K sets equal K single-set runs bit for bit
+        const int R = pick_rows(p->M, fp16, fp16 ? 8 : 4);
         const CUtensorMap* map = nullptr;
         const bool use_tma = batched_tma_supported(fp16, kp, R) && tma_allowed(p);
         if (use_tma) {

@@ -33,14 +33,26 @@ inline int largest_divisor_le(int M, int cap) {
     return 1;
 }
 
-// Rows merged per block by the register-staged kernels (direct and batched): the largest divisor of the
-// window length that keeps 128 B per thread in flight (4 rows fp32, 8 rows fp16); RFI_DIRECT_ROWS lowers the cap.
-inline int pick_rows(int M, bool fp16) {
-    const int max_r = fp16 ? 8 : 4;
-    int cap = env_int("RFI_DIRECT_ROWS", max_r);
-    if (cap < 1) cap = 1;
-    if (cap > max_r) cap = max_r;
-    return largest_divisor_le(M, cap);
+// Rows merged per block by the register-staged kernels (direct and batched): a divisor of the window length T.
+// fp16: the largest divisor <= 8 (16 B rows, 4 CTAs of 4 warps per SM).  fp32: rows are 32 B = 8 registers per
+// buffered row, so R <= 4 runs 4 CTAs/SM (16 warps), R = 5 three (12 warps), R = 6..8 two (8 warps); pick the divisor
+// with the most bytes in flight per SM, R * warps(R), smaller R on ties.  T = 16 -> 4, T = 10 -> 5, T = 5 -> 5,
+// T = 7 -> 7, T = 6 -> 3.  `cap` bounds R (the batched kernels are instantiated up to 4 / 8 only);
+// RFI_DIRECT_ROWS lowers it further.
+inline int direct_warps_per_sm(int R, bool fp16) { return (fp16 || R <= 4) ? 16 : (R == 5 ? 12 : 8); }
+inline int pick_rows(int M, bool fp16, int cap = 8) {
+    const int max_r = fp16 ? 8 : 8;
+    int lim = env_int("RFI_DIRECT_ROWS", max_r);
+    if (lim < 1) lim = 1;
+    if (lim > max_r) lim = max_r;
+    if (lim > cap) lim = cap;
+    int best = 1, best_score = 0;
+    for (int r = 1; r <= lim; ++r) {
+        if (M % r) continue;
+        const int score = r * direct_warps_per_sm(r, fp16);
+        if (score > best_score) { best = r; best_score = score; }
+    }
+    return best;
 }
 
 // Each returns RFI_OK or RFI_ECUDA / RFI_EINVAL; all only enqueue work on `st`.

@@ -25,7 +25,7 @@ __device__ __forceinline__ void load_block(const uint8_t* ptr, size_t row_stride
 }
 
 template <int R, bool FP16, bool ALIGN32>
-__global__ void __launch_bounds__(128, 4) rfi_direct_kernel(const KParams p) {
+__global__ void __launch_bounds__(128, (FP16 || R <= 4) ? 4 : (R == 5 ? 3 : 2)) rfi_direct_kernel(const KParams p) {
     constexpr int SAMPLE_BYTES = FP16 ? 16 : 32;
     const int lane = threadIdx.x & 31;
     const int n_tiles = (p.n_cells + 31) >> 5;

@@ -27,7 +27,7 @@ int launch_r(const rfi::KParams& kp, const rfi::BatchThr& bt, cudaStream_t st) {
 
 int launch_batched(bool fp16, const rfi::KParams& kp, const rfi::BatchThr& bt, cudaStream_t st) {
     if (kp.K < 1 || kp.K > rfi::kMaxBatch) return RFI_EINVAL;
-    const int R = pick_rows(kp.M, fp16);
+    const int R = pick_rows(kp.M, fp16, fp16 ? 8 : 4);
     if (!fp16) {
         switch (R) {
             case 1: return launch_r<1, false>(kp, bt, st);

@@ -27,7 +27,11 @@ int launch_direct(bool fp16, const rfi::KParams& kp, cudaStream_t st) {
             case 1: return launch_r<1, false>(kp, st);
             case 2: return launch_r<2, false>(kp, st);
             case 3: return launch_r<3, false>(kp, st);
-            default: return launch_r<4, false>(kp, st);
+            case 4: return launch_r<4, false>(kp, st);
+            case 5: return launch_r<5, false>(kp, st);
+            case 6: return launch_r<6, false>(kp, st);
+            case 7: return launch_r<7, false>(kp, st);
+            default: return launch_r<8, false>(kp, st);
         }
     }
     switch (R) {

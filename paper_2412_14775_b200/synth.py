@@ -79,7 +79,12 @@ WORKLOADS = {
                            burst_cell_frac=0.02, tone_chan_frac=0.01),
     "large": Workload("large", 76, True, 256, 3072, 32, 3072, channel_gain=True, mixed_cell_frac=0.03),
     "sweep": Workload("sweep", 48, True, 64, 7680, 16, 768, channel_gain=True, burst_cell_frac=0.02),
+    # the paper's own footprints, W = 20 as 10 x 2 and 5 x 4, on the LOFAR-subband shape;
+    # 760 samples per integration so that T = 10 and T = 5 divide it (not BASELINE.json configs: SURVEY 8(f) NEXT-1)
+    "lofar_tf10x2": Workload("lofar_tf10x2", 48, True, 64, 7600, 10, 760, window_F=2, channel_gain=True, burst_cell_frac=0.02),
+    "lofar_tf5x4": Workload("lofar_tf5x4", 48, True, 64, 7600, 5, 760, window_F=4, channel_gain=True, burst_cell_frac=0.02),
 }
+BASELINE_CONFIG_INDEX = {"tiny": 0, "lofar": 1, "lofar_fp16": 2, "large": 3, "sweep": 4}
 
 
 def auto_baseline_mask(w: Workload, device="cpu") -> torch.Tensor:
@@ -259,7 +264,7 @@ def _quantiles(M: int):
     return xq, rq
 
 
-def default_thresholds(M: int, d: float = 1.0):
+def default_thresholds(M: int, d: float = 1.0):  # M = window size W (T*F for footprints)
     """One (d, s_low, s_high, gamma) set near the 1 % / 99 % null quantiles."""
     xq, rq = _quantiles(M)
     c = (M * d + 1) / (M - 1)
