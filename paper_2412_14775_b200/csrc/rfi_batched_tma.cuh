@@ -101,6 +101,7 @@ rfi_batched_tma_kernel(const __grid_constant__ CUtensorMap tmap, const KParams p
     const int total = my_units * my_n * bpw;                  // stages this warp consumes in its lifetime
     const float inv_M = p.inv_W;                             // 1/W, W = T*F
     const size_t flag_words_per_win = (size_t)p.n_baselines * p.wpb;
+    const size_t flag_set_stride = (size_t)p.n_win_total * flag_words_per_win;
 
     if (lane == 0) {
         for (int s = 0; s < stages; ++s) mbar_init(bars + 8 * s, 1);
@@ -163,6 +164,9 @@ rfi_batched_tma_kernel(const __grid_constant__ CUtensorMap tmap, const KParams p
         g.valid = true;
         g.word = tile; g.bit = lane; g.group = 0xffffffffu; g.leader = lane == 0;
 
+        // this lane's flag word of set warp*SPW, window (round 0, lane): later sets / rounds are fixed strides away
+        uint32_t* const flag_ptr = p.flags + ((size_t)(p.k_first + warp * SPW) * p.n_win_total
+                                              + (size_t)o_global * p.wpo + lane) * flag_words_per_win + tile;
         f2 acc[SPW][4];
         float cnt[SPW];
 #pragma unroll
@@ -228,13 +232,10 @@ rfi_batched_tma_kernel(const __grid_constant__ CUtensorMap tmap, const KParams p
                 }
             }
             if (lane < n_w) {
-                const size_t w_global = (size_t)o_global * p.wpo + round * NW + lane;
+                uint32_t* fp = flag_ptr + (size_t)round * NW * flag_words_per_win;
 #pragma unroll
-                for (int i = 0; i < SPW; ++i) {
-                    const int k = warp * SPW + i;
-                    if (k < p.K)
-                        p.flags[((size_t)(p.k_first + k) * p.n_win_total + w_global) * flag_words_per_win + tile] = myw[i];
-                }
+                for (int i = 0; i < SPW; ++i, fp += flag_set_stride)
+                    if (warp * SPW + i < p.K) *fp = myw[i];
             }
         }
 #pragma unroll

@@ -188,9 +188,9 @@ __device__ __forceinline__ void store_output(const KParams& p, const LaneGeom& g
     for (int i = 0; i < 4; ++i) unpack2(acc[i], a[2 * i], a[2 * i + 1]);
     float4 lo, hi;
     if (wt) {
-        const float fw = (float)wt;
-        lo = make_float4(a[0] / fw, a[1] / fw, a[2] / fw, a[3] / fw);
-        hi = make_float4(a[4] / fw, a[5] / fw, a[6] / fw, a[7] / fw);
+        const float iw = 1.0f / (float)wt;                      // one IEEE division, then 8 multiplies (<= 1.5 ulp)
+        lo = make_float4(a[0] * iw, a[1] * iw, a[2] * iw, a[3] * iw);
+        hi = make_float4(a[4] * iw, a[5] * iw, a[6] * iw, a[7] * iw);
     } else {
         lo = hi = make_float4(0.f, 0.f, 0.f, 0.f);
     }
