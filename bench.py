@@ -102,18 +102,21 @@ class ClockSampler:
 
 def oracle_baseline(vis_np, w, thr, target_cpu_seconds=15.0):
     """Time the fp64 oracle, as it stands, on a bounded sample of the workload (all host cores)."""
+    import numpy as np
     from oracle import rfi_oracle as orc
     cores = orc.max_threads()
     n_cells = vis_np.shape[1]
     probe = min(n_cells, 1024)
-    orc.process(vis_np[:, :probe], w.window_M, w.n_int, thr, n_threads=cores, want_stats=False)   # warm-up: threads, pages
+    first = np.ascontiguousarray(vis_np[:, :probe])
+    orc.process(first, w.window_M, w.n_int, thr, n_threads=cores, want_stats=False)   # warm-up: threads, pages
     t0 = time.perf_counter()
-    orc.process(vis_np[:, :probe], w.window_M, w.n_int, thr, n_threads=cores, want_stats=False)
+    orc.process(first, w.window_M, w.n_int, thr, n_threads=cores, want_stats=False)
     dt = max(time.perf_counter() - t0, 1e-4)
     per_cell_cpu = dt * cores / probe                       # CPU-seconds per cell
     use = int(max(probe, min(n_cells, target_cpu_seconds / per_cell_cpu)))
+    sample = np.ascontiguousarray(vis_np[:, :use])          # the oracle's input, resident and contiguous before timing
     t0 = time.perf_counter()
-    orc.process(vis_np[:, :use], w.window_M, w.n_int, thr, n_threads=cores, want_stats=False)
+    orc.process(sample, w.window_M, w.n_int, thr, n_threads=cores, want_stats=False)
     dt = time.perf_counter() - t0
     samples = use * vis_np.shape[0]
     return {"value": samples / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
