@@ -16,6 +16,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "rfi_oracle.cpp")
+_SRC_TABLES = os.path.join(_HERE, "rfi_oracle_tables.cpp")
 _LIB = os.path.join(_HERE, "liboracle_rfi.so")
 _lib = None
 
@@ -25,11 +26,11 @@ _STORAGE = {np.dtype(np.float32): 0, np.dtype(np.float16): 1, np.dtype(np.float6
 def build(force: bool = False) -> str:
     """Compile oracle/rfi_oracle.cpp -> oracle/liboracle_rfi.so (g++ -O2 -fopenmp)."""
     if (not force and os.path.exists(_LIB)
-            and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC)):
+            and os.path.getmtime(_LIB) >= max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_TABLES))):
         return _LIB
     tmp = _LIB + f".tmp{os.getpid()}"
     cmd = ["g++", "-O2", "-std=c++17", "-fopenmp", "-fPIC", "-shared",
-           "-ffp-contract=off", "-o", tmp, _SRC]
+           "-ffp-contract=off", "-o", tmp, _SRC, _SRC_TABLES]
     subprocess.run(cmd, check=True)
     os.replace(tmp, _LIB)
     return _LIB
@@ -57,6 +58,18 @@ def _load():
         lib.oracle_rfi_pack_flags.argtypes = [ctypes.c_void_p, ctypes.c_int64, ctypes.c_int64,
                                               ctypes.c_int64, ctypes.c_void_p]
         lib.oracle_rfi_pack_flags.restype = ctypes.c_int
+        c_fp = ctypes.POINTER(ctypes.c_float)
+        cf, cu = ctypes.c_float, ctypes.c_uint32
+        lib.oracle_tables_sk.argtypes = [c_fp, c_fp, ctypes.c_int, cf, cf, cf, cu, c_fp]
+        lib.oracle_tables_sk.restype = ctypes.c_int
+        lib.oracle_tables_ds.argtypes = [c_fp, c_fp, c_fp, ctypes.c_int, cf, cu, c_fp]
+        lib.oracle_tables_ds.restype = ctypes.c_int
+        lib.oracle_tables_process.argtypes = [
+            ctypes.c_void_p, ctypes.c_int64, ctypes.c_int64, ctypes.c_int, ctypes.c_int64, cf, cf, cf, cf, cu,
+            ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, c_dp, ctypes.c_void_p, ctypes.c_int]
+        lib.oracle_tables_process.restype = ctypes.c_int
+        lib.oracle_tables_to_half.argtypes = [cf]
+        lib.oracle_tables_to_half.restype = cf
         lib.oracle_rfi_max_threads.argtypes = []
         lib.oracle_rfi_max_threads.restype = ctypes.c_int
         _lib = lib
@@ -150,3 +163,47 @@ def pack_flags(flags, n_baselines: int, n_chan: int) -> np.ndarray:
 
 def max_threads() -> int:
     return _load().oracle_rfi_max_threads()
+
+
+# ---- paper-literal mixed-precision arithmetic (Tables 1-2, oracle/rfi_oracle_tables.cpp) -----------------------
+def _fp(a):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_float))
+
+
+def tables_sk(xr, xi, d, s_low, s_high, mask):
+    """Table 1 on one window of I = xr + j xi (float32).  Returns (tau, flag)."""
+    xr = np.ascontiguousarray(xr, np.float32); xi = np.ascontiguousarray(xi, np.float32)
+    t = ctypes.c_float()
+    f = _load().oracle_tables_sk(_fp(xr), _fp(xi), len(xr), d, s_low, s_high, int(mask), ctypes.byref(t))
+    return t.value, f
+
+
+def tables_ds(q, u, v, gamma, mask):
+    """Table 2 on one window of real (or imaginary) parts q, u, v (float32).  Returns (r, flag)."""
+    q = np.ascontiguousarray(q, np.float32); u = np.ascontiguousarray(u, np.float32); v = np.ascontiguousarray(v, np.float32)
+    r = ctypes.c_float()
+    f = _load().oracle_tables_ds(_fp(q), _fp(u), _fp(v), len(q), gamma, int(mask), ctypes.byref(r))
+    return r.value, f
+
+
+def to_half(x: float) -> float:
+    return _load().oracle_tables_to_half(float(x))
+
+
+def tables_process(vis, M: int, n_int: int, threshold, mask: int, n_threads: int = 0) -> OracleResult:
+    """The whole path in the tables' arithmetic.  vis float32 [n_time, n_cells, 4, 2]; threshold (d, s_low, s_high, gamma)."""
+    a = np.ascontiguousarray(vis, np.float32)
+    n_time, n_cells = a.shape[0], a.shape[1]
+    assert a.shape[2:] == (4, 2), a.shape
+    n_win, n_out = n_time // M, n_time // n_int
+    tau = np.empty((n_win, n_cells), np.float32); r_re = np.empty_like(tau); r_im = np.empty_like(tau)
+    flags = np.empty((n_win, n_cells), np.uint8)
+    avg = np.empty((n_out, n_cells, 8), np.float64)
+    weight = np.empty((n_out, n_cells), np.int64)
+    d, lo, hi, g = [float(np.float32(x)) for x in threshold]
+    rc = _load().oracle_tables_process(a.ctypes.data, n_time, n_cells, int(M), int(n_int), d, lo, hi, g, int(mask),
+                                       tau.ctypes.data, r_re.ctypes.data, r_im.ctypes.data, flags.ctypes.data,
+                                       _dp(avg), weight.ctypes.data, int(n_threads))
+    if rc != 0:
+        raise ValueError("oracle_tables_process: invalid arguments")
+    return OracleResult(tau[None], r_re, r_im, flags[None], avg.view(np.complex128).reshape(1, n_out, n_cells, 4), weight[None])
