@@ -68,7 +68,14 @@ enum {
     RFI_VARIANT_AUTO   = 0,   /* the fastest measured variant for the shape (currently: direct) */
     RFI_VARIANT_DIRECT = 1,   /* per-thread 256-bit (fp32) / 128-bit (fp16) streaming loads, register double buffer */
     RFI_VARIANT_TMA    = 2,   /* warp-private TMA (cp.async.bulk.tensor) ring in shared memory */
-    RFI_VARIANT_BATCHED = 3   /* reported by rfi_plan_last_variant when K > 1 (not selectable: K decides) */
+    RFI_VARIANT_BATCHED = 3,  /* reported by rfi_plan_last_variant when K > 1 (not selectable: K decides) */
+    RFI_VARIANT_TABLES = 4    /* reported when the arithmetic mode is RFI_ARITH_TABLES */
+};
+
+/* arithmetic modes (rfi_plan_set_arithmetic) */
+enum {
+    RFI_ARITH_FAST   = 0,     /* default: all-single reformulation (centred SK moment, exact-zero guards) */
+    RFI_ARITH_TABLES = 1      /* the paper's Tables 1-2 step by step, each group in single or half precision */
 };
 
 /* One threshold set: d of Eq.(4), s_low/s_high of Eq.(5), gamma of Eq.(10)
@@ -95,6 +102,18 @@ int rfi_plan_set_integration(rfi_plan *plan, int n_int);
  * buffer layouts are unchanged (the F channels of a footprint carry the same statistics and flag bit).
  * RFI_EINVAL unless F is a power of two, F <= 32 and n_chan % F == 0. */
 int rfi_plan_set_window_freq(rfi_plan *plan, int F);
+
+/* Arithmetic mode.  RFI_ARITH_TABLES runs the paper's operation tables literally (Table 1, PAPER.md:131-143:
+ * y = xr^2+xi^2, z = sqrt(y), s1 = sum z, s2 = sum y, tau = (Wd+1)/(W-1), s12 = s1^2, tau = tau (W s2/(s12+eps) - 1)
+ * [Eq.(4) brackets], compare; Table 2: a,b,c = q^2,u^2,v^2, p = sqrt(a+b+c)+eps, q/p,u/p,v/p,
+ * sums, squares, r = sqrt(q+u+v)/W, compare; once on the real and once on the imaginary parts), every operation an
+ * IEEE round-to-nearest operation in the precision of its group: bit g-1 of mask14 (g = 1..7) puts Table 1 group g
+ * in half precision, bit 7+g-1 Table 2 group g; eps = machine epsilon of the group's format
+ * (PAPER.md:131); operands are converted into the consuming group's format.  Results are bit-identical to the
+ * step-by-step CPU restatement.  Needs RFI_FP32 storage (the stream is single precision), F = 1 and
+ * K = 1 (else rfi_process_chunk returns RFI_EINVAL).  Half-precision overflow yields a non-finite statistic and
+ * hence a flag.  RFI_ARITH_FAST takes mask14 = 0.  RFI_EINVAL for an unknown mode or mask bits above 13. */
+int rfi_plan_set_arithmetic(rfi_plan *plan, int mode, uint32_t mask14);
 
 /* Multi-GPU sharding (every baseline stream is mitigated separately, so streams partition across
  * devices with no exchange).  Declares that this plan processes only baselines [b_first, b_first + b_count) of the

@@ -17,9 +17,11 @@ from . import build as _build
 RFI_FP32, RFI_FP16 = 0, 1
 VARIANT_AUTO, VARIANT_DIRECT, VARIANT_TMA = 0, 1, 2
 _VARIANTS = {"auto": 0, "direct": 1, "tma": 2}
+ARITH_FAST, ARITH_TABLES = 0, 1
+MASK_PAPER_LEARNED = 0x3C50      # Tables 3-4: Table 1 groups 5,7 and Table 2 groups 4-7 in half
 
 EXPORTS = [
-    "rfi_plan_create", "rfi_plan_set_integration", "rfi_plan_set_baseline_shard", "rfi_plan_set_window_freq", "rfi_set_thresholds", "rfi_plan_set_variant",
+    "rfi_plan_create", "rfi_plan_set_integration", "rfi_plan_set_baseline_shard", "rfi_plan_set_window_freq", "rfi_plan_set_arithmetic", "rfi_set_thresholds", "rfi_plan_set_variant",
     "rfi_process_chunk", "rfi_get_flags", "rfi_process_chunk_host", "rfi_plan_destroy",
     "rfi_strerror", "rfi_last_cuda_error", "rfi_flags_bytes", "rfi_avg_bytes", "rfi_weight_bytes",
     "rfi_stats_bytes", "rfi_vis_bytes", "rfi_plan_launch_count", "rfi_plan_last_variant", "rfi_version",
@@ -63,6 +65,7 @@ def load_library(build_if_missing: bool = True):
     lib.rfi_plan_set_integration.argtypes = [vp, ci]
     lib.rfi_plan_set_baseline_shard.argtypes = [vp, ci, ci]
     lib.rfi_plan_set_window_freq.argtypes = [vp, ci]
+    lib.rfi_plan_set_arithmetic.argtypes = [vp, ci, ctypes.c_uint32]
     lib.rfi_set_thresholds.argtypes = [vp, ci, ctypes.POINTER(RfiThresholds)]
     lib.rfi_plan_set_variant.argtypes = [vp, ci]
     lib.rfi_process_chunk.argtypes = [vp, vp, vp, vp, vp, vp]
@@ -70,7 +73,7 @@ def load_library(build_if_missing: bool = True):
     lib.rfi_process_chunk_host.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.rfi_plan_destroy.argtypes = [vp]
     for name in ("rfi_plan_create", "rfi_plan_set_integration", "rfi_plan_set_baseline_shard",
-                 "rfi_plan_set_window_freq", "rfi_set_thresholds", "rfi_plan_set_variant",
+                 "rfi_plan_set_window_freq", "rfi_plan_set_arithmetic", "rfi_set_thresholds", "rfi_plan_set_variant",
                  "rfi_process_chunk", "rfi_get_flags", "rfi_process_chunk_host", "rfi_plan_destroy",
                  "rfi_plan_last_variant"):
         getattr(lib, name).restype = ci
@@ -132,6 +135,11 @@ class RfiPlan:
         """rfi_plan_set_window_freq: T x F footprints, W = window_M * F."""
         _check(self._lib.rfi_plan_set_window_freq(self._h, F), "rfi_plan_set_window_freq")
         self.window_F = F
+
+    def set_arithmetic(self, mode, mask14: int = 0):
+        """rfi_plan_set_arithmetic: "fast" (default) or "tables" (paper-literal Tables 1-2 with a 14-bit half-precision mask)."""
+        m = {"fast": ARITH_FAST, "tables": ARITH_TABLES}[mode] if isinstance(mode, str) else int(mode)
+        _check(self._lib.rfi_plan_set_arithmetic(self._h, m, mask14), "rfi_plan_set_arithmetic")
 
     def set_baseline_shard(self, b_first: int, b_count: int):
         """rfi_plan_set_baseline_shard: this plan processes baselines [b_first, b_first + b_count) only."""
@@ -206,7 +214,7 @@ class RfiPlan:
     @property
     def last_variant(self) -> str:
         v = self._lib.rfi_plan_last_variant(self._h)
-        return {0: "none", 1: "direct", 2: "tma", 3: "batched"}.get(v, str(v))
+        return {0: "none", 1: "direct", 2: "tma", 3: "batched", 4: "tables"}.get(v, str(v))
 
     def destroy(self):
         if self._h:

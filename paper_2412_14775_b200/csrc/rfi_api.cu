@@ -45,6 +45,8 @@ struct MapEntry {
 
 struct rfi_plan {
     int n_stations, n_baselines, n_chan, n_time, M, precision, n_int;
+    int arith = RFI_ARITH_FAST;               // arithmetic mode
+    uint32_t arith_mask = 0;                  // 14-bit precision mask of the tables mode
     int F = 1;                                // window extent in frequency (channels), W = M * F
     int n_baselines_total = 0, b_first = 0;   // n_baselines is the shard this plan processes (default: all)
     int K = 0;
@@ -203,6 +205,22 @@ int enqueue_slab(rfi_plan* p, const void* d_vis_slab, int o_first, int n_out_sla
     kp.flags_atomic = (p->n_chan % 32 != 0 && 32 % p->n_chan != 0) ? 1 : 0;
 
     const bool fp16 = p->precision == RFI_FP16;
+    if (p->arith == RFI_ARITH_TABLES) {
+        // paper-literal Tables 1-2: single-precision stream, per-channel windows, one threshold set
+        if (fp16 || p->F != 1 || p->K != 1) {
+            snprintf(g_cuda_err, sizeof(g_cuda_err), "tables arithmetic needs RFI_FP32 storage, F = 1 and K = 1");
+            return RFI_EINVAL;
+        }
+        kp.d = p->thr[0].d;
+        kp.s_low = p->thr[0].s_low;
+        kp.s_high = p->thr[0].s_high;
+        kp.thr0.gamma = p->thr[0].gamma;
+        kp.arith_mask = p->arith_mask;
+        p->last_variant = RFI_VARIANT_TABLES;
+        const int rc = launch_tables(kp, st);
+        if (rc == RFI_OK) p->launches++;
+        return rc;
+    }
     if (p->K > 1) {
         // batched-threshold mode: all sets in one pass over the data, 64 sets per launch
         p->last_variant = RFI_VARIANT_BATCHED;
@@ -300,6 +318,15 @@ int rfi_plan_set_integration(rfi_plan* p, int n_int) {
 int rfi_plan_set_window_freq(rfi_plan* p, int F) {
     if (!p || F < 1 || F > 32 || (F & (F - 1)) != 0 || p->n_chan % F != 0) return RFI_EINVAL;
     p->F = F;
+    p->have_result = false;
+    return RFI_OK;
+}
+
+int rfi_plan_set_arithmetic(rfi_plan* p, int mode, uint32_t mask14) {
+    if (!p || (mode != RFI_ARITH_FAST && mode != RFI_ARITH_TABLES) || (mask14 >> 14) != 0) return RFI_EINVAL;
+    if (mode == RFI_ARITH_FAST && mask14 != 0) return RFI_EINVAL;
+    p->arith = mode;
+    p->arith_mask = mask14;
     p->have_result = false;
     return RFI_OK;
 }

@@ -54,6 +54,9 @@ struct KParams {
     int K;                    // sets handled by this launch (batched kernel: <= kMaxBatch)
     int k_first;              // global index of this launch's first set
     int flags_atomic;         // 1: flag words may be shared between warps -> atomicOr into a zeroed buffer
+    // paper-literal tables mode (rfi_tables.cuh) only: raw thresholds of set 0 and the 14-bit precision mask
+    float d, s_low, s_high;
+    uint32_t arith_mask;
 };
 
 struct BatchThr { Thr t[kMaxBatch]; };            // by-value kernel parameter (constant bank), 1 KiB

@@ -85,6 +85,18 @@ def test_integration_and_threshold_validation():
     p.destroy()
 
 
+def test_arithmetic_mode_validation():
+    plan = rfi.RfiPlan(4, 10, 24, 40, 10)
+    plan.set_arithmetic("tables", 0x3C50)
+    plan.set_arithmetic("tables", 0x3FFF)
+    plan.set_arithmetic("fast")
+    for mode, mask in ((1, 1 << 14), (2, 0), (-1, 0), (0, 1)):
+        with pytest.raises(rfi.RfiError) as e:
+            plan.set_arithmetic(mode, mask)
+        assert e.value.code == -1
+    plan.destroy()
+
+
 def test_window_freq_validation():
     plan = rfi.RfiPlan(4, 10, 24, 40, 10)
     for F in (1, 2, 4, 8):
