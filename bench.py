@@ -188,6 +188,8 @@ def run_ours(args):
                        rfi.RFI_FP16 if w.fp16 else rfi.RFI_FP32, n_int=w.n_int)
     if w.window_F > 1:
         plan.set_window_freq(w.window_F)
+    if args.arith == "tables":
+        plan.set_arithmetic("tables", args.mask)
     plan.set_thresholds(thr)
     plan.set_variant(args.variant)
     avg, weight, _ = plan.alloc_outputs(device=dev)
@@ -298,6 +300,7 @@ def run_ours(args):
                                 if w.name in synth.BASELINE_CONFIG_INDEX else f"{w.name}: SURVEY 8(f) NEXT-1, not a BASELINE.json config"),
                    "n_stations": w.n_stations, "n_baselines": w.n_baselines, "n_chan": w.n_chan, "n_time": w.n_time,
                    "window_M": w.window_M, "window_F": w.window_F, "n_int": w.n_int, "K": max(plan.K, 1), "variant": variant,
+                   "arithmetic": args.arith if args.arith == "fast" else f"tables, mask {args.mask:#06x}",
                    "input_bytes": w.input_bytes, "l2": "input (>= 9 GB) is far larger than the 126 MB L2: no flush needed",
                    "sharding": "by baseline, no collective" if world > 1 else "single GPU"},
         "gbytes_per_s": world * algo_bytes / (ms_per_step * 1e-3) / 1e9,
@@ -319,6 +322,9 @@ def main():
     ap.add_argument("--workload", default="lofar")
     ap.add_argument("--variant", default="auto", choices=["auto", "direct", "tma"])
     ap.add_argument("--K", type=int, default=1, help="threshold sets (K > 1: batched sweep)")
+    ap.add_argument("--arith", default="fast", choices=["fast", "tables"],
+                    help="tables: the paper's Tables 1-2 literally, per-group precision from --mask (DESIGN.md section 11)")
+    ap.add_argument("--mask", type=lambda x: int(x, 0), default=0x3C50, help="14-bit half-precision mask for --arith tables")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
