@@ -231,13 +231,16 @@ def run_ours(args):
     ms_per_step = total_ms / args.steps
     value = world * samples / (ms_per_step * 1e-3)
 
-    # a little science on the way out (not timed): detection quality against the injected ground truth
-    flags = rfi.unpack_flags(plan.get_flags(), w.n_chan).reshape(max(plan.K, 1), plan.n_win, plan.n_cells)
+    # a little science on the way out (not timed): per-set detection quality against the injected ground truth
+    # (BASELINE.json configs[4]; false-alarm / missed-detection probabilities of PAPER.md:235) via rfi_confusion_counts
     tr = truth.reshape(plan.n_win, plan.n_cells)
     if w.window_F > 1:                 # a footprint is RFI-bearing if any of its F channels is
         tr = tr.reshape(plan.n_win, -1, w.window_F).any(-1, keepdim=True).expand(-1, -1, w.window_F).reshape(plan.n_win, plan.n_cells)
-    fa = float((flags[0] & ~tr).sum() / max((~tr).sum(), 1))
-    md = float((~flags[0] & tr).sum() / max(tr.sum(), 1))
+    counts = plan.confusion_counts(rfi.pack_flags(tr.reshape(plan.n_win, plan.n_baselines, w.n_chan)))
+    counts = sharding.sum_over_ranks(counts)
+    p_fa, p_md = sharding.rates(counts.cpu())
+    flag_frac = (counts[:, 0] + counts[:, 3] - counts[:, 2]).double().cpu() / (counts[:, 1] + counts[:, 3]).double().cpu()
+    fa, md = float(p_fa[0]), float(p_md[0])
 
     if rank != 0:
         if dist is not None:
@@ -305,7 +308,10 @@ def run_ours(args):
                    "sharding": "by baseline, no collective" if world > 1 else "single GPU"},
         "gbytes_per_s": world * algo_bytes / (ms_per_step * 1e-3) / 1e9,
         "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
-        "detection": {"false_alarm": fa, "missed_detection": md, "flag_fraction": float(flags[0].float().mean())},
+        "detection": {"false_alarm": fa, "missed_detection": md, "flag_fraction": float(flag_frac[0]),
+                      "per_set": {"K": int(counts.shape[0]), "false_alarm_min_max": [float(p_fa.min()), float(p_fa.max())],
+                                  "missed_detection_min_max": [float(p_md.min()), float(p_md.max())],
+                                  "flag_fraction_min_max": [float(flag_frac.min()), float(flag_frac.max())]}},
     }
     print(json.dumps(line))
     if dist is not None:

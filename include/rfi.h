@@ -142,6 +142,14 @@ int rfi_process_chunk(rfi_plan *plan, const void *d_vis, void *d_avg, void *d_we
  * ordered after the kernel only on the stream that was passed to rfi_process_chunk. */
 int rfi_get_flags(rfi_plan *plan, const uint32_t **d_flags, size_t *n_words);
 
+/* Per-set confusion counters of the last processed chunk against a ground-truth mask (BASELINE.json configs[4];
+ * false-alarm / missed-detection probabilities as defined at PAPER.md:235).  d_truth: bit-packed like the flag
+ * mask of ONE set, [n_win][n_baselines][ceil(n_chan/32)] uint32_t, 1 = the window of that cell carries RFI.
+ * d_counts: uint64_t [K][4] = {false alarms, clean windows, missed detections, RFI windows}, counted per
+ * (window, cell); zeroed and filled on the stream.  P_fa = [0]/[1], P_md = [2]/[3].  Exact integers.
+ * RFI_ESTATE before the first process call; RFI_EINVAL for NULL / misaligned pointers. */
+int rfi_confusion_counts(rfi_plan *plan, const uint32_t *d_truth, uint64_t *d_counts, void *cuda_stream);
+
 /* End-to-end host path: vis in HOST memory (pinned for full speed), results to HOST memory.  Streams the
  * chunk to the device one output integration at a time on two internal streams so that host->device copies
  * overlap the kernel, then copies avg / weight / flags (and stats if non-NULL) back and synchronises.

@@ -22,7 +22,7 @@ MASK_PAPER_LEARNED = 0x3C50      # Tables 3-4: Table 1 groups
 
 EXPORTS = [
     "rfi_plan_create", "rfi_plan_set_integration", "rfi_plan_set_baseline_shard", "rfi_plan_set_window_freq", "rfi_plan_set_arithmetic", "rfi_set_thresholds", "rfi_plan_set_variant",
-    "rfi_process_chunk", "rfi_get_flags", "rfi_process_chunk_host", "rfi_plan_destroy",
+    "rfi_process_chunk", "rfi_get_flags", "rfi_confusion_counts", "rfi_process_chunk_host", "rfi_plan_destroy",
     "rfi_strerror", "rfi_last_cuda_error", "rfi_flags_bytes", "rfi_avg_bytes", "rfi_weight_bytes",
     "rfi_stats_bytes", "rfi_vis_bytes", "rfi_plan_launch_count", "rfi_plan_last_variant", "rfi_version",
 ]
@@ -71,10 +71,12 @@ def load_library(build_if_missing: bool = True):
     lib.rfi_process_chunk.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.rfi_get_flags.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(sz)]
     lib.rfi_process_chunk_host.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.rfi_confusion_counts.argtypes = [vp, vp, vp, vp]
+    lib.rfi_confusion_counts.restype = ci
     lib.rfi_plan_destroy.argtypes = [vp]
     for name in ("rfi_plan_create", "rfi_plan_set_integration", "rfi_plan_set_baseline_shard",
                  "rfi_plan_set_window_freq", "rfi_plan_set_arithmetic", "rfi_set_thresholds", "rfi_plan_set_variant",
-                 "rfi_process_chunk", "rfi_get_flags", "rfi_process_chunk_host", "rfi_plan_destroy",
+                 "rfi_process_chunk", "rfi_get_flags", "rfi_confusion_counts", "rfi_process_chunk_host", "rfi_plan_destroy",
                  "rfi_plan_last_variant"):
         getattr(lib, name).restype = ci
     lib.rfi_strerror.argtypes = [ci]
@@ -189,6 +191,18 @@ class RfiPlan:
         holder = type("_FlagView", (), {"__cuda_array_interface__": iface})()
         return torch.as_tensor(holder, device="cuda").view(shape)
 
+    def confusion_counts(self, truth_words: torch.Tensor, stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+        """rfi_confusion_counts: truth_words = pack_flags(bool truth) on the device; returns int64 [K, 4] on the device."""
+        if not (truth_words.is_cuda and truth_words.is_contiguous() and truth_words.dtype == torch.int32):
+            raise ValueError("truth_words must be a contiguous int32 CUDA tensor (pack_flags)")
+        if truth_words.numel() != self.n_win * self.n_baselines * self.wpb:
+            raise ValueError("truth_words has the wrong size for this plan")
+        counts = torch.empty(max(self.K, 1), 4, dtype=torch.int64, device=truth_words.device)
+        s = stream if stream is not None else torch.cuda.current_stream(truth_words.device)
+        _check(self._lib.rfi_confusion_counts(self._h, truth_words.data_ptr(), counts.data_ptr(), s.cuda_stream),
+               "rfi_confusion_counts")
+        return counts
+
     def process_chunk_host(self, vis: torch.Tensor, want_stats: bool = False):
         """rfi_process_chunk_host: vis is a (preferably pinned) CPU tensor; returns CPU tensors."""
         if vis.is_cuda or not vis.is_contiguous():
@@ -233,3 +247,13 @@ def unpack_flags(flags: torch.Tensor, n_chan: int) -> torch.Tensor:
     bits = torch.arange(32, device=flags.device, dtype=torch.int32)
     b = ((flags.unsqueeze(-1) >> bits) & 1).bool()
     return b.flatten(-2)[..., :n_chan]
+
+
+def pack_flags(mask: torch.Tensor) -> torch.Tensor:
+    """bool [.., n_baselines, n_chan] -> int32 words [.., n_baselines, ceil(n_chan/32)] (inverse of unpack_flags)."""
+    n_chan = mask.shape[-1]
+    wpb = (n_chan + 31) // 32
+    pad = wpb * 32 - n_chan
+    m = torch.nn.functional.pad(mask.to(torch.int64), (0, pad)).reshape(*mask.shape[:-1], wpb, 32)
+    w = (m << torch.arange(32, device=mask.device, dtype=torch.int64)).sum(-1)
+    return torch.where(w >= 2 ** 31, w - 2 ** 32, w).to(torch.int32)

@@ -383,6 +383,17 @@ int rfi_get_flags(rfi_plan* p, const uint32_t** d_flags, size_t* n_words) {
     return RFI_OK;
 }
 
+int rfi_confusion_counts(rfi_plan* p, const uint32_t* d_truth, uint64_t* d_counts, void* cuda_stream) {
+    if (!p || !d_truth || !d_counts) return RFI_EINVAL;
+    if (reinterpret_cast<uintptr_t>(d_truth) % 4 || reinterpret_cast<uintptr_t>(d_counts) % 8) return RFI_EINVAL;
+    if (!p->have_result) return RFI_ESTATE;
+    const size_t n_words = (size_t)p->n_win() * p->n_baselines * p->wpb();
+    const int rc = launch_confusion(p->d_flags, d_truth, d_counts, p->K, n_words, p->wpb(), p->n_chan, p->sm_count,
+                                    static_cast<cudaStream_t>(cuda_stream));
+    if (rc == RFI_OK) p->launches++;
+    return rc;
+}
+
 int rfi_process_chunk_host(rfi_plan* p, const void* h_vis, void* h_avg, void* h_weight, void* h_flags,
                            void* h_stats) {
     if (!p) return RFI_EINVAL;

@@ -85,6 +85,19 @@ def test_integration_and_threshold_validation():
     p.destroy()
 
 
+def test_pack_flags_is_the_boundary_layout():
+    """binding.pack_flags (argument marshalling for the ground-truth mask) against the oracle's layout pin."""
+    import torch
+    from oracle import rfi_oracle as orc
+    g = torch.Generator().manual_seed(3)
+    for B, C in ((3, 64), (4, 45), (2, 7)):
+        m = torch.rand(5, B, C, generator=g) < 0.4
+        got = rfi.pack_flags(m).numpy().view("uint32")
+        ref = orc.pack_flags(m.numpy().reshape(5, B * C).astype("uint8"), B, C)
+        assert (got == ref).all()
+        assert torch.equal(rfi.unpack_flags(rfi.pack_flags(m), C), m)
+
+
 def test_arithmetic_mode_validation():
     plan = rfi.RfiPlan(4, 10, 24, 40, 10)
     plan.set_arithmetic("tables", 0x3C50)

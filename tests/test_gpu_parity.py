@@ -284,3 +284,33 @@ def test_tf_footprints_batched(fp16):
     assert rep["K"] == 9
     w2 = synth.Workload("tf_k2", 5, False, 12, 5 * 16, 5, 5 * 8, fp16=fp16, window_F=4, burst_cell_frac=0.15)   # ragged: old batched kernel
     check(w2, synth.sweep_thresholds(20, 5, seed=5), "auto")
+
+
+# ------------------------------------------------------------------------------------------------------
+# per-set confusion counters against the injected ground truth (BASELINE.json configs[4])
+# ------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n_chan,K", [(64, 7), (45, 3), (16, 1)])
+def test_confusion_counts_are_exact(n_chan, K):
+    from oracle import rfi_oracle as orc
+    w = synth.Workload("conf", 5, True, n_chan, 256, 16, 64, burst_cell_frac=0.2, channel_gain=True)
+    thr = synth.sweep_thresholds(16, K, seed=8) if K > 1 else synth.default_thresholds(16)
+    vis, truth = synth.make_chunk(w, seed=77)
+    plan = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M, n_int=w.n_int)
+    plan.set_thresholds(thr)
+    avg, weight, _ = plan.alloc_outputs()
+    plan.process_chunk(vis.cuda(), avg, weight)
+    tw = rfi.pack_flags(truth.reshape(plan.n_win, w.n_baselines, n_chan).cuda())
+    counts = plan.confusion_counts(tw).cpu().numpy()
+    torch.cuda.synchronize()
+    flags = rfi.unpack_flags(plan.get_flags(), n_chan).reshape(K, plan.n_win, plan.n_cells).cpu().numpy()
+    plan.destroy()
+    t = truth.numpy().reshape(plan.n_win, plan.n_cells)
+    # the oracle's flags on the same data (thresholds as float32, like the kernel's)
+    ref = orc.process(vis.numpy().reshape(w.n_time, w.n_cells, 4, 2), 16, w.n_int,
+                      np.asarray(thr, np.float32).astype(np.float64), want_stats=False).flags.astype(bool)
+    for k in range(K):
+        want = [(flags[k] & ~t).sum(), (~t).sum(), (~flags[k] & t).sum(), t.sum()]
+        assert counts[k].tolist() == [int(x) for x in want]
+        if (flags[k] == ref[k]).all():
+            assert counts[k].tolist() == [int((ref[k] & ~t).sum()), int((~t).sum()), int((~ref[k] & t).sum()), int(t.sum())]
+    assert counts[:, 1].min() > 0 and counts[:, 3].min() > 0
