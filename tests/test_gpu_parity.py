@@ -314,3 +314,44 @@ def test_confusion_counts_are_exact(n_chan, K):
         if (flags[k] == ref[k]).all():
             assert counts[k].tolist() == [int((ref[k] & ~t).sum()), int((~t).sum()), int((~ref[k] & t).sum()), int(t.sum())]
     assert counts[:, 1].min() > 0 and counts[:, 3].min() > 0
+
+
+# ------------------------------------------------------------------------------------------------------
+# guard bands: compute-sanitizer is not available on the pool, so out-of-bounds stores are caught by canaries
+# ------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("mode", ["direct", "tma", "batched", "batched_ragged", "tables", "tf", "fp16"])
+def test_no_writes_outside_the_output_buffers(mode):
+    n_chan = 45 if mode == "batched_ragged" else 64
+    w = synth.Workload("guard", 5, True, n_chan, 320, 16 if mode != "tf" else 10, 160, fp16=(mode == "fp16"),
+                       burst_cell_frac=0.2, window_F=2 if mode == "tf" else 1)
+    vis, _ = synth.make_chunk(w, seed=5)
+    K = 5 if mode.startswith("batched") else 1
+    thr = synth.sweep_thresholds(16, K, seed=1) if K > 1 else synth.default_thresholds(w.window_M * w.window_F)
+    plan = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M,
+                       rfi.RFI_FP16 if w.fp16 else rfi.RFI_FP32, n_int=w.n_int)
+    if w.window_F > 1:
+        plan.set_window_freq(w.window_F)
+    if mode == "tables":
+        plan.set_arithmetic("tables", 0x3C50)
+    plan.set_thresholds(thr)
+    if mode in ("direct", "tma"):
+        plan.set_variant(mode)
+    G = 4096                                                   # guard elements on each side
+    n_avg = K * plan.n_out * plan.n_cells * 8
+    n_wt = K * plan.n_out * plan.n_cells
+    n_st = 3 * plan.n_win * plan.n_cells
+    fbuf = torch.full((G + n_avg + G + n_st + G,), -777.0, device="cuda")
+    ibuf = torch.full((G + n_wt + G,), -777, dtype=torch.int32, device="cuda")
+    avg = fbuf[G:G + n_avg]
+    stats = fbuf[G + n_avg + G:G + n_avg + G + n_st]
+    weight = ibuf[G:G + n_wt]
+    # the input sits between guards too: a stray READ cannot be seen, but the guards make sure it stays in bounds of an allocation
+    vbuf = torch.zeros(G + vis.numel() + G, dtype=vis.dtype, device="cuda")
+    vbuf[G:G + vis.numel()] = vis.flatten().cuda()
+    plan.process_chunk(vbuf[G:G + vis.numel()], avg, weight, stats)
+    torch.cuda.synchronize()
+    assert (fbuf[:G] == -777).all() and (fbuf[G + n_avg:G + n_avg + G] == -777).all() and (fbuf[-G:] == -777).all()
+    assert (ibuf[:G] == -777).all() and (ibuf[-G:] == -777).all()
+    assert (avg != -777).all() and (weight != -777).all() and (stats != -777).all()      # and everything inside was written
+    assert (vbuf[:G] == 0).all() and (vbuf[-G:] == 0).all()
+    plan.destroy()
