@@ -21,6 +21,10 @@
  * Guards: an all-zero window has tau = -(W d + 1)/(W - 1); a sample with p_i = 0 adds the zero vector
  * (the epsilon -> 0 limit of the paper's epsilon guards).
  * Arithmetic: fp32 throughout (accumulation included); RFI_FP16 only changes the storage type of the input.
+ * Eq.(5) is decided on x = tau/c against s_low/c and s_high/c (c = (W d + 1)/(W - 1) > 0; one division per threshold
+ * on the host), so a decision can differ from one taken on the rounded tau only within one ulp of a threshold.
+ * W = window_M, or window_M * F for T x F footprints (rfi_plan_set_window_freq).
+ * rfi_plan_set_arithmetic(RFI_ARITH_TABLES) selects the paper's operation tables in per-group single/half precision instead.
  * Finite inputs must satisfy 1e-18 <= |x| <= 1e18 or x == 0 (fp32 squares must neither overflow nor
  * underflow); outside that range the statistics are unspecified (never a fault).
  *
