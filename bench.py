@@ -278,7 +278,9 @@ def run_ours(args):
                 plan.process_chunk_host_into(h_vis, h_avg, h_weight, h_flags)      # synchronises before returning
             dt = (time.perf_counter() - t0) / n_e2e
             same = bool(torch.equal(h_avg, avg.cpu()) and torch.equal(h_weight, weight.cpu()))
-            e2e = {"value": world * samples / dt, "unit": UNIT, "h2d_bytes_per_step": w.input_bytes,
+            # N > 1: measured on rank 0 alone (pinning N x 18.5 GB of host memory is not safe on every box), so the
+            # figure is ONE GPU's end-to-end rate and is not multiplied by N
+            e2e = {"value": samples / dt, "unit": UNIT, "ranks_measured": 1, "h2d_bytes_per_step": w.input_bytes,
                    "d2h_bytes_per_step": out_bytes, "ms_per_step": dt * 1e3, "steps": n_e2e,
                    "h2d_gbs": w.input_bytes / dt / 1e9, "matches_device_path": same,
                    "api": "rfi_process_chunk_host (pinned host buffers; per-integration H2D overlapped with the kernel)"}
