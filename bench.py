@@ -242,6 +242,26 @@ def run_ours(args):
     flag_frac = (counts[:, 0] + counts[:, 3] - counts[:, 2]).double().cpu() / (counts[:, 1] + counts[:, 3]).double().cpu()
     fa, md = float(p_fa[0]), float(p_md[0])
 
+    # the paper's SK-only / DS-only / BOTH comparison in one batched pass: disabling a detector is
+    # a threshold at infinity (include/rfi.h).  Not timed.
+    by_detector = None
+    if plan.K == 1 and args.arith == "fast" and rank == 0:
+        INF = float("inf")
+        d0, lo0, hi0, g0 = thr[0]
+        plan3 = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M,
+                            rfi.RFI_FP16 if w.fp16 else rfi.RFI_FP32, n_int=w.n_int)
+        if w.window_F > 1:
+            plan3.set_window_freq(w.window_F)
+        plan3.set_thresholds([[d0, lo0, hi0, g0], [d0, lo0, hi0, INF], [d0, -INF, INF, g0]])
+        a3, w3, _ = plan3.alloc_outputs(device=dev)
+        plan3.process_chunk(vis, a3, w3)
+        c3 = plan3.confusion_counts(rfi.pack_flags(tr.reshape(plan.n_win, plan.n_baselines, w.n_chan))).cpu()
+        fa3, md3 = sharding.rates(c3)
+        by_detector = {name: {"false_alarm": float(fa3[i]), "missed_detection": float(md3[i])}
+                       for i, name in enumerate(("both", "sk_only", "ds_only"))}
+        plan3.destroy()
+        del a3, w3
+
     if rank != 0:
         if dist is not None:
             dist.barrier()
@@ -310,7 +330,7 @@ def run_ours(args):
                    "sharding": "by baseline, no collective" if world > 1 else "single GPU"},
         "gbytes_per_s": world * algo_bytes / (ms_per_step * 1e-3) / 1e9,
         "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
-        "detection": {"false_alarm": fa, "missed_detection": md, "flag_fraction": float(flag_frac[0]),
+        "detection": {"false_alarm": fa, "missed_detection": md, "flag_fraction": float(flag_frac[0]), "by_detector": by_detector,
                       "per_set": {"K": int(counts.shape[0]), "false_alarm_min_max": [float(p_fa.min()), float(p_fa.max())],
                                   "missed_detection_min_max": [float(p_md.min()), float(p_md.max())],
                                   "flag_fraction_min_max": [float(flag_frac.min()), float(flag_frac.max())]}},
