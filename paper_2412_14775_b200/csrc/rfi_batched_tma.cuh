@@ -75,7 +75,7 @@ __device__ __forceinline__ void lds128_head(uint32_t addr, float& a, float& b) {
     asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(a), "=f"(b), "=f"(c), "=f"(d) : "r"(addr));
 }
 
-template <int R, bool FP16, int SPW>
+template <int R, bool FP16, int SPW, bool FULLWORD>
 __global__ void __launch_bounds__(kBtWarps * 32, 1)
 rfi_batched_tma_kernel(const __grid_constant__ CUtensorMap tmap, const KParams p,
                        const __grid_constant__ BatchThr bt, const int stages) {
@@ -91,7 +91,8 @@ rfi_batched_tma_kernel(const __grid_constant__ CUtensorMap tmap, const KParams p
     const uint32_t rec_base = smem_base + (uint32_t)NW * stages * STAGE_BYTES;          // [2][NW][32 lanes][48 B]
     const uint32_t bars = rec_base + 2u * NW * 32u * kRecBytes + (uint32_t)warp * stages * 8;
 
-    const int n_tiles = p.n_cells >> 5;                       // n_chan % 32 == 0: whole tiles only
+    const int n_tiles = (p.n_cells + 31) >> 5;                // FULLWORD (n_chan % 32 == 0): whole tiles only; else the
+                                                              // last tile is ragged (TMA zero-fills, invalid lanes are masked)
     const int n_units = n_tiles * p.n_out_slab;
     if ((int)blockIdx.x >= n_units) return;
     const int my_units = (n_units - 1 - (int)blockIdx.x) / (int)gridDim.x + 1;
@@ -160,9 +161,13 @@ rfi_batched_tma_kernel(const __grid_constant__ CUtensorMap tmap, const KParams p
         const int tile = unit - o_local * n_tiles;
         const int o_global = p.o_first + o_local;
         LaneGeom g;
-        g.cell = tile * 32 + lane;
-        g.valid = true;
-        g.word = tile; g.bit = lane; g.group = 0xffffffffu; g.leader = lane == 0;
+        if constexpr (FULLWORD) {
+            g.cell = tile * 32 + lane;
+            g.valid = true;
+            g.word = tile; g.bit = lane; g.group = 0xffffffffu; g.leader = lane == 0;
+        } else {
+            g = lane_geom(p, tile, lane);                      // several flag words per tile, ragged last tile
+        }
 
         // this lane's flag word of set warp*SPW, window (round 0, lane): later sets / rounds are fixed strides away
         uint32_t* const flag_ptr = p.flags + ((size_t)(p.k_first + warp * SPW) * p.n_win_total
@@ -228,10 +233,21 @@ rfi_batched_tma_kernel(const __grid_constant__ CUtensorMap tmap, const KParams p
 #pragma unroll
                 for (int i = 0; i < SPW; ++i) {
                     const uint32_t word = contract_one(x, r_max, xl[i], xh[i], gm[i], acc[i], cnt[i], s);
-                    myw[i] = mine ? word : myw[i];
+                    if constexpr (FULLWORD) {
+                        myw[i] = mine ? word : myw[i];
+                    } else {
+                        // the lanes of one flag word are contiguous: the leader shifts its group's bits into place
+                        const int k = warp * SPW + i;
+                        if (g.leader && k < p.K) {
+                            const uint32_t v = ((word & g.group) >> lane) << g.bit;
+                            uint32_t* dst = p.flags + ((size_t)(p.k_first + k) * p.n_win_total + (size_t)o_global * p.wpo
+                                                       + round * NW + j) * flag_words_per_win + g.word;
+                            if (p.flags_atomic) atomicOr(dst, v); else *dst = v;
+                        }
+                    }
                 }
             }
-            if (lane < n_w) {
+            if (FULLWORD && lane < n_w) {
                 uint32_t* fp = flag_ptr + (size_t)round * NW * flag_words_per_win;
 #pragma unroll
                 for (int i = 0; i < SPW; ++i, fp += flag_set_stride)

@@ -18,12 +18,20 @@ int launch_rs(const rfi::KParams& kp, const rfi::BatchThr& bt, const CUtensorMap
     while (stages > 1 && NW * stages * (stage_bytes + 8) > budget) --stages;
     if (NW * stages * (stage_bytes + 8) > budget) return RFI_EINVAL;
     const size_t smem = (size_t)NW * stages * (stage_bytes + 8) + rec_bytes + 1024;
-    const int n_tiles = kp.n_cells / 32;
+    const int n_tiles = (kp.n_cells + 31) / 32;
     const long n_units = (long)n_tiles * kp.n_out_slab;
     long grid = n_units < sm_count ? n_units : sm_count;
-    auto kern = rfi::rfi_batched_tma_kernel<R, FP16, SPW>;
-    RFI_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    kern<<<(unsigned)grid, NW * 32, smem, st>>>(*map, kp, bt, stages);
+    // whole 32-channel flag words (one word per tile, no invalid lane) take the ballot-per-round store;
+    // anything else the generic per-word store
+    if (kp.n_chan % 32 == 0) {
+        auto kern = rfi::rfi_batched_tma_kernel<R, FP16, SPW, true>;
+        RFI_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        kern<<<(unsigned)grid, NW * 32, smem, st>>>(*map, kp, bt, stages);
+    } else {
+        auto kern = rfi::rfi_batched_tma_kernel<R, FP16, SPW, false>;
+        RFI_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        kern<<<(unsigned)grid, NW * 32, smem, st>>>(*map, kp, bt, stages);
+    }
     RFI_CUDA(cudaGetLastError());
     return RFI_OK;
 }
@@ -39,11 +47,10 @@ int launch_r(const rfi::KParams& kp, const rfi::BatchThr& bt, const CUtensorMap*
 
 }  // namespace
 
-// Shapes the TMA-staged batched kernel covers: whole 32-channel flag words (no ragged tile) and a block length
-// it is instantiated for.  Everything else runs the register-staged batched kernel.
+// Shapes the TMA-staged batched kernel covers: a block length it is instantiated for (and, checked by the caller,
+// a cell count the tensor map can describe).  Everything else runs the register-staged batched kernel.
 bool batched_tma_supported(bool fp16, const rfi::KParams& kp, int R) {
     if (env_int("RFI_BATCHED_TMA", 1) == 0) return false;
-    if (kp.n_chan % 32 != 0) return false;
     return fp16 ? (R == 8 || R == 4 || R == 2) : (R == 4 || R == 2);
 }
 
