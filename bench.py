@@ -190,7 +190,13 @@ def run_ours(args):
         plan.set_window_freq(w.window_F)
     if args.arith == "tables":
         plan.set_arithmetic("tables", args.mask)
-    plan.set_thresholds(thr)
+    two_classes = w.autos and args.classes
+    if two_classes:       # cross / auto threshold classes: autos have their own null statistics
+        plan.set_baseline_classes(synth.auto_baseline_mask(w).int().tolist())
+        auto = synth.auto_thresholds(W)
+        plan.set_thresholds([[t, auto if args.K <= 1 else [t[0]] + auto[1:]] for t in thr])
+    else:
+        plan.set_thresholds(thr)
     plan.set_variant(args.variant)
     avg, weight, _ = plan.alloc_outputs(device=dev)
     out_bytes = avg.numel() * 4 + weight.numel() * 4 + max(plan.K, 1) * plan.n_win * plan.n_baselines * plan.wpb * 4
@@ -245,7 +251,7 @@ def run_ours(args):
     # the paper's SK-only / DS-only / BOTH comparison in one batched pass: disabling a detector is
     # a threshold at infinity (include/rfi.h).  Not timed.
     by_detector = None
-    if plan.K == 1 and args.arith == "fast" and rank == 0:
+    if plan.K == 1 and args.arith == "fast" and rank == 0 and not two_classes:
         INF = float("inf")
         d0, lo0, hi0, g0 = thr[0]
         plan3 = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M,
@@ -326,6 +332,7 @@ def run_ours(args):
                    "n_stations": w.n_stations, "n_baselines": w.n_baselines, "n_chan": w.n_chan, "n_time": w.n_time,
                    "window_M": w.window_M, "window_F": w.window_F, "n_int": w.n_int, "K": max(plan.K, 1), "variant": variant,
                    "arithmetic": args.arith if args.arith == "fast" else f"tables, mask {args.mask:#06x}",
+                   "threshold_classes": 2 if two_classes else 1,
                    "input_bytes": w.input_bytes, "l2": "input (>= 9 GB) is far larger than the 126 MB L2: no flush needed",
                    "sharding": "by baseline, no collective" if world > 1 else "single GPU"},
         "gbytes_per_s": world * algo_bytes / (ms_per_step * 1e-3) / 1e9,
@@ -353,6 +360,8 @@ def main():
     ap.add_argument("--arith", default="fast", choices=["fast", "tables"],
                     help="tables: the paper's Tables 1-2 literally, per-group precision from --mask (DESIGN.md section 11)")
     ap.add_argument("--mask", type=lambda x: int(x, 0), default=0x3C50, help="14-bit half-precision mask for --arith tables")
+    ap.add_argument("--classes", action="store_true",
+                    help="separate threshold class for the auto-correlations (rfi_plan_set_baseline_classes)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -98,6 +98,16 @@ int rfi_plan_create(rfi_plan **out, int n_stations, int n_baselines, int n_chan,
 /* Samples per output integration: n_time % n_int == 0 and n_int % window_M == 0, else RFI_EINVAL. */
 int rfi_plan_set_integration(rfi_plan *plan, int n_int);
 
+/* Per-baseline threshold classes.  Every baseline stream is mitigated separately and its null
+ * statistics depend on the kind of stream: an auto-correlation is Hermitian with a large constant part, so its
+ * SK and alignment statistics under noise differ from a cross-correlation's (d "is given a priori").
+ * n_classes = 2 assigns each baseline of the array (h_class[n_baselines], values 0/1, e.g. 0 = cross, 1 = auto;
+ * copied) to a class; rfi_set_thresholds then takes K * 2 sets ordered [k][class] and every kernel decides each
+ * window with the set of its baseline's class (the stats plane carries tau with the d of the cell's class).
+ * n_classes = 1 (h_class ignored) restores one set per k.  Clears the thresholds: set them again afterwards.
+ * RFI_EINVAL for n_classes outside {1, 2}, a NULL table or a class value above 1. */
+int rfi_plan_set_baseline_classes(rfi_plan *plan, int n_classes, const uint8_t *h_class);
+
 /* Window footprint in frequency ("a data window of size W divided into T time samples and F
  * frequency samples, W = T x F"; the paper uses 10 x 2 and 5 x 4).  T is the window_M of
  * rfi_plan_create, F defaults to 1.  With F > 1 a window covers F adjacent channels of one baseline: the
@@ -129,7 +139,8 @@ int rfi_plan_set_baseline_shard(rfi_plan *plan, int b_first, int b_count);
 /* Copy K >= 1 threshold sets from host memory (d > 0 and not NaN; s_low/s_high/gamma may be +-inf, not NaN).
  * K == 1 runs the single-set kernel; K > 1 the batched kernel that evaluates up to 64 sets in one pass over the
  * data (one launch per 64 sets; the paper tunes its thresholds with a host-side search).
- * The statistics planes (d_stats) always carry tau with the d of set 0. */
+ * With two baseline classes (rfi_plan_set_baseline_classes) h_sets holds K * 2 sets ordered [k][class].
+ * The statistics planes (d_stats) always carry tau with the d of set 0 (of the cell's class). */
 int rfi_set_thresholds(rfi_plan *plan, int K, const rfi_thresholds *h_sets);
 
 /* Choose a kernel variant (default RFI_VARIANT_AUTO).  RFI_EINVAL if unknown. */

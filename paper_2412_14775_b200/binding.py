@@ -21,8 +21,8 @@ ARITH_FAST, ARITH_TABLES = 0, 1
 MASK_PAPER_LEARNED = 0x3C50      # Tables 3-4: Table 1 groups 5,7 and Table 2 groups 4-7 in half
 
 EXPORTS = [
-    "rfi_plan_create", "rfi_plan_set_integration", "rfi_plan_set_baseline_shard", "rfi_plan_set_window_freq", "rfi_plan_set_arithmetic", "rfi_set_thresholds", "rfi_plan_set_variant",
-    "rfi_process_chunk", "rfi_get_flags", "rfi_confusion_counts", "rfi_process_chunk_host", "rfi_plan_destroy",
+    "rfi_plan_create", "rfi_plan_set_integration", "rfi_plan_set_baseline_shard", "rfi_plan_set_window_freq", "rfi_plan_set_arithmetic", "rfi_plan_set_baseline_classes", "rfi_set_thresholds",
+    "rfi_plan_set_variant", "rfi_process_chunk", "rfi_get_flags", "rfi_confusion_counts", "rfi_process_chunk_host", "rfi_plan_destroy",
     "rfi_strerror", "rfi_last_cuda_error", "rfi_flags_bytes", "rfi_avg_bytes", "rfi_weight_bytes",
     "rfi_stats_bytes", "rfi_vis_bytes", "rfi_plan_launch_count", "rfi_plan_last_variant", "rfi_version",
 ]
@@ -65,6 +65,8 @@ def load_library(build_if_missing: bool = True):
     lib.rfi_plan_set_integration.argtypes = [vp, ci]
     lib.rfi_plan_set_baseline_shard.argtypes = [vp, ci, ci]
     lib.rfi_plan_set_window_freq.argtypes = [vp, ci]
+    lib.rfi_plan_set_baseline_classes.argtypes = [vp, ci, ctypes.c_char_p]
+    lib.rfi_plan_set_baseline_classes.restype = ci
     lib.rfi_plan_set_arithmetic.argtypes = [vp, ci, ctypes.c_uint32]
     lib.rfi_set_thresholds.argtypes = [vp, ci, ctypes.POINTER(RfiThresholds)]
     lib.rfi_plan_set_variant.argtypes = [vp, ci]
@@ -115,6 +117,8 @@ class RfiPlan:
         self.K = 0
         self.b_first = 0
         self.window_F = 1
+        self.n_classes = 1
+        self._n_baselines_total = n_baselines
         if n_int is not None:
             self.set_integration(n_int)
 
@@ -148,8 +152,29 @@ class RfiPlan:
         _check(self._lib.rfi_plan_set_baseline_shard(self._h, b_first, b_count), "rfi_plan_set_baseline_shard")
         self.b_first, self.n_baselines = b_first, b_count
 
-    def set_thresholds(self, sets: Sequence[Sequence[float]]):
-        arr = (RfiThresholds * len(sets))(*[RfiThresholds(*map(float, s)) for s in sets])
+    def set_baseline_classes(self, classes: Optional[Sequence[int]]):
+        """rfi_plan_set_baseline_classes: classes[b] in {0, 1} for every baseline of the array (None: one class).
+        Thresholds must be set again afterwards; with two classes set_thresholds takes [[set_class0, set_class1], ...]."""
+        if classes is None:
+            _check(self._lib.rfi_plan_set_baseline_classes(self._h, 1, None), "rfi_plan_set_baseline_classes")
+            self.n_classes = 1
+        else:
+            buf = bytes(bytearray(int(c) for c in classes))
+            if len(buf) != self._n_baselines_total:
+                raise ValueError("classes must have one entry per baseline of the array")
+            _check(self._lib.rfi_plan_set_baseline_classes(self._h, 2, buf), "rfi_plan_set_baseline_classes")
+            self.n_classes = 2
+        self.K = 0
+
+    def set_thresholds(self, sets):
+        """K sets (d, s_low, s_high, gamma); with two baseline classes K pairs [[class 0 set, class 1 set], ...]."""
+        if self.n_classes == 2:
+            flat = [s for pair in sets for s in pair]
+            if len(flat) != 2 * len(sets):
+                raise ValueError("with two baseline classes every entry must be a pair of sets")
+        else:
+            flat = list(sets)
+        arr = (RfiThresholds * len(flat))(*[RfiThresholds(*map(float, s)) for s in flat])
         _check(self._lib.rfi_set_thresholds(self._h, len(sets), arr), "rfi_set_thresholds")
         self.K = len(sets)
 

@@ -48,6 +48,10 @@ struct rfi_plan {
     int arith = RFI_ARITH_FAST;               // arithmetic mode
     uint32_t arith_mask = 0;                  // 14-bit precision mask of the tables mode
     int F = 1;                                // window extent in frequency (channels), W = M * F
+    int n_classes = 1;                        // baseline threshold classes (1 or 2); thr holds K * n_classes sets, [k][class]
+    std::vector<uint8_t> h_cls;               // class of every baseline of the whole array (n_classes == 2)
+    uint8_t* d_cls = nullptr;
+    bool cls_uploaded = false;
     int n_baselines_total = 0, b_first = 0;   // n_baselines is the shard this plan processes (default: all)
     int K = 0;
     std::vector<rfi_thresholds> thr;
@@ -186,7 +190,11 @@ int enqueue_slab(rfi_plan* p, const void* d_vis_slab, int o_first, int n_out_sla
     kp.weight = d_weight;
     kp.stats = d_stats;
     kp.flags = p->d_flags;
+    const int nc = p->n_classes;
     kp.thr0 = to_device_thr(p->thr[0], p->M * p->F);
+    kp.thr1 = to_device_thr(p->thr[nc - 1], p->M * p->F);
+    kp.cls = nc > 1 ? p->d_cls : nullptr;
+    kp.b_first = p->b_first;
     kp.n_cells = (int)p->n_cells();
     kp.n_chan = p->n_chan;
     kp.n_baselines = p->n_baselines;
@@ -215,6 +223,10 @@ int enqueue_slab(rfi_plan* p, const void* d_vis_slab, int o_first, int n_out_sla
         kp.s_low = p->thr[0].s_low;
         kp.s_high = p->thr[0].s_high;
         kp.thr0.gamma = p->thr[0].gamma;
+        kp.d1 = p->thr[nc - 1].d;
+        kp.s_low1 = p->thr[nc - 1].s_low;
+        kp.s_high1 = p->thr[nc - 1].s_high;
+        kp.thr1.gamma = p->thr[nc - 1].gamma;
         kp.arith_mask = p->arith_mask;
         p->last_variant = RFI_VARIANT_TABLES;
         const int rc = launch_tables(kp, st);
@@ -238,7 +250,10 @@ int enqueue_slab(rfi_plan* p, const void* d_vis_slab, int o_first, int n_out_sla
             memset(&bt, 0, sizeof(bt));
             kp.k_first = k0;
             kp.K = p->K - k0 < rfi::kMaxBatch ? p->K - k0 : rfi::kMaxBatch;
-            for (int k = 0; k < kp.K; ++k) bt.t[k] = to_device_thr(p->thr[k0 + k], p->M * p->F);
+            for (int k = 0; k < kp.K; ++k) {
+                bt.t[k] = to_device_thr(p->thr[(size_t)(k0 + k) * nc], p->M * p->F);
+                bt.t1[k] = to_device_thr(p->thr[(size_t)(k0 + k) * nc + nc - 1], p->M * p->F);
+            }
             const int rc = use_tma ? launch_batched_tma(fp16, kp, bt, map, R, p->sm_count, p->smem_optin, st)
                                    : launch_batched(fp16, kp, bt, st);
             if (rc != RFI_OK) return rc;
@@ -273,6 +288,11 @@ int prepare(rfi_plan* p, cudaStream_t st) {
     if (rc != RFI_OK) return rc;
     rc = ensure_flags(p);
     if (rc != RFI_OK) return rc;
+    if (p->n_classes > 1 && !p->cls_uploaded) {
+        if (!p->d_cls && cudaMalloc(&p->d_cls, p->h_cls.size()) != cudaSuccess) { cudaGetLastError(); return RFI_ENOMEM; }
+        RFI_CUDA(cudaMemcpy(p->d_cls, p->h_cls.data(), p->h_cls.size(), cudaMemcpyHostToDevice));
+        p->cls_uploaded = true;
+    }
     const bool flags_atomic = (p->n_chan % 32 != 0 && 32 % p->n_chan != 0);
     if (flags_atomic) RFI_CUDA(cudaMemsetAsync(p->d_flags, 0, p->flags_words() * sizeof(uint32_t), st));
     return RFI_OK;
@@ -315,6 +335,24 @@ int rfi_plan_set_integration(rfi_plan* p, int n_int) {
     return RFI_OK;
 }
 
+int rfi_plan_set_baseline_classes(rfi_plan* p, int n_classes, const uint8_t* h_class) {
+    if (!p || n_classes < 1 || n_classes > 2) return RFI_EINVAL;
+    if (n_classes == 2) {
+        if (!h_class) return RFI_EINVAL;
+        for (int b = 0; b < p->n_baselines_total; ++b)
+            if (h_class[b] > 1) return RFI_EINVAL;
+        p->h_cls.assign(h_class, h_class + p->n_baselines_total);
+    } else {
+        p->h_cls.clear();
+    }
+    p->n_classes = n_classes;
+    p->cls_uploaded = false;
+    p->K = 0;                                 // the threshold table changes shape: thresholds must be set again
+    p->thr.clear();
+    p->have_result = false;
+    return RFI_OK;
+}
+
 int rfi_plan_set_window_freq(rfi_plan* p, int F) {
     if (!p || F < 1 || F > 32 || (F & (F - 1)) != 0 || p->n_chan % F != 0) return RFI_EINVAL;
     p->F = F;
@@ -342,12 +380,13 @@ int rfi_plan_set_baseline_shard(rfi_plan* p, int b_first, int b_count) {
 
 int rfi_set_thresholds(rfi_plan* p, int K, const rfi_thresholds* h_sets) {
     if (!p || K < 1 || !h_sets || K > 4096) return RFI_EINVAL;
-    for (int k = 0; k < K; ++k) {
+    const int n_sets = K * p->n_classes;                      // [k][class]
+    for (int k = 0; k < n_sets; ++k) {
         const rfi_thresholds& t = h_sets[k];
         if (!(t.d > 0.f) || std::isinf(t.d)) return RFI_EINVAL;
         if (std::isnan(t.s_low) || std::isnan(t.s_high) || std::isnan(t.gamma)) return RFI_EINVAL;
     }
-    p->thr.assign(h_sets, h_sets + K);
+    p->thr.assign(h_sets, h_sets + n_sets);
     p->K = K;
     p->have_result = false;
     return RFI_OK;
@@ -454,6 +493,7 @@ int rfi_plan_destroy(rfi_plan* p) {
     if (!p) return RFI_EINVAL;
     if (p->dev_ready) {
         if (p->d_flags) cudaFree(p->d_flags);
+        if (p->d_cls) cudaFree(p->d_cls);
         if (p->d_avg) cudaFree(p->d_avg);
         if (p->d_weight) cudaFree(p->d_weight);
         if (p->d_stats) cudaFree(p->d_stats);

@@ -102,7 +102,7 @@ rfi_batched_kernel(const KParams p, const __grid_constant__ BatchThr bt) {
                 my[3 + 2 * q][lane] = lo;
                 my[4 + 2 * q][lane] = hi;
             }
-            if (p.k_first == 0) store_stats(p, g, o_global * p.wpo + round * NW + warp, p.thr0.c * x, r_re, r_im);
+            if (p.k_first == 0) store_stats(p, g, o_global * p.wpo + round * NW + warp, (g.cls ? p.thr1.c : p.thr0.c) * x, r_re, r_im);
             w.reset();
             b_in_win = 0;
         }
@@ -120,7 +120,7 @@ rfi_batched_kernel(const KParams p, const __grid_constant__ BatchThr bt) {
             for (int i = 0; i < SPW; ++i) {
                 const int k = warp * SPW + i;
                 if (k < p.K) {                                         // warp-uniform
-                    const bool flag = decide(x, max_nan(r_re, r_im), bt.t[k]);
+                    const bool flag = decide(x, max_nan(r_re, r_im), g.cls ? bt.t1[k] : bt.t[k]);
                     store_flags(p, g, p.k_first + k, w_global, flag);
                     if (!flag) {
 #pragma unroll

@@ -165,6 +165,7 @@ rfi_batched_tma_kernel(const __grid_constant__ CUtensorMap tmap, const KParams p
             g.cell = tile * 32 + lane;
             g.valid = true;
             g.word = tile; g.bit = lane; g.group = 0xffffffffu; g.leader = lane == 0;
+            g.cls = p.cls ? (int)p.cls[p.b_first + (tile * 32) / p.n_chan] : 0;   // a whole-word tile lies in one baseline
         } else {
             g = lane_geom(p, tile, lane);                      // several flag words per tile, ragged last tile
         }
@@ -208,7 +209,7 @@ rfi_batched_tma_kernel(const __grid_constant__ CUtensorMap tmap, const KParams p
                 const bool fin = finite2(w.s[0]) && finite2(w.s[1]) && finite2(w.s[2]) && finite2(w.s[3]);
                 sts128_f2(ra + 16, fin ? w.s[0] : 0ull, fin ? w.s[1] : 0ull);
                 sts128_f2(ra + 32, fin ? w.s[2] : 0ull, fin ? w.s[3] : 0ull);
-                if (p.k_first == 0) store_stats(p, g, o_global * p.wpo + wl, p.thr0.c * x, r_re, r_im);
+                if (p.k_first == 0) store_stats(p, g, o_global * p.wpo + wl, (g.cls ? p.thr1.c : p.thr0.c) * x, r_re, r_im);
             }
             __syncthreads();
             // ---- contract: this thread's sets against the round's records ----
@@ -217,7 +218,7 @@ rfi_batched_tma_kernel(const __grid_constant__ CUtensorMap tmap, const KParams p
             uint32_t myw[SPW];
 #pragma unroll
             for (int i = 0; i < SPW; ++i) {
-                const Thr t = bt.t[warp * SPW + i];
+                const Thr t = g.cls ? bt.t1[warp * SPW + i] : bt.t[warp * SPW + i];   // the lane's baseline class
                 xl[i] = t.x_low; xh[i] = t.x_high; gm[i] = t.gamma;
                 myw[i] = 0;
             }

@@ -43,7 +43,10 @@ struct KParams {
     uint32_t* weight;         // [K][n_out_total][n_cells]
     float* stats;             // [3][n_win_total][n_cells] or nullptr
     uint32_t* flags;          // [K][n_win_total][n_baselines*wpb]
-    Thr thr0;                 // set 0 (single-set kernels; stats use its c)
+    Thr thr0;                 // set 0, baseline class 0 (single-set kernels; stats use its c)
+    Thr thr1;                 // set 0, baseline class 1 (= thr0 when the plan has one class)
+    const uint8_t* cls;       // [n_baselines of the whole array] class of each baseline (0/1), or nullptr: all class 0
+    int b_first;              // first baseline of this plan's shard (index into cls)
     int n_cells, n_chan, n_baselines, wpb;
     int M, n_int, wpo;        // window length in time (T), samples per output, windows per output
     int F;                    // window extent in frequency: F adjacent channels (lanes), power of two <= 32
@@ -56,10 +59,11 @@ struct KParams {
     int flags_atomic;         // 1: flag words may be shared between warps -> atomicOr into a zeroed buffer
     // paper-literal tables mode (rfi_tables.cuh) only: raw thresholds of set 0 and the 14-bit precision mask
     float d, s_low, s_high;
+    float d1, s_low1, s_high1;   // class 1
     uint32_t arith_mask;
 };
 
-struct BatchThr { Thr t[kMaxBatch]; };            // by-value kernel parameter (constant bank), 1 KiB
+struct BatchThr { Thr t[kMaxBatch]; Thr t1[kMaxBatch]; };   // by-value kernel parameter (constant bank), 2 KiB: class 0, class 1
 
 // ------------------------------------------------------------------------------------------------
 // PTX wrappers

@@ -89,15 +89,17 @@ __device__ __forceinline__ void tables_sample(TabWin& w, const f2 (&x)[4], uint3
 
 // Window tail: Table 1 groups 5-7, Table 2 groups 5-7, decision.
 template <int MASK>
-__device__ __forceinline__ bool tables_tail(const TabWin& w, const KParams& p, float& tau, float& r_re, float& r_im) {
+__device__ __forceinline__ bool tables_tail(const TabWin& w, const KParams& p, int cls, float& tau, float& r_re, float& r_im) {
     const uint32_t mask = p.arith_mask;
+    const float d = cls ? p.d1 : p.d, s_low = cls ? p.s_low1 : p.s_low, s_high = cls ? p.s_high1 : p.s_high;
+    const float gamma = cls ? p.thr1.gamma : p.thr0.gamma;
     const Fmt g5 = table_fmt<MASK>(mask, 4), g6 = table_fmt<MASK>(mask, 5), g7 = table_fmt<MASK>(mask, 6);
     const float Wf = (float)p.M;
-    tau = g5.div(g5.add(g5.mul(Wf, p.d), 1.0f), g5.sub(Wf, 1.0f));           // group 5
+    tau = g5.div(g5.add(g5.mul(Wf, d), 1.0f), g5.sub(Wf, 1.0f));           // group 5
     const float s12 = g6.mul(w.s1, w.s1);                                    // group 6
     const float ratio = g7.div(g7.mul(Wf, w.s2), g7.add(s12, g7.eps()));     // group 7
     tau = g7.mul(tau, g7.sub(ratio, 1.0f));
-    bool keep = (g7.cv(tau) >= g7.cv(p.s_low)) && (g7.cv(tau) <= g7.cv(p.s_high));
+    bool keep = (g7.cv(tau) >= g7.cv(s_low)) && (g7.cv(tau) <= g7.cv(s_high));
     const Fmt d5 = table_fmt<MASK>(mask, 11), d6 = table_fmt<MASK>(mask, 12), d7 = table_fmt<MASK>(mask, 13);
     float r[2];
 #pragma unroll
@@ -106,7 +108,7 @@ __device__ __forceinline__ bool tables_tail(const TabWin& w, const KParams& p, f
         const float u2 = d5.mul(w.us[part], w.us[part]);
         const float v2 = d5.mul(w.vs[part], w.vs[part]);
         r[part] = d6.div(d6.sqrt(d6.add(d6.add(q2, u2), v2)), Wf);           // group 6
-        keep = keep && (d7.cv(r[part]) <= d7.cv(p.thr0.gamma));              // group 7
+        keep = keep && (d7.cv(r[part]) <= d7.cv(gamma));              // group 7
     }
     r_re = r[0];
     r_im = r[1];
@@ -152,7 +154,7 @@ __global__ void __launch_bounds__(128, 4) rfi_tables_kernel(const KParams p) {
         ++blk;
         if (++b_in_win == bpw) {
             float tau, r_re, r_im;
-            const bool flag = tables_tail<MASK>(w, p, tau, r_re, r_im);
+            const bool flag = tables_tail<MASK>(w, p, g.cls, tau, r_re, r_im);
             store_flags(p, g, p.k_first, w_global, flag);
             store_stats(p, g, w_global, tau, r_re, r_im);
             if (!flag) {

@@ -141,6 +141,7 @@ struct LaneGeom {
     int word;          // b * wpb + c/32
     int bit;           // c % 32
     unsigned group;    // lanes of this warp that share `word`
+    int cls;           // threshold class of the lane's baseline (0/1)
     bool leader;       // lowest lane of the group
 };
 
@@ -153,6 +154,7 @@ __device__ __forceinline__ LaneGeom lane_geom(const KParams& p, int tile, int la
     const int c = g.cell - b * p.n_chan;
     g.word = g.valid ? b * p.wpb + (c >> 5) : -1 - lane;      // invalid lanes form singleton groups
     g.bit = c & 31;
+    g.cls = p.cls ? (int)p.cls[p.b_first + b] : 0;
     g.group = __match_any_sync(0xffffffffu, g.word);
     g.leader = g.valid && ((__ffs(g.group) - 1) == lane);
     return g;
@@ -207,9 +209,10 @@ __device__ __forceinline__ void finish_window(const KParams& p, const LaneGeom& 
     float x, r_re, r_im;
     if (p.F > 1) combine_group(w, p.F, p.M);
     window_stats(w, inv_W, x, r_re, r_im);
-    const bool flag = decide(x, max_nan(r_re, r_im), p.thr0);
+    const Thr& t = g.cls ? p.thr1 : p.thr0;                   // per-baseline-class thresholds (cross / auto)
+    const bool flag = decide(x, max_nan(r_re, r_im), t);
     store_flags(p, g, p.k_first, w_global, flag);
-    store_stats(p, g, w_global, p.thr0.c * x, r_re, r_im);
+    store_stats(p, g, w_global, t.c * x, r_re, r_im);
     if (!flag) {
 #pragma unroll
         for (int q = 0; q < 4; ++q) acc[q] = add2(acc[q], w.s[q]);

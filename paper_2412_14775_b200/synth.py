@@ -253,6 +253,24 @@ _NULL_Q = {
 }
 
 
+# The same for the auto-correlations of this noise model (Hermitian, Sigma + H/sqrt(n_acc)): |I| is nearly constant,
+# so x sits far below the cross-correlation values; r_im = 0 exactly.  Written by a throw-away run of oracle/ on
+# make_chunk output (40 stations, 20480+ windows); only used to place the class-1 thresholds.
+_NULL_Q_AUTO = {
+    16: ((0.024, 0.0386, 0.0546, 0.207, 0.2571, 0.3342), (0.418, 0.496, 0.575)),
+    20: ((0.031, 0.0447, 0.0602, 0.198, 0.2430, 0.3030), (0.377, 0.449, 0.522)),
+    32: ((0.046, 0.0578, 0.0724, 0.183, 0.2158, 0.2601), (0.307, 0.365, 0.432)),
+    64: ((0.064, 0.0750, 0.0867, 0.165, 0.1870, 0.2147), (0.230, 0.273, 0.323)),
+}
+
+
+def auto_thresholds(M: int, d: float = 1.0):
+    """One (d, s_low, s_high, gamma) set near the 1 % / 99 % null quantiles of the auto-correlations (class 1)."""
+    xq, rq = _NULL_Q_AUTO[M] if M in _NULL_Q_AUTO else _NULL_Q_AUTO[min(_NULL_Q_AUTO, key=lambda k: abs(k - M))]
+    c = (M * d + 1) / (M - 1)
+    return [d, c * xq[1], c * xq[4], rq[1]]
+
+
 def _quantiles(M: int):
     if M in _NULL_Q:
         return _NULL_Q[M]

@@ -98,6 +98,25 @@ def test_pack_flags_is_the_boundary_layout():
         assert torch.equal(rfi.unpack_flags(rfi.pack_flags(m), C), m)
 
 
+def test_baseline_classes_validation():
+    plan = rfi.RfiPlan(4, 10, 24, 40, 10)
+    plan.set_thresholds([[1.0, 0.1, 1.0, 0.5]])
+    plan.set_baseline_classes([0, 1] * 5)
+    assert plan.K == 0                                     # thresholds must be set again
+    plan.set_thresholds([[[1.0, 0.1, 1.0, 0.5], [0.5, 0.0, 2.0, 0.9]]])
+    assert plan.K == 1
+    with pytest.raises(ValueError):
+        plan.set_thresholds([[1.0, 0.1, 1.0, 0.5]] * 3)   # not pairs
+    with pytest.raises(ValueError):
+        plan.set_baseline_classes([0] * 9)
+    with pytest.raises(rfi.RfiError) as e:
+        plan.set_baseline_classes([0] * 9 + [2])
+    assert e.value.code == -1
+    plan.set_baseline_classes(None)
+    plan.set_thresholds([[1.0, 0.1, 1.0, 0.5]])
+    plan.destroy()
+
+
 def test_arithmetic_mode_validation():
     plan = rfi.RfiPlan(4, 10, 24, 40, 10)
     plan.set_arithmetic("tables", 0x3C50)

@@ -355,3 +355,63 @@ def test_no_writes_outside_the_output_buffers(mode):
     assert (avg != -777).all() and (weight != -777).all() and (stats != -777).all()      # and everything inside was written
     assert (vbuf[:G] == 0).all() and (vbuf[-G:] == 0).all()
     plan.destroy()
+
+
+# ------------------------------------------------------------------------------------------------------
+# per-baseline threshold classes (cross / auto): each cell against the oracle run with its class's thresholds
+# ------------------------------------------------------------------------------------------------------
+def _run_classes(w, vis, classes, pairs, variant="auto", shard=None):
+    plan = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M,
+                       rfi.RFI_FP16 if w.fp16 else rfi.RFI_FP32, n_int=w.n_int)
+    if w.window_F > 1:
+        plan.set_window_freq(w.window_F)
+    plan.set_baseline_classes(classes)
+    v = vis
+    if shard is not None:
+        plan.set_baseline_shard(*shard)
+        v = vis[:, shard[0]:shard[0] + shard[1]].contiguous()
+    plan.set_thresholds(pairs)
+    plan.set_variant(variant)
+    avg, weight, st = plan.alloc_outputs(stats=True)
+    plan.process_chunk(v.cuda(), avg, weight, st)
+    torch.cuda.synchronize()
+    out = gpu_outputs_to_numpy(plan, avg, weight, st, rfi.unpack_flags(plan.get_flags(), w.n_chan))
+    used = plan.last_variant
+    plan.destroy()
+    return out, used
+
+
+@pytest.mark.parametrize("mode", ["direct", "tma", "batched", "batched_ragged", "fp16", "tf", "shard"])
+def test_baseline_classes(mode):
+    n_chan = 24 if mode == "batched_ragged" else 64
+    F = 2 if mode == "tf" else 1
+    w = synth.Workload("cls", 6, True, n_chan, 512, 16, 256, fp16=(mode == "fp16"), window_F=F,
+                       burst_cell_frac=0.15, channel_gain=True)
+    vis, _ = synth.make_chunk(w, seed=91)
+    autos = synth.auto_baseline_mask(w).numpy()
+    classes = autos.astype(int).tolist()
+    W = 16 * F
+    K = 6 if mode.startswith("batched") else 1
+    cross_sets = synth.sweep_thresholds(W, K, seed=2) if K > 1 else synth.default_thresholds(W)
+    c = (W * 0.7 + 1) / (W - 1)
+    auto_sets = [[0.7, -float("inf"), c * (0.02 + 0.01 * k), 0.9 - 0.02 * k] for k in range(K)]   # autos: tau ~ 0, r_re ~ 1
+    pairs = [[cross_sets[k], auto_sets[k]] for k in range(K)]
+    shard = (5, 9) if mode == "shard" else None
+    out, used = _run_classes(w, vis, classes, pairs, variant=mode if mode in ("direct", "tma") else "auto", shard=shard)
+    b0, bc = shard if shard else (0, w.n_baselines)
+    v = vis[:, b0:b0 + bc].numpy().reshape(w.n_time, bc * n_chan, 4, 2)
+    cell_auto = np.repeat(autos[b0:b0 + bc], n_chan)
+    tol = 2e-3 if w.fp16 else 1e-5
+    n_flagged = 0
+    for cls, sets in ((0, cross_sets), (1, auto_sets)):
+        sel = np.nonzero(cell_auto == bool(cls))[0]
+        sub = {"avg": out["avg"][:, :, sel], "weight": out["weight"][:, :, sel], "flags": out["flags"][:, :, sel],
+               "tau": out["tau"][:, sel], "r_re": out["r_re"][:, sel], "r_im": out["r_im"][:, sel]}
+        rep = compare(v[:, sel], 16, w.n_int, sets, sub, tol=tol, fp16=w.fp16, F=F)
+        n_flagged += rep["oracle_flag_fraction"] > 0
+    assert n_flagged >= 1
+    # the classes really matter: the same data with the cross thresholds everywhere differs on the autos only
+    if shard is None:
+        single, _ = run_gpu(w, vis, cross_sets[:1], "auto")
+        assert (single["flags"][0][:, ~cell_auto] == out["flags"][0][:, ~cell_auto]).all()
+        assert (single["flags"][0][:, cell_auto] != out["flags"][0][:, cell_auto]).mean() > 0.05

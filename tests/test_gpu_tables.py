@@ -116,3 +116,28 @@ def test_flag_agreement_of_the_learned_assignment_with_the_fast_path():
     plan.destroy()
     agree = float((fast == tab["flags"]).mean())
     assert agree > 0.99, agree
+
+
+def test_tables_mode_with_baseline_classes():
+    """Per-class thresholds in the tables arithmetic: every cell bit-exact against the oracle run with its class's set."""
+    w = synth.Workload("tab_cls", 5, True, 32, 256, 16, 128, burst_cell_frac=0.15)
+    vis, _ = synth.make_chunk(w, seed=3)
+    autos = synth.auto_baseline_mask(w).numpy()
+    sets = [(1.0, 0.1, 0.7, 0.5), (0.6, 0.02, 0.3, 0.52)]
+    plan = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M, n_int=w.n_int)
+    plan.set_arithmetic("tables", PAPER)
+    plan.set_baseline_classes(autos.astype(int).tolist())
+    plan.set_thresholds([[list(sets[0]), list(sets[1])]])
+    avg, weight, stats = plan.alloc_outputs(stats=True)
+    plan.process_chunk(vis.cuda(), avg, weight, stats)
+    torch.cuda.synchronize()
+    flags = rfi.unpack_flags(plan.get_flags(), w.n_chan).reshape(plan.n_win, plan.n_cells).cpu().numpy()
+    tau = stats.cpu().numpy().reshape(3, plan.n_win, plan.n_cells)[0]
+    plan.destroy()
+    v = vis.numpy().reshape(w.n_time, w.n_cells, 4, 2)
+    cell_auto = np.repeat(autos, w.n_chan)
+    for cls in (0, 1):
+        sel = np.nonzero(cell_auto == bool(cls))[0]
+        ref = orc.tables_process(v[:, sel], w.window_M, w.n_int, sets[cls], PAPER)
+        np.testing.assert_array_equal(tau[:, sel].view(np.uint32), ref.tau[0].view(np.uint32))
+        np.testing.assert_array_equal(flags[:, sel], ref.flags[0].astype(bool))
