@@ -43,6 +43,7 @@
  * rfi_process_chunk enqueues work on the stream and returns without synchronising the host.
  *
  * Errors: every function returns RFI_OK (0) or a negative code; nothing throws or aborts.
+ * Threads: a plan is not internally locked; use one plan from one host thread at a time (different plans are independent).
  */
 #ifndef RFI_H_
 #define RFI_H_
