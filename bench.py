@@ -318,7 +318,7 @@ def run_ours(args):
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         g = torch.Generator().manual_seed(7)
-        n_s = min(w.n_cells, 16384)
+        n_s = min(w.n_cells, 24576)           # ~12 CPU-seconds of oracle work on the lofar shape
         idx = torch.randperm(w.n_cells, generator=g)[:n_s].sort().values.to(dev)
         sub = vis.reshape(w.n_time, w.n_cells, 4, 2)[:, idx].cpu().numpy()
         cpu = oracle_baseline(sub, w, thr)
