@@ -148,7 +148,9 @@ int rfi_set_thresholds(rfi_plan *plan, int K, const rfi_thresholds *h_sets);
 int rfi_plan_set_variant(rfi_plan *plan, int variant);
 
 /* Process one chunk resident in device memory.  d_stats may be NULL.  cuda_stream is a cudaStream_t
- * (NULL = legacy default stream).  Asynchronous.  RFI_ESTATE if thresholds were never set; RFI_EINVAL for
+ * (NULL = legacy default stream).  Asynchronous.  After one warm-up call (which allocates the plan's flag buffer
+ * and, for the TMA kernels, encodes the tensor map of this d_vis) a call is pure stream work -- kernel launches and
+ * at most one memset -- and can be captured in a CUDA graph and replayed on the same buffers.  RFI_ESTATE if thresholds were never set; RFI_EINVAL for
  * NULL / misaligned (16 B) pointers; RFI_ECUDA if a launch failed. */
 int rfi_process_chunk(rfi_plan *plan, const void *d_vis, void *d_avg, void *d_weight,
                       void *d_stats, void *cuda_stream);

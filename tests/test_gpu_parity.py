@@ -415,3 +415,38 @@ def test_baseline_classes(mode):
         single, _ = run_gpu(w, vis, cross_sets[:1], "auto")
         assert (single["flags"][0][:, ~cell_auto] == out["flags"][0][:, ~cell_auto]).all()
         assert (single["flags"][0][:, cell_auto] != out["flags"][0][:, cell_auto]).mean() > 0.05
+
+
+# ------------------------------------------------------------------------------------------------------
+# CUDA graphs: after one warm-up call (lazy allocations), rfi_process_chunk is pure stream work and can be captured
+# ------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("K", [1, 6])
+def test_process_chunk_is_cuda_graph_capturable(K):
+    w = synth.WORKLOADS["tiny"]
+    thr = synth.default_thresholds(w.window_M) if K == 1 else synth.sweep_thresholds(w.window_M, K, seed=1)
+    vis_a, _ = synth.make_chunk(w, seed=1)
+    vis_b, _ = synth.make_chunk(w, seed=2)
+    plan = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M, n_int=w.n_int)
+    plan.set_thresholds(thr)
+    avg, weight, stats = plan.alloc_outputs(stats=True)
+    d_vis = vis_a.cuda()
+    plan.process_chunk(d_vis, avg, weight, stats)                 # warm-up: flag buffer, tensor map, attributes
+    torch.cuda.synchronize()
+    ref_a = (avg.clone(), weight.clone(), plan.get_flags().clone())
+    d_vis.copy_(vis_b.cuda())
+    plan.process_chunk(d_vis, avg, weight, stats)
+    torch.cuda.synchronize()
+    ref_b = (avg.clone(), weight.clone(), plan.get_flags().clone())
+    side = torch.cuda.Stream()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(graph, stream=side):
+            plan.process_chunk(d_vis, avg, weight, stats, stream=side)
+    for vis, ref in ((vis_a, ref_a), (vis_b, ref_b), (vis_a, ref_a)):
+        d_vis.copy_(vis.cuda())
+        avg.zero_(); weight.zero_()
+        torch.cuda.synchronize()
+        graph.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(avg, ref[0]) and torch.equal(weight, ref[1]) and torch.equal(plan.get_flags(), ref[2])
+    plan.destroy()
