@@ -188,6 +188,10 @@ def run_ours(args):
                        rfi.RFI_FP16 if w.fp16 else rfi.RFI_FP32, n_int=w.n_int)
     if w.window_F > 1:
         plan.set_window_freq(w.window_F)
+    if args.layout == "cell_major":
+        plan.set_layout("cell_major")
+        vis = vis.permute(1, 2, 0, 3, 4).contiguous()          # [b][c][t][pol][re,im]
+        args.no_e2e = True                                     # the host path is time-major only
     if args.arith == "tables":
         plan.set_arithmetic("tables", args.mask)
     two_classes = w.autos and args.classes
@@ -255,7 +259,7 @@ def run_ours(args):
     # the paper's SK-only / DS-only / BOTH comparison in one batched pass: disabling a detector is
     # a threshold at infinity (include/rfi.h).  Not timed.
     by_detector = None
-    if plan.K == 1 and args.arith == "fast" and rank == 0 and not two_classes:
+    if plan.K == 1 and args.arith == "fast" and rank == 0 and not two_classes and args.layout == "time_major":
         INF = float("inf")
         d0, lo0, hi0, g0 = thr[0]
         plan3 = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M,
@@ -336,7 +340,7 @@ def run_ours(args):
                    "n_stations": w.n_stations, "n_baselines": w.n_baselines, "n_chan": w.n_chan, "n_time": w.n_time,
                    "window_M": w.window_M, "window_F": w.window_F, "n_int": w.n_int, "K": max(plan.K, 1), "variant": variant,
                    "arithmetic": args.arith if args.arith == "fast" else f"tables, mask {args.mask:#06x}",
-                   "threshold_classes": 2 if two_classes else 1,
+                   "threshold_classes": 2 if two_classes else 1, "layout": args.layout,
                    "input_bytes": w.input_bytes,
                    "l2": ("L2 flushed between timed iterations (256 MB write, outside the timed events)" if small
                           else "input (>= 9 GB) is far larger than the 126 MB L2: no flush needed"),
@@ -366,6 +370,8 @@ def main():
     ap.add_argument("--arith", default="fast", choices=["fast", "tables"],
                     help="tables: the paper's Tables 1-2 literally, per-group precision from --mask (DESIGN.md section 11)")
     ap.add_argument("--mask", type=lambda x: int(x, 0), default=0x3C50, help="14-bit half-precision mask for --arith tables")
+    ap.add_argument("--layout", default="time_major", choices=["time_major", "cell_major"],
+                    help="cell_major: vis[b][c][t][pol] through the transposing tensor map (rfi_plan_set_layout)")
     ap.add_argument("--classes", action="store_true",
                     help="separate threshold class for the auto-correlations (rfi_plan_set_baseline_classes)")
     ap.add_argument("--no-e2e", action="store_true")

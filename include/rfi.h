@@ -77,6 +77,12 @@ enum {
     RFI_VARIANT_TABLES = 4    /* reported when the arithmetic mode is RFI_ARITH_TABLES */
 };
 
+/* input layouts (rfi_plan_set_layout) */
+enum {
+    RFI_LAYOUT_TIME_MAJOR = 0,   /* default: vis[t][b][c][pol], correlator dump order */
+    RFI_LAYOUT_CELL_MAJOR = 1    /* vis[b][c][t][pol]: each (baseline, channel) time series contiguous */
+};
+
 /* arithmetic modes (rfi_plan_set_arithmetic) */
 enum {
     RFI_ARITH_FAST   = 0,     /* default: all-single reformulation (centred SK moment, exact-zero guards) */
@@ -98,6 +104,13 @@ int rfi_plan_create(rfi_plan **out, int n_stations, int n_baselines, int n_chan,
 
 /* Samples per output integration: n_time % n_int == 0 and n_int % window_M == 0, else RFI_EINVAL. */
 int rfi_plan_set_integration(rfi_plan *plan, int n_int);
+
+/* Input layout.  RFI_LAYOUT_CELL_MAJOR reads vis[n_baselines][n_chan][n_time][4 pols][re,im] (e.g. after a corner
+ * turn): the TMA kernel stages 128-byte lines (4 fp32 / 8 fp16 samples) of 32 cells through a transposing tensor
+ * map, after which the arithmetic -- and therefore every output bit -- is that of the time-major TMA kernel.
+ * Outputs keep their layouts.  Restrictions (rfi_process_chunk returns RFI_EINVAL otherwise): K = 1,
+ * window_M % 4 == 0 (fp32) or % 8 == 0 (fp16), RFI_ARITH_FAST, device buffers (rfi_process_chunk_host rejects it). */
+int rfi_plan_set_layout(rfi_plan *plan, int layout);
 
 /* Per-baseline threshold classes.  Every baseline stream is mitigated separately and its null
  * statistics depend on the kind of stream: an auto-correlation is Hermitian with a large constant part, so its

@@ -21,7 +21,7 @@ ARITH_FAST, ARITH_TABLES = 0, 1
 MASK_PAPER_LEARNED = 0x3C50      # Tables 3-4: Table 1 groups 5,7 and Table 2 groups 4-7 in half
 
 EXPORTS = [
-    "rfi_plan_create", "rfi_plan_set_integration", "rfi_plan_set_baseline_shard", "rfi_plan_set_window_freq", "rfi_plan_set_arithmetic", "rfi_plan_set_baseline_classes", "rfi_set_thresholds",
+    "rfi_plan_create", "rfi_plan_set_integration", "rfi_plan_set_baseline_shard", "rfi_plan_set_window_freq", "rfi_plan_set_arithmetic", "rfi_plan_set_baseline_classes", "rfi_plan_set_layout", "rfi_set_thresholds",
     "rfi_plan_set_variant", "rfi_process_chunk", "rfi_get_flags", "rfi_confusion_counts", "rfi_process_chunk_host", "rfi_plan_destroy",
     "rfi_strerror", "rfi_last_cuda_error", "rfi_flags_bytes", "rfi_avg_bytes", "rfi_weight_bytes",
     "rfi_stats_bytes", "rfi_vis_bytes", "rfi_plan_launch_count", "rfi_plan_last_variant", "rfi_version",
@@ -65,6 +65,8 @@ def load_library(build_if_missing: bool = True):
     lib.rfi_plan_set_integration.argtypes = [vp, ci]
     lib.rfi_plan_set_baseline_shard.argtypes = [vp, ci, ci]
     lib.rfi_plan_set_window_freq.argtypes = [vp, ci]
+    lib.rfi_plan_set_layout.argtypes = [vp, ci]
+    lib.rfi_plan_set_layout.restype = ci
     lib.rfi_plan_set_baseline_classes.argtypes = [vp, ci, ctypes.c_char_p]
     lib.rfi_plan_set_baseline_classes.restype = ci
     lib.rfi_plan_set_arithmetic.argtypes = [vp, ci, ctypes.c_uint32]
@@ -141,6 +143,11 @@ class RfiPlan:
         """rfi_plan_set_window_freq: T x F footprints, W = window_M * F."""
         _check(self._lib.rfi_plan_set_window_freq(self._h, F), "rfi_plan_set_window_freq")
         self.window_F = F
+
+    def set_layout(self, layout):
+        """rfi_plan_set_layout: "time_major" (vis[t][b][c][pol], default) or "cell_major" (vis[b][c][t][pol])."""
+        v = {"time_major": 0, "cell_major": 1}[layout] if isinstance(layout, str) else int(layout)
+        _check(self._lib.rfi_plan_set_layout(self._h, v), "rfi_plan_set_layout")
 
     def set_arithmetic(self, mode, mask14: int = 0):
         """rfi_plan_set_arithmetic: "fast" (default) or "tables" (paper-literal Tables 1-2 with a 14-bit half-precision mask)."""

@@ -37,7 +37,7 @@ EncodeTiledFn get_encode_fn() {
 struct MapEntry {
     const void* ptr;
     int rows;
-    int R;
+    int R;                     // rows per box; -1: cell-major transposing map
     CUtensorMap map;
 };
 
@@ -45,6 +45,7 @@ struct MapEntry {
 
 struct rfi_plan {
     int n_stations, n_baselines, n_chan, n_time, M, precision, n_int;
+    int layout = RFI_LAYOUT_TIME_MAJOR;       // input layout
     int arith = RFI_ARITH_FAST;               // arithmetic mode
     uint32_t arith_mask = 0;                  // 14-bit precision mask of the tables mode
     int F = 1;                                // window extent in frequency (channels), W = M * F
@@ -131,7 +132,18 @@ int get_tensor_map(rfi_plan* p, const void* vis, int rows, int R, const CUtensor
     e.ptr = vis; e.rows = rows; e.R = R;
     CUresult rc;
     const size_t ncell = p->n_cells();
-    if (p->precision == RFI_FP32) {
+    if (R < 0) {
+        // cell-major vis[cell][t][sample]: {32 words = one 128-byte line = 4 (fp32) / 8 (fp16) samples of a cell,
+        // rows / samples-per-line, n_cells}; box {32, 1, 32 cells}; 128-byte swizzle
+        const size_t sb = p->sample_bytes();
+        cuuint64_t dims[3] = {32, (cuuint64_t)((size_t)rows * sb / 128), (cuuint64_t)ncell};
+        cuuint64_t strides[2] = {128, (cuuint64_t)rows * sb};
+        cuuint32_t box[3] = {32, 1, 32};
+        cuuint32_t estr[3] = {1, 1, 1};
+        rc = enc(&e.map, CU_TENSOR_MAP_DATA_TYPE_UINT32, 3, const_cast<void*>(vis), dims, strides, box, estr,
+                 CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                 CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    } else if (p->precision == RFI_FP32) {
         // {32 floats = 4 cells, n_cells/4 groups, rows}; box {32, 8, R}; 128-byte swizzle
         cuuint64_t dims[3] = {32, (cuuint64_t)(ncell / 4), (cuuint64_t)rows};
         cuuint64_t strides[2] = {128, (cuuint64_t)ncell * 32};
@@ -215,8 +227,8 @@ int enqueue_slab(rfi_plan* p, const void* d_vis_slab, int o_first, int n_out_sla
     const bool fp16 = p->precision == RFI_FP16;
     if (p->arith == RFI_ARITH_TABLES) {
         // paper-literal Tables 1-2: single-precision stream, per-channel windows, one threshold set
-        if (fp16 || p->F != 1 || p->K != 1) {
-            snprintf(g_cuda_err, sizeof(g_cuda_err), "tables arithmetic needs RFI_FP32 storage, F = 1 and K = 1");
+        if (fp16 || p->F != 1 || p->K != 1 || p->layout != RFI_LAYOUT_TIME_MAJOR) {
+            snprintf(g_cuda_err, sizeof(g_cuda_err), "tables arithmetic needs RFI_FP32 storage, F = 1, K = 1 and the time-major layout");
             return RFI_EINVAL;
         }
         kp.d = p->thr[0].d;
@@ -230,6 +242,20 @@ int enqueue_slab(rfi_plan* p, const void* d_vis_slab, int o_first, int n_out_sla
         kp.arith_mask = p->arith_mask;
         p->last_variant = RFI_VARIANT_TABLES;
         const int rc = launch_tables(kp, st);
+        if (rc == RFI_OK) p->launches++;
+        return rc;
+    }
+    if (p->layout == RFI_LAYOUT_CELL_MAJOR) {
+        const int R = fp16 ? 8 : 4;                       // samples per 128-byte line
+        if (p->K != 1 || p->M % R != 0 || n_out_slab != p->n_out()) {
+            snprintf(g_cuda_err, sizeof(g_cuda_err), "cell-major layout needs K = 1, window_M %% %d == 0 and device buffers", R);
+            return RFI_EINVAL;
+        }
+        const CUtensorMap* map = nullptr;
+        int rc = get_tensor_map(p, kp.vis, p->n_time, -1, &map);
+        if (rc != RFI_OK) return rc;
+        p->last_variant = RFI_VARIANT_TMA;
+        rc = launch_tma_cellmajor(fp16, kp, map, p->sm_count, p->smem_optin, st);
         if (rc == RFI_OK) p->launches++;
         return rc;
     }
@@ -353,6 +379,14 @@ int rfi_plan_set_baseline_classes(rfi_plan* p, int n_classes, const uint8_t* h_c
     return RFI_OK;
 }
 
+int rfi_plan_set_layout(rfi_plan* p, int layout) {
+    if (!p || (layout != RFI_LAYOUT_TIME_MAJOR && layout != RFI_LAYOUT_CELL_MAJOR)) return RFI_EINVAL;
+    p->layout = layout;
+    p->have_result = false;
+    p->maps.clear();
+    return RFI_OK;
+}
+
 int rfi_plan_set_window_freq(rfi_plan* p, int F) {
     if (!p || F < 1 || F > 32 || (F & (F - 1)) != 0 || p->n_chan % F != 0) return RFI_EINVAL;
     p->F = F;
@@ -438,6 +472,7 @@ int rfi_process_chunk_host(rfi_plan* p, const void* h_vis, void* h_avg, void* h_
     if (!p) return RFI_EINVAL;
     if (p->K < 1) return RFI_ESTATE;
     if (!h_vis || !h_avg || !h_weight || !h_flags) return RFI_EINVAL;
+    if (p->layout != RFI_LAYOUT_TIME_MAJOR) return RFI_EINVAL;   // integrations are contiguous slabs only in time-major order
     int rc = ensure_device(p);
     if (rc != RFI_OK) return rc;
     const size_t slab_bytes = (size_t)p->n_int * p->n_cells() * p->sample_bytes();

@@ -59,6 +59,8 @@ inline int pick_rows(int M, bool fp16, int cap = 8) {
 int launch_direct(bool fp16, const rfi::KParams& kp, cudaStream_t st);
 int launch_tma(bool fp16, const rfi::KParams& kp, const CUtensorMap* map, int R, int sm_count, int smem_optin,
                cudaStream_t st);
+int launch_tma_cellmajor(bool fp16, const rfi::KParams& kp, const CUtensorMap* map, int sm_count, int smem_optin,
+                         cudaStream_t st);
 int tma_rows(int M);                                   // rows per TMA stage for window length M
 int launch_batched(bool fp16, const rfi::KParams& kp, const rfi::BatchThr& bt, cudaStream_t st);
 int launch_tables(const rfi::KParams& kp, cudaStream_t st);

@@ -121,12 +121,20 @@ __global__ void __launch_bounds__(128, (FP16 || R <= 4) ? 4 : (R == 5 ? 3 : 2)) 
 //       chunk index is XORed with the 128-byte line index (mod 8), which makes the two 128-bit
 //       shared loads of a lane (32-byte stride between lanes) bank-conflict free.
 // fp16: 2-D tensor {n_cells*4 words, n_time}, box {128, R}: lanes read consecutive 16 B, no swizzle needed.
+//
+// CM = true: the CELL-MAJOR input layout vis[b][c][t][pol] (each cell's time series contiguous).  The same kernel
+// with a transposing tensor map: 3-D tensor {32 words = 128 B = R samples of one cell, n_time/R, n_cells}, box
+// {32, 1, 32 cells}, SWIZZLE_128B.  A stage is 32 lines of 128 B, line l = the R samples of the tile's cell l; lane l
+// reads its own line, chunk index XOR (l mod 8): conflict free per quarter warp.  After that a thread owns a cell
+// and R consecutive samples exactly as in the time-major kernels, so the results are bit-identical to them.
+// R is fixed by the 128-byte line: 4 (fp32) or 8 (fp16).
 // ------------------------------------------------------------------------------------------------
-template <int R, bool FP16>
+template <int R, bool FP16, bool CM = false>
 __global__ void __launch_bounds__(512, 1) rfi_tma_kernel(const __grid_constant__ CUtensorMap tmap,
                                                            const KParams p, const int stages) {
+    static_assert(!CM || R == (FP16 ? 8 : 4), "cell-major stages hold one 128-byte line per cell");
     constexpr int ROW_BYTES = FP16 ? 512 : 1024;
-    constexpr int STAGE_BYTES = R * ROW_BYTES;
+    constexpr int STAGE_BYTES = CM ? 4096 : R * ROW_BYTES;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = ((uint32_t)__cvta_generic_to_shared(smem_raw) + 1023u) & ~1023u;
 
@@ -167,8 +175,9 @@ __global__ void __launch_bounds__(512, 1) rfi_tma_kernel(const __grid_constant__
         const uint32_t bar = bars + 8 * s;
         const uint32_t dst = ring + (uint32_t)s * STAGE_BYTES;
         mbar_expect_tx(bar, STAGE_BYTES);
-        if constexpr (FP16) tma_load_2d(dst, &tmap, pr_tile * 128, pr_row0 + pr_blk * R, bar, pol);
-        else                tma_load_3d(dst, &tmap, 0, pr_tile * 8, pr_row0 + pr_blk * R, bar, pol);
+        if constexpr (CM)        tma_load_3d(dst, &tmap, 0, pr_row0 / R + pr_blk, pr_tile * 32, bar, pol);
+        else if constexpr (FP16) tma_load_2d(dst, &tmap, pr_tile * 128, pr_row0 + pr_blk * R, bar, pol);
+        else                     tma_load_3d(dst, &tmap, 0, pr_tile * 8, pr_row0 + pr_blk * R, bar, pol);
         ++pr_i;
         if (++pr_blk == bpu) { pr_blk = 0; pr_unit += GW; pr_locate(); }
     };
@@ -210,7 +219,15 @@ __global__ void __launch_bounds__(512, 1) rfi_tma_kernel(const __grid_constant__
                 const uint32_t sbase = ring + (uint32_t)stage * STAGE_BYTES;
                 Raw<FP16> buf[R];
 #pragma unroll
-                for (int r = 0; r < R; ++r) lds_raw(sbase + r * ROW_BYTES + off0, sbase + r * ROW_BYTES + off1, buf[r]);
+                for (int r = 0; r < R; ++r) {
+                    if constexpr (CM) {
+                        const uint32_t line = sbase + (uint32_t)lane * 128u, x = (uint32_t)lane & 7u;
+                        if constexpr (FP16) lds_raw(line + (((uint32_t)r ^ x) << 4), 0, buf[r]);
+                        else                lds_raw(line + (((uint32_t)(2 * r) ^ x) << 4), line + (((uint32_t)(2 * r + 1) ^ x) << 4), buf[r]);
+                    } else {
+                        lds_raw(sbase + r * ROW_BYTES + off0, sbase + r * ROW_BYTES + off1, buf[r]);
+                    }
+                }
                 __syncwarp();                                  // all lanes have read the stage into registers
                 if (lane == 0 && it + stages < total) pr_issue();
                 accumulate_block<R, FP16>(w, buf, b);

@@ -5,10 +5,10 @@
 namespace rfi_host {
 namespace {
 
-template <int R, bool FP16>
+template <int R, bool FP16, bool CM = false>
 int launch_r(const rfi::KParams& kp, const CUtensorMap* map, int sm_count, int smem_optin, cudaStream_t st) {
     const int row_bytes = FP16 ? 512 : 1024;
-    const int stage_bytes = R * row_bytes;
+    const int stage_bytes = CM ? 4096 : R * row_bytes;
     int warps = env_int("RFI_TMA_WARPS", 16);
     int stages = env_int("RFI_TMA_STAGES", 0);
     if (warps < 1) warps = 1;
@@ -26,7 +26,7 @@ int launch_r(const rfi::KParams& kp, const CUtensorMap* map, int sm_count, int s
     long grid = (n_units + warps - 1) / warps;
     const int ctas_per_sm = env_int("RFI_TMA_CTAS_PER_SM", 1);
     if (grid > (long)sm_count * ctas_per_sm) grid = (long)sm_count * ctas_per_sm;
-    auto kern = rfi::rfi_tma_kernel<R, FP16>;
+    auto kern = rfi::rfi_tma_kernel<R, FP16, CM>;
     RFI_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     kern<<<(unsigned)grid, warps * 32, smem, st>>>(*map, kp, stages);
     RFI_CUDA(cudaGetLastError());
@@ -48,6 +48,13 @@ int launch_f(const rfi::KParams& kp, const CUtensorMap* map, int R, int sm_count
 }
 
 }  // namespace
+
+// Cell-major input (vis[b][c][t][pol]): the same kernel behind a transposing tensor map; R = samples per 128-byte line.
+int launch_tma_cellmajor(bool fp16, const rfi::KParams& kp, const CUtensorMap* map, int sm_count, int smem_optin,
+                         cudaStream_t st) {
+    return fp16 ? launch_r<8, true, true>(kp, map, sm_count, smem_optin, st)
+                : launch_r<4, false, true>(kp, map, sm_count, smem_optin, st);
+}
 
 int tma_rows(int M) {
     const int cap = env_int("RFI_TMA_ROWS", 8);

@@ -450,3 +450,58 @@ def test_process_chunk_is_cuda_graph_capturable(K):
         torch.cuda.synchronize()
         assert torch.equal(avg, ref[0]) and torch.equal(weight, ref[1]) and torch.equal(plan.get_flags(), ref[2])
     plan.destroy()
+
+
+# ------------------------------------------------------------------------------------------------------
+# cell-major input layout vis[b][c][t][pol] (rfi_plan_set_layout): same arithmetic behind a transposing tensor map
+# ------------------------------------------------------------------------------------------------------
+def _run_cell_major(w, vis, thr, classes=None):
+    plan = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M,
+                       rfi.RFI_FP16 if w.fp16 else rfi.RFI_FP32, n_int=w.n_int)
+    if w.window_F > 1:
+        plan.set_window_freq(w.window_F)
+    plan.set_layout("cell_major")
+    plan.set_thresholds(thr)
+    avg, weight, st = plan.alloc_outputs(stats=True)
+    avg.fill_(float("nan")); weight.fill_(-1); st.fill_(float("nan"))
+    cm = vis.permute(1, 2, 0, 3, 4).contiguous().cuda()            # [b][c][t][pol][re,im]
+    plan.process_chunk(cm, avg, weight, st)
+    torch.cuda.synchronize()
+    out = gpu_outputs_to_numpy(plan, avg, weight, st, rfi.unpack_flags(plan.get_flags(), w.n_chan))
+    assert plan.last_variant == "tma" and plan.launch_count == 1
+    plan.destroy()
+    return out
+
+
+@pytest.mark.parametrize("fp16,M,n_chan,F", [(False, 16, 64, 1), (False, 4, 13 * 4, 1), (False, 64, 16, 1), (True, 16, 64, 1),
+                                            (True, 8, 24, 1), (False, 8, 20, 2), (False, 12, 45, 1)])
+def test_cell_major_layout(fp16, M, n_chan, F):
+    w = synth.Workload("cm", 5, True, n_chan, M * 24, M, M * 8, fp16=fp16, window_F=F, burst_cell_frac=0.15, channel_gain=True)
+    W = M * F
+    thr = synth.default_thresholds(W) if W >= 8 else [[1.0, 0.01, 2.0, 0.95]]
+    vis, _ = synth.make_chunk(w, seed=M + n_chan)
+    out = _run_cell_major(w, vis, thr)
+    v = vis.numpy().reshape(w.n_time, w.n_cells, 4, 2)
+    compare(v, M, w.n_int, thr, out, tol=2e-3 if fp16 else 1e-5, fp16=fp16, F=F)
+    # bit-identical to the time-major TMA kernel with the same block length
+    import os
+    os.environ["RFI_TMA_ROWS"] = "8" if fp16 else "4"
+    try:
+        if w.fp16 or w.n_cells % 4 == 0:
+            tm, used = run_gpu(w, vis, thr, "tma")
+            for key in ("avg", "weight", "flags", "tau", "r_re", "r_im"):
+                np.testing.assert_array_equal(out[key], tm[key])
+    finally:
+        del os.environ["RFI_TMA_ROWS"]
+
+
+def test_cell_major_rejects_unsupported_plans():
+    plan = rfi.RfiPlan(4, 10, 32, 60, 6)                            # window_M = 6 is not a multiple of 4
+    plan.set_layout("cell_major")
+    plan.set_thresholds([[1.0, 0.1, 1.0, 0.5]])
+    avg, weight, _ = plan.alloc_outputs()
+    vis = torch.zeros(10, 32, 60, 4, 2, device="cuda")
+    with pytest.raises(rfi.RfiError) as e:
+        plan.process_chunk(vis, avg, weight)
+    assert e.value.code == -1
+    plan.destroy()
