@@ -108,8 +108,9 @@ int rfi_plan_set_integration(rfi_plan *plan, int n_int);
 /* Input layout.  RFI_LAYOUT_CELL_MAJOR reads vis[n_baselines][n_chan][n_time][4 pols][re,im] (e.g. after a corner
  * turn): the TMA kernel stages 128-byte lines (4 fp32 / 8 fp16 samples) of 32 cells through a transposing tensor
  * map, after which the arithmetic -- and therefore every output bit -- is that of the time-major TMA kernel.
- * Outputs keep their layouts.  Restrictions (rfi_process_chunk returns RFI_EINVAL otherwise): K = 1,
- * window_M % 4 == 0 (fp32) or % 8 == 0 (fp16), RFI_ARITH_FAST, device buffers (rfi_process_chunk_host rejects it). */
+ * Outputs keep their layouts; K > 1 runs the batched kernel behind the same map.  Restrictions (rfi_process_chunk
+ * returns RFI_EINVAL otherwise): window_M % 4 == 0 (fp32) or % 8 == 0 (fp16), RFI_ARITH_FAST, device buffers
+ * (rfi_process_chunk_host rejects it). */
 int rfi_plan_set_layout(rfi_plan *plan, int layout);
 
 /* Per-baseline threshold classes.  Every baseline stream is mitigated separately and its null

@@ -247,17 +247,34 @@ int enqueue_slab(rfi_plan* p, const void* d_vis_slab, int o_first, int n_out_sla
     }
     if (p->layout == RFI_LAYOUT_CELL_MAJOR) {
         const int R = fp16 ? 8 : 4;                       // samples per 128-byte line
-        if (p->K != 1 || p->M % R != 0 || n_out_slab != p->n_out()) {
-            snprintf(g_cuda_err, sizeof(g_cuda_err), "cell-major layout needs K = 1, window_M %% %d == 0 and device buffers", R);
+        if (p->M % R != 0 || n_out_slab != p->n_out()) {
+            snprintf(g_cuda_err, sizeof(g_cuda_err), "cell-major layout needs window_M %% %d == 0 and device buffers", R);
             return RFI_EINVAL;
         }
         const CUtensorMap* map = nullptr;
         int rc = get_tensor_map(p, kp.vis, p->n_time, -1, &map);
         if (rc != RFI_OK) return rc;
-        p->last_variant = RFI_VARIANT_TMA;
-        rc = launch_tma_cellmajor(fp16, kp, map, p->sm_count, p->smem_optin, st);
-        if (rc == RFI_OK) p->launches++;
-        return rc;
+        if (p->K == 1) {
+            p->last_variant = RFI_VARIANT_TMA;
+            rc = launch_tma_cellmajor(fp16, kp, map, p->sm_count, p->smem_optin, st);
+            if (rc == RFI_OK) p->launches++;
+            return rc;
+        }
+        p->last_variant = RFI_VARIANT_BATCHED;
+        for (int k0 = 0; k0 < p->K; k0 += rfi::kMaxBatch) {
+            rfi::BatchThr bt;
+            memset(&bt, 0, sizeof(bt));
+            kp.k_first = k0;
+            kp.K = p->K - k0 < rfi::kMaxBatch ? p->K - k0 : rfi::kMaxBatch;
+            for (int k = 0; k < kp.K; ++k) {
+                bt.t[k] = to_device_thr(p->thr[(size_t)(k0 + k) * nc], p->M * p->F);
+                bt.t1[k] = to_device_thr(p->thr[(size_t)(k0 + k) * nc + nc - 1], p->M * p->F);
+            }
+            rc = launch_batched_tma_cellmajor(fp16, kp, bt, map, p->sm_count, p->smem_optin, st);
+            if (rc != RFI_OK) return rc;
+            p->launches++;
+        }
+        return RFI_OK;
     }
     if (p->K > 1) {
         // batched-threshold mode: all sets in one pass over the data, 64 sets per launch

@@ -75,13 +75,14 @@ __device__ __forceinline__ void lds128_head(uint32_t addr, float& a, float& b) {
     asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(a), "=f"(b), "=f"(c), "=f"(d) : "r"(addr));
 }
 
-template <int R, bool FP16, int SPW, bool FULLWORD>
+template <int R, bool FP16, int SPW, bool FULLWORD, bool CM = false>
 __global__ void __launch_bounds__(kBtWarps * 32, 1)
 rfi_batched_tma_kernel(const __grid_constant__ CUtensorMap tmap, const KParams p,
                        const __grid_constant__ BatchThr bt, const int stages) {
     constexpr int NW = kBtWarps;
     constexpr int ROW_BYTES = FP16 ? 512 : 1024;
-    constexpr int STAGE_BYTES = R * ROW_BYTES;
+    static_assert(!CM || R == (FP16 ? 8 : 4), "cell-major stages hold one 128-byte line per cell");
+    constexpr int STAGE_BYTES = CM ? 4096 : R * ROW_BYTES;   // CM: cell-major input, see rfi_tma_kernel
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = ((uint32_t)__cvta_generic_to_shared(smem_raw) + 1023u) & ~1023u;
 
@@ -125,8 +126,9 @@ rfi_batched_tma_kernel(const __grid_constant__ CUtensorMap tmap, const KParams p
         const uint32_t dst = ring + (uint32_t)s * STAGE_BYTES;
         const int row = pr_row0 + pr_wl * p.M + pr_b * R;
         mbar_expect_tx(bar, STAGE_BYTES);
-        if constexpr (FP16) tma_load_2d(dst, &tmap, pr_tile * 128, row, bar, pol);
-        else                tma_load_3d(dst, &tmap, 0, pr_tile * 8, row, bar, pol);
+        if constexpr (CM)        tma_load_3d(dst, &tmap, 0, row / R, pr_tile * 32, bar, pol);
+        else if constexpr (FP16) tma_load_2d(dst, &tmap, pr_tile * 128, row, bar, pol);
+        else                     tma_load_3d(dst, &tmap, 0, pr_tile * 8, row, bar, pol);
         ++pr_i;
         if (++pr_b == bpw) {
             pr_b = 0;
@@ -194,9 +196,19 @@ rfi_batched_tma_kernel(const __grid_constant__ CUtensorMap tmap, const KParams p
                     const uint32_t sbase = ring + (uint32_t)stage * STAGE_BYTES;
                     Raw<FP16> buf[R];
 #pragma unroll
-                    for (int r = 0; r < R; ++r) lds_raw(sbase + r * ROW_BYTES + off0, sbase + r * ROW_BYTES + off1, buf[r]);
+                    for (int r = 0; r < R; ++r) {
+                        if constexpr (CM) {
+                            const uint32_t line = sbase + (uint32_t)lane * 128u, sx = (uint32_t)lane & 7u;
+                            if constexpr (FP16) lds_raw(line + (((uint32_t)r ^ sx) << 4), 0, buf[r]);
+                            else                lds_raw(line + (((uint32_t)(2 * r) ^ sx) << 4), line + (((uint32_t)(2 * r + 1) ^ sx) << 4), buf[r]);
+                        } else {
+                            lds_raw(sbase + r * ROW_BYTES + off0, sbase + r * ROW_BYTES + off1, buf[r]);
+                        }
+                    }
+#pragma unroll
+                    for (int r = 0; r < R; ++r) loads_done(buf[r]);
                     __syncwarp();                              // all lanes hold the stage in registers
-                    if (lane == 0 && it + stages < total) pr_issue();
+                    if (lane == 0 && it + stages < total) { fence_proxy_async(); pr_issue(); }
                     accumulate_block<R, FP16>(w, buf, b);
                     ++it;
                     if (++stage == stages) { stage = 0; parity ^= 1u; }

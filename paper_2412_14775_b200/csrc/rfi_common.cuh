@@ -119,6 +119,13 @@ __device__ __forceinline__ void lds_raw(uint32_t a0, uint32_t, Raw<true>& r) {
     asm volatile("ld.shared.v4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(r.p[0]), "=r"(r.p[1]), "=r"(r.p[2]), "=r"(r.p[3]) : "r"(a0));
 }
 
+// Stage reuse (read by the generic proxy, then overwritten by the async proxy): make the warp's shared-memory loads
+// of a stage complete -- a register dependency on the last load of every row -- and order them before the TMA
+// refill with a proxy fence.  The data is needed by the very next instructions anyway, so this costs nothing.
+__device__ __forceinline__ void loads_done(const Raw<false>& r) { asm volatile("" ::"l"(r.p[3]) : "memory"); }
+__device__ __forceinline__ void loads_done(const Raw<true>& r) { asm volatile("" ::"r"(r.p[3]) : "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
 // Widen one sample to four fp32 (re,im) pairs: xx, xy, yx, yy (row-major Eq.(1)).
 __device__ __forceinline__ void widen(const Raw<false>& r, f2 (&x)[4]) {
 #pragma unroll

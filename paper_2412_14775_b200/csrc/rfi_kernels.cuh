@@ -228,8 +228,10 @@ __global__ void __launch_bounds__(512, 1) rfi_tma_kernel(const __grid_constant__
                         lds_raw(sbase + r * ROW_BYTES + off0, sbase + r * ROW_BYTES + off1, buf[r]);
                     }
                 }
+#pragma unroll
+                for (int r = 0; r < R; ++r) loads_done(buf[r]);
                 __syncwarp();                                  // all lanes have read the stage into registers
-                if (lane == 0 && it + stages < total) pr_issue();
+                if (lane == 0 && it + stages < total) { fence_proxy_async(); pr_issue(); }
                 accumulate_block<R, FP16>(w, buf, b);
                 ++it;
                 if (++stage == stages) { stage = 0; parity ^= 1u; }

@@ -505,3 +505,25 @@ def test_cell_major_rejects_unsupported_plans():
         plan.process_chunk(vis, avg, weight)
     assert e.value.code == -1
     plan.destroy()
+
+
+@pytest.mark.parametrize("fp16,n_chan,K", [(False, 64, 5), (True, 64, 20), (False, 24, 40)])
+def test_cell_major_layout_batched(fp16, n_chan, K):
+    """K > 1 behind the transposing tensor map: parity with the oracle and bit-identical to the time-major batched run."""
+    w = synth.Workload("cm_k", 5, True, n_chan, 16 * 40, 16, 16 * 20, fp16=fp16, burst_cell_frac=0.15, channel_gain=True)
+    thr = synth.sweep_thresholds(16, K, seed=K)
+    vis, _ = synth.make_chunk(w, seed=K)
+    plan = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M,
+                       rfi.RFI_FP16 if fp16 else rfi.RFI_FP32, n_int=w.n_int)
+    plan.set_layout("cell_major")
+    plan.set_thresholds(thr)
+    avg, weight, st = plan.alloc_outputs(stats=True)
+    plan.process_chunk(vis.permute(1, 2, 0, 3, 4).contiguous().cuda(), avg, weight, st)
+    torch.cuda.synchronize()
+    out = gpu_outputs_to_numpy(plan, avg, weight, st, rfi.unpack_flags(plan.get_flags(), w.n_chan))
+    assert plan.last_variant == "batched"
+    plan.destroy()
+    compare(vis.numpy().reshape(w.n_time, w.n_cells, 4, 2), 16, w.n_int, thr, out, tol=2e-3 if fp16 else 1e-5, fp16=fp16)
+    tm, _ = run_gpu(w, vis, thr, "auto")
+    for key in ("avg", "weight", "flags", "tau", "r_re", "r_im"):
+        np.testing.assert_array_equal(out[key], tm[key])
