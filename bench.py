@@ -12,6 +12,14 @@ N > 1 (launched by torchrun): the path shards by baseline with no data-path coll
 independent stream), so every rank processes its own chunk ("scaling": "weak"); the timed region
 is bracketed by a barrier and the time is the max over ranks.
 
+--scaling strong (N > 1) shards ONE chunk by baseline with rfi_plan_set_baseline_shard; the default
+"weak" gives every rank its own subband chunk.
+
+Besides the headline line (configs[1], fp32, K = 1) the default N = 1 run appends `configs`: one sub-record per
+BASELINE.json config (tiny, lofar_fp16, large, sweep K = 64) plus the paper's 10 x 2 footprint, each with best and
+median kernel time over the timed launches, samples/s, roofline fractions and a sampled-cell parity check against
+the oracle (verification outside every timed region).
+
 --impl reference times the fp64 CPU oracle (oracle/), as it stands, on the host cores.
 """
 from __future__ import annotations
@@ -119,9 +127,17 @@ def oracle_baseline(vis_np, w, thr, target_cpu_seconds=15.0):
     orc.process(sample, w.window_M, w.n_int, thr, n_threads=cores, want_stats=False)
     dt = time.perf_counter() - t0
     samples = use * vis_np.shape[0]
+    # "... plus a 1-thread figure" -- the same oracle, one thread, on a smaller slice of the same sample
+    use1 = int(max(64, min(use, 4.0 / max(per_cell_cpu, 1e-9))))
+    one = np.ascontiguousarray(sample[:, :use1])
+    t0 = time.perf_counter()
+    orc.process(one, w.window_M, w.n_int, thr, n_threads=1, want_stats=False)
+    dt1 = time.perf_counter() - t0
     return {"value": samples / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": f"{use} of {w.n_cells} cells x all {vis_np.shape[0]} time samples of the same chunk "
-                      f"({samples} samples, {dt:.2f} s wall, OpenMP over cells)"}
+                      f"({samples} samples, {dt:.2f} s wall, OpenMP over cells)",
+            "value_1thread": use1 * vis_np.shape[0] / dt1,
+            "sample_1thread": f"{use1} cells x all {vis_np.shape[0]} time samples, 1 thread, {dt1:.2f} s wall"}
 
 
 def run_reference(args):
@@ -162,6 +178,124 @@ def run_reference(args):
     }))
 
 
+def _pctl_stats(ms):
+    return {"kernel_ms_best": min(ms), "kernel_ms_median": statistics.median(ms), "kernel_ms_mean": statistics.mean(ms),
+            "launches_timed": len(ms)}
+
+
+def sampled_parity(w, plan, vis, truth, thr, avg, weight, stats, n_clean, n_rfi):
+    """Verification leg (outside every timed region): a seeded sample of cells of the chunk the timed kernel just
+    processed -- all time samples of each -- is brought back and compared with the fp64 oracle element by element
+    with the comparators and tolerances of tests/ (the logic of tests/test_gpu_full_size.py)."""
+    import numpy as np
+    import torch
+    import paper_2412_14775_b200 as rfi
+    from tests.parity_util import compare
+    K = max(plan.K, 1)
+    try:
+        g = torch.Generator().manual_seed(3)
+        tr = truth.reshape(plan.n_win, plan.n_cells)
+        has = tr.any(0).cpu()
+        r_cells, c_cells = torch.nonzero(has).flatten(), torch.nonzero(~has).flatten()
+        idx = torch.cat([r_cells[torch.randperm(r_cells.numel(), generator=g)[:n_rfi]],
+                         c_cells[torch.randperm(c_cells.numel(), generator=g)[:n_clean]]]).sort().values
+        if w.window_F > 1:                                  # whole footprints: the F channels of a window share a flag
+            F = w.window_F
+            idx = torch.unique((idx // F)[:, None] * F + torch.arange(F)[None, :]).sort().values
+        idx = idx.to(vis.device)
+        flags = rfi.unpack_flags(plan.get_flags(), w.n_chan).reshape(K, plan.n_win, plan.n_cells)
+        wt = weight.reshape(K, plan.n_out, plan.n_cells).long()
+        kept = (~flags).reshape(K, plan.n_out, w.n_int // w.window_M, plan.n_cells).sum(2) * w.window_M
+        weight_ok = bool(torch.equal(wt, kept))            # property at FULL size: weight = unflagged sample count
+        finite_ok = bool(torch.isfinite(avg).all())
+        sub = vis.reshape(w.n_time, plan.n_cells, 4, 2)[:, idx].cpu().numpy()
+        s = stats.reshape(3, plan.n_win, plan.n_cells)
+        out = {"avg": avg.reshape(K, plan.n_out, plan.n_cells, 4, 2)[:, :, idx].cpu().numpy().view(np.complex64).reshape(K, plan.n_out, -1, 4),
+               "weight": wt[:, :, idx].cpu().numpy(), "flags": flags[:, :, idx].cpu().numpy(),
+               "tau": s[0][:, idx].cpu().numpy(), "r_re": s[1][:, idx].cpu().numpy(), "r_im": s[2][:, idx].cpu().numpy()}
+        del flags, wt, kept
+        rep = compare(sub, w.window_M, w.n_int, thr, out, tol=2e-3 if w.fp16 else 1e-5, fp16=w.fp16, F=w.window_F)
+        ok = weight_ok and finite_ok
+        return {"status": "ok" if ok else "FAILED", "against": "fp64 oracle (oracle/), same seeded chunk",
+                "cells_sampled": int(idx.numel()), "windows_compared": rep["n_windows"] * K,
+                "tolerance": 2e-3 if w.fp16 else 1e-5, "flag_mismatch": rep["flag_mismatch"],
+                "flag_mismatch_near_threshold": rep["flag_mismatch_near_threshold"],
+                "flag_mismatch_unexplained": rep["flag_mismatch_unexplained"], "flag_agreement": rep["flag_agreement"],
+                "tau_worst_over_bound": rep.get("tau_worst_over_bound"), "r_re_worst_over_bound": rep.get("r_re_worst_over_bound"),
+                "avg_worst_over_bound": rep["avg_worst_over_bound"], "outputs_skipped": rep["outputs_skipped"],
+                "weight_equals_unflagged_samples_full_size": weight_ok, "avg_finite_full_size": finite_ok}
+    except AssertionError as exc:
+        return {"status": "FAILED", "error": str(exc)[:300]}
+
+
+def measure_config(name, K, dev, steps, warmup, peak, read_probe_gbs, vis=None, truth=None, n_clean=512, n_rfi=128):
+    """One sub-record of `configs`: generate (or reuse) the chunk, time `steps` launches one by one with CUDA events
+    after `warmup` untimed ones, then check a sample of cells against the oracle."""
+    import torch
+    import paper_2412_14775_b200 as rfi
+    from paper_2412_14775_b200 import synth
+    w = synth.WORKLOADS[name]
+    W = w.window_M * w.window_F
+    rec = {"workload": name, "baseline_config": (f"BASELINE.json configs[{synth.BASELINE_CONFIG_INDEX[name]}]"
+                                                 if name in synth.BASELINE_CONFIG_INDEX else "SURVEY 8(f) NEXT-1 (paper's 10 x 2 footprint)"),
+           "K": K, "storage": "f16" if w.fp16 else "f32", "window": f"{w.window_M} x {w.window_F}",
+           "input_bytes": w.input_bytes}
+    free = torch.cuda.mem_get_info(dev)[0]
+    need = (0 if vis is not None else w.input_bytes * 1.12) + 8e9
+    if free < need:
+        rec["skipped"] = f"needs {need / 1e9:.1f} GB of free device memory, {free / 1e9:.1f} GB available"
+        return rec
+    own = vis is None
+    if own:
+        vis, truth = synth.make_chunk(w, seed=1234, device=dev)
+    thr = synth.default_thresholds(W) if K <= 1 else synth.sweep_thresholds(W, K)
+    plan = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M,
+                       rfi.RFI_FP16 if w.fp16 else rfi.RFI_FP32, n_int=w.n_int)
+    if w.window_F > 1:
+        plan.set_window_freq(w.window_F)
+    plan.set_thresholds(thr)
+    avg, weight, stats = plan.alloc_outputs(device=dev, stats=True)
+    out_bytes = avg.numel() * 4 + weight.numel() * 4 + max(plan.K, 1) * plan.n_win * plan.n_baselines * plan.wpb * 4
+    algo = w.input_bytes + out_bytes
+    small = w.input_bytes < 4 * 126e6
+    flush = torch.empty(256 << 20, dtype=torch.int8, device=dev) if small else None
+    for _ in range(warmup):
+        plan.process_chunk(vis, avg, weight)
+    torch.cuda.synchronize(dev)
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    l0 = plan.launch_count
+    for a, b in evs:
+        if flush is not None:
+            flush.zero_()
+        a.record()
+        plan.process_chunk(vis, avg, weight)
+        b.record()
+    torch.cuda.synchronize(dev)
+    ms = [a.elapsed_time(b) for a, b in evs]
+    st = _pctl_stats(ms)
+    samples = w.n_time * w.n_cells
+    gbs_best, gbs_med = algo / (st["kernel_ms_best"] * 1e-3) / 1e9, algo / (st["kernel_ms_median"] * 1e-3) / 1e9
+    rec.update(variant=plan.last_variant, gpu_launches=int(plan.launch_count - l0), **st,
+               ms_per_step=st["kernel_ms_mean"], samples_per_s=samples / (st["kernel_ms_median"] * 1e-3),
+               algorithmic_bytes_per_launch=algo,
+               roofline={"bound": "hbm" if not small else "latency", "achieved": gbs_med, "achieved_best": gbs_best, "unit": "GB/s",
+                         "peak": peak, "frac": gbs_med / peak, "frac_of_nominal_8TBs": gbs_med / 8000.0,
+                         "frac_of_read_stream_probe": (gbs_med / read_probe_gbs) if read_probe_gbs else None},
+               l2=("L2 flushed between timed launches (256 MB write outside the events)" if small else "input far larger than the 126 MB L2"))
+    if small:
+        rec["latency_us"] = {"best": st["kernel_ms_best"] * 1e3, "median": st["kernel_ms_median"] * 1e3}
+    # one more launch with the statistics planes, then the sampled-cell oracle check (not timed)
+    plan.process_chunk(vis, avg, weight, stats)
+    torch.cuda.synchronize(dev)
+    rec["parity"] = sampled_parity(w, plan, vis, truth, thr, avg, weight, stats, n_clean, n_rfi)
+    plan.destroy()
+    del avg, weight, stats, flush
+    if own:
+        del vis, truth
+    torch.cuda.empty_cache()
+    return rec
+
+
 def run_ours(args):
     import numpy as np
     import torch
@@ -183,9 +317,18 @@ def run_ours(args):
     w = synth.WORKLOADS[args.workload]
     W = w.window_M * w.window_F
     thr = synth.default_thresholds(W) if args.K <= 1 else synth.sweep_thresholds(W, args.K)
-    vis, truth = synth.make_chunk(w, seed=1234 + rank, device=dev)
+    work = sharding.rank_work(w.n_baselines, world, rank, args.scaling)
+    vis, truth = synth.make_chunk(w, seed=work["seed"], device=dev)
     plan = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M,
                        rfi.RFI_FP16 if w.fp16 else rfi.RFI_FP32, n_int=w.n_int)
+    if work["sharded"]:
+        # strong scaling: every rank draws the SAME chunk and keeps its contiguous baseline range;
+        # the plan then processes b_count baselines (no exchange: PAPER.md:44, streams are mitigated separately)
+        b0, bc = work["b_first"], work["b_count"]
+        vis = vis[:, b0:b0 + bc].contiguous()
+        truth = truth.reshape(-1, w.n_baselines, w.n_chan)[:, b0:b0 + bc].reshape(truth.shape[0], -1).contiguous()
+        plan.set_baseline_shard(b0, bc)
+        torch.cuda.empty_cache()
     if w.window_F > 1:
         plan.set_window_freq(w.window_F)
     if args.layout == "cell_major":
@@ -204,8 +347,9 @@ def run_ours(args):
     plan.set_variant(args.variant)
     avg, weight, _ = plan.alloc_outputs(device=dev)
     out_bytes = avg.numel() * 4 + weight.numel() * 4 + max(plan.K, 1) * plan.n_win * plan.n_baselines * plan.wpb * 4
-    algo_bytes = w.input_bytes + out_bytes
-    samples = w.n_time * w.n_cells
+    in_bytes = vis.numel() * vis.element_size()            # this rank's input (the whole chunk unless sharded)
+    algo_bytes = in_bytes + out_bytes
+    samples = w.n_time * plan.n_cells
 
     def barrier():
         if dist is not None:
@@ -226,7 +370,7 @@ def run_ours(args):
     barrier()
     t_start = torch.cuda.Event(enable_timing=True); t_end = torch.cuda.Event(enable_timing=True)
     t_start.record()
-    small = w.input_bytes < 4 * 126e6                      # fits (or nearly fits) the 126 MB L2: flush between iterations
+    small = in_bytes < 4 * 126e6                           # fits (or nearly fits) the 126 MB L2: flush between iterations
     flush = torch.empty(256 << 20, dtype=torch.int8, device=dev) if small else None
     for a, b in evs:
         if flush is not None:
@@ -243,7 +387,9 @@ def run_ours(args):
     clocks = sampler.stop() if sampler else None
     total_ms = sharding.max_over_ranks(total_ms, device=dev)       # device-measured, MAX over ranks
     ms_per_step = total_ms / args.steps
-    value = world * samples / (ms_per_step * 1e-3)
+    total_samples = sharding.sum_scalar_over_ranks(samples, device=dev)      # weak: N chunks; strong: one chunk
+    total_algo = sharding.sum_scalar_over_ranks(algo_bytes, device=dev)
+    value = total_samples / (ms_per_step * 1e-3)
 
     # a little science on the way out (not timed): per-set detection quality against the injected ground truth
     # (BASELINE.json configs[4]; false-alarm / missed-detection probabilities of PAPER.md:235) via rfi_confusion_counts
@@ -259,7 +405,7 @@ def run_ours(args):
     # the paper's SK-only / DS-only / BOTH comparison in one batched pass: disabling a detector is
     # a threshold at infinity (include/rfi.h).  Not timed.
     by_detector = None
-    if plan.K == 1 and args.arith == "fast" and rank == 0 and not two_classes and args.layout == "time_major":
+    if plan.K == 1 and args.arith == "fast" and rank == 0 and not two_classes and args.layout == "time_major" and not work["sharded"]:
         INF = float("inf")
         d0, lo0, hi0, g0 = thr[0]
         plan3 = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M,
@@ -286,18 +432,40 @@ def run_ours(args):
     k_ms = statistics.mean(kernel_ms)
     achieved = algo_bytes / (k_ms * 1e-3) / 1e9
     variant = plan.last_variant
+    # like-for-like denominator for a one-touch READ stream, measured live on this device (rfi_probe_read_bandwidth):
+    # `peak` (MEASURED_PEAKS.json) is a read+write copy, which a read-only stream can exceed -- so `frac` may read > 1
+    try:
+        read_probe = rfi.probe_read_bandwidth(vis if in_bytes <= (40 << 30) else vis.reshape(-1)[: (40 << 30) // vis.element_size()])
+    except Exception:
+        read_probe = None
+    traffic = load_ncu_traffic(w.name, variant)
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": load_ncu_traffic(w.name, variant), "peak_source": peak_src,
+                "traffic": traffic,
+                "traffic_source": ("profiles/ncu_traffic.json (committed ncu --set full capture of this kernel on this workload; "
+                                   "not re-measured by this run)" if traffic is not None else None),
+                "peak_source": peak_src,
                 "kernel": f"rfi_{variant}_kernel", "kernel_ms_mean": k_ms, "kernel_ms_min": min(kernel_ms),
+                "kernel_ms_best": min(kernel_ms), "kernel_ms_median": statistics.median(kernel_ms),
+                "launches_timed": len(kernel_ms),
                 "algorithmic_bytes_per_launch": algo_bytes,
-                "frac_of_nominal_8TBs": achieved / 8000.0}
+                "frac_of_nominal_8TBs": achieved / 8000.0,
+                "read_stream_probe_gbs": read_probe,
+                "frac_of_read_stream_probe": (achieved / read_probe) if read_probe else None,
+                "note": "frac = achieved / MEASURED_PEAKS hbm_gbs, a read+write copy_ figure; this kernel is a read-only "
+                        "stream, so frac_of_read_stream_probe (same-device read-only probe) and frac_of_nominal_8TBs are the "
+                        "fractions that cannot exceed 1"}
 
     # end to end through the C ABI with HOST buffers (H2D of the inputs and D2H of the results inside the timed region)
     e2e = None
-    if not args.no_e2e and w.input_bytes > 32e9:
+    if args.no_e2e:
+        pass
+    elif work["sharded"]:
+        e2e = {"value": None, "unit": UNIT, "h2d_bytes_per_step": in_bytes, "d2h_bytes_per_step": out_bytes,
+               "skipped": "strong-scaling run: the end-to-end host path is measured by the N = 1 run"}
+    elif w.input_bytes > 32e9:
         e2e = {"value": None, "unit": UNIT, "h2d_bytes_per_step": w.input_bytes, "d2h_bytes_per_step": out_bytes,
                "skipped": "chunk larger than the pinned host memory this bench allows itself (32 GB)"}
-    elif not args.no_e2e:
+    else:
         try:
             h_vis = torch.empty(vis.shape, dtype=vis.dtype, pin_memory=True)
             h_vis.copy_(vis)
@@ -306,7 +474,7 @@ def run_ours(args):
             h_weight = torch.empty(weight.shape, dtype=torch.int32, pin_memory=True)
             h_flags = torch.empty(K, plan.n_win, plan.n_baselines, plan.wpb, dtype=torch.int32, pin_memory=True)
             plan.process_chunk_host_into(h_vis, h_avg, h_weight, h_flags)          # warm-up (allocates staging)
-            n_e2e = max(2, min(args.steps, 3))
+            n_e2e = max(5, min(args.steps, 6))               # >= 5 timed end-to-end steps (333 ms each on the lofar shape)
             t0 = time.perf_counter()
             for _ in range(n_e2e):
                 plan.process_chunk_host_into(h_vis, h_avg, h_weight, h_flags)      # synchronises before returning
@@ -330,10 +498,30 @@ def run_ours(args):
         idx = torch.randperm(w.n_cells, generator=g)[:n_s].sort().values.to(dev)
         sub = vis.reshape(w.n_time, w.n_cells, 4, 2)[:, idx].cpu().numpy()
         cpu = oracle_baseline(sub, w, thr)
+        del sub
+
+    # every BASELINE.json config in the SAME run: sub-records, each timed launch by launch with
+    # CUDA events (best and median over the launches) and parity-checked on sampled cells
+    configs = None
+    if (world == 1 and not args.no_configs and args.workload == "lofar" and args.K == 1 and args.arith == "fast"
+            and args.layout == "time_major" and not two_classes and args.variant == "auto"):
+        configs = []
+        n_sub = max(args.steps, 20)
+        plan.destroy()
+        del avg, weight
+        torch.cuda.empty_cache()
+        # configs[4] re-uses the resident lofar chunk (it IS "config 2 data")
+        configs.append(measure_config("sweep", 64, dev, n_sub, 3, peak, read_probe, vis=vis, truth=truth, n_clean=160, n_rfi=64))
+        del vis, truth
+        torch.cuda.empty_cache()
+        configs.append(measure_config("lofar_fp16", 1, dev, n_sub, 3, peak, read_probe))
+        configs.append(measure_config("lofar_tf10x2", 1, dev, n_sub, 3, peak, read_probe))
+        configs.append(measure_config("large", 1, dev, n_sub, 3, peak, read_probe, n_clean=256, n_rfi=256))
+        configs.append(measure_config("tiny", 1, dev, max(n_sub, 50), 5, peak, read_probe, n_clean=96, n_rfi=6))
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": args.scaling if world > 1 else "weak", "vs_baseline": None,
         "dtype": "f32" if not w.fp16 else "f32 (f16 storage)", "data": "synthetic (seeded; stands in for LOFAR data)",
         "config": {"workload": (f"{w.name}: BASELINE.json configs[{synth.BASELINE_CONFIG_INDEX[w.name]}]"
                                 if w.name in synth.BASELINE_CONFIG_INDEX else f"{w.name}: SURVEY 8(f) NEXT-1, not a BASELINE.json config"),
@@ -344,14 +532,17 @@ def run_ours(args):
                    "input_bytes": w.input_bytes,
                    "l2": ("L2 flushed between timed iterations (256 MB write, outside the timed events)" if small
                           else "input (>= 9 GB) is far larger than the 126 MB L2: no flush needed"),
-                   "sharding": "by baseline, no collective" if world > 1 else "single GPU"},
-        "gbytes_per_s": world * algo_bytes / (ms_per_step * 1e-3) / 1e9,
+                   "sharding": (("ONE chunk partitioned by baseline (rfi_plan_set_baseline_shard), no collective" if work["sharded"]
+                                 else "one subband chunk per rank, no collective") if world > 1 else "single GPU")},
+        "gbytes_per_s": total_algo / (ms_per_step * 1e-3) / 1e9,
         "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
         "detection": {"false_alarm": fa, "missed_detection": md, "flag_fraction": float(flag_frac[0]), "by_detector": by_detector,
                       "per_set": {"K": int(counts.shape[0]), "false_alarm_min_max": [float(p_fa.min()), float(p_fa.max())],
                                   "missed_detection_min_max": [float(p_md.min()), float(p_md.max())],
                                   "flag_fraction_min_max": [float(flag_frac.min()), float(flag_frac.max())]}},
     }
+    if configs is not None:
+        line["configs"] = configs
     print(json.dumps(line))
     if dist is not None:
         dist.barrier()
@@ -374,6 +565,9 @@ def main():
                     help="cell_major: vis[b][c][t][pol] through the transposing tensor map (rfi_plan_set_layout)")
     ap.add_argument("--classes", action="store_true",
                     help="separate threshold class for the auto-correlations (rfi_plan_set_baseline_classes)")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: weak = one chunk per rank; strong = ONE chunk sharded by baseline (rfi_plan_set_baseline_shard)")
+    ap.add_argument("--no-configs", action="store_true", help="skip the per-config sub-records of the default run")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

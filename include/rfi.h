@@ -44,6 +44,8 @@
  *
  * Errors: every function returns RFI_OK (0) or a negative code; nothing throws or aborts.
  * Threads: a plan is not internally locked; use one plan from one host thread at a time (different plans are independent).
+ * Devices: a plan binds to the CUDA device that is current at its first process call (its flag buffer, class table
+ * and staging buffers live there); a later process call with another device current returns RFI_EINVAL.
  */
 #ifndef RFI_H_
 #define RFI_H_
@@ -191,9 +193,19 @@ int rfi_process_chunk_host(rfi_plan *plan, const void *h_vis, void *h_avg, void 
 
 int rfi_plan_destroy(rfi_plan *plan);
 
+/* Diagnostics (not part of the method): read-only streaming bandwidth of the current device.  Reads `bytes` (>= 32,
+ * a multiple of 32 is used) of the 32-byte aligned device buffer d_buf once per launch with the 256-bit streaming
+ * load of the direct kernel, `repeats` timed launches after two warm-up launches, CUDA events on the stream;
+ * *h_ms_best (host) receives the best launch time in milliseconds.  Synchronises the stream.  The flag-and-average
+ * pass is a one-touch read stream (the correlator output is read once and averaged down), so this is
+ * the like-for-like denominator for its achieved GB/s; MEASURED_PEAKS.json's figure is a read+write copy. */
+int rfi_probe_read_bandwidth(const void *d_buf, size_t bytes, int repeats, float *h_ms_best, void *cuda_stream);
+
 /* helpers */
 const char *rfi_strerror(int code);
-const char *rfi_last_cuda_error(void);                 /* text of the last failed CUDA call (this thread) */
+const char *rfi_last_cuda_error(void);                 /* detail text of the last failed process call of this thread: the
+                                                          CUDA error string, or which shape rule an RFI_EINVAL broke;
+                                                          cleared at the start of every rfi_process_chunk* call */
 size_t rfi_flags_bytes(const rfi_plan *plan);          /* bytes of the flag mask for the current K */
 size_t rfi_avg_bytes(const rfi_plan *plan);            /* bytes the caller must provide for d_avg */
 size_t rfi_weight_bytes(const rfi_plan *plan);

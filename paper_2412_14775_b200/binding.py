@@ -25,6 +25,7 @@ EXPORTS = [
     "rfi_plan_set_variant", "rfi_process_chunk", "rfi_get_flags", "rfi_confusion_counts", "rfi_process_chunk_host", "rfi_plan_destroy",
     "rfi_strerror", "rfi_last_cuda_error", "rfi_flags_bytes", "rfi_avg_bytes", "rfi_weight_bytes",
     "rfi_stats_bytes", "rfi_vis_bytes", "rfi_plan_launch_count", "rfi_plan_last_variant", "rfi_version",
+    "rfi_probe_read_bandwidth",
 ]
 
 
@@ -38,7 +39,7 @@ class RfiError(RuntimeError):
         lib = load_library()
         msg = lib.rfi_strerror(code).decode()
         cuda = lib.rfi_last_cuda_error().decode()
-        super().__init__(f"{where}: {msg} ({code})" + (f" [{cuda}]" if code in (-2, -5) and cuda else ""))
+        super().__init__(f"{where}: {msg} ({code})" + (f" [{cuda}]" if cuda and where.startswith("rfi_process") else ""))
         self.code = code
 
 
@@ -78,6 +79,8 @@ def load_library(build_if_missing: bool = True):
     lib.rfi_confusion_counts.argtypes = [vp, vp, vp, vp]
     lib.rfi_confusion_counts.restype = ci
     lib.rfi_plan_destroy.argtypes = [vp]
+    lib.rfi_probe_read_bandwidth.argtypes = [vp, sz, ci, ctypes.POINTER(ctypes.c_float), vp]
+    lib.rfi_probe_read_bandwidth.restype = ci
     for name in ("rfi_plan_create", "rfi_plan_set_integration", "rfi_plan_set_baseline_shard",
                  "rfi_plan_set_window_freq", "rfi_plan_set_arithmetic", "rfi_set_thresholds", "rfi_plan_set_variant",
                  "rfi_process_chunk", "rfi_get_flags", "rfi_confusion_counts", "rfi_process_chunk_host", "rfi_plan_destroy",
@@ -209,6 +212,7 @@ class RfiPlan:
         if stats is not None and stats.numel() * 4 != self._lib.rfi_stats_bytes(self._h):
             raise ValueError("stats has the wrong size for this plan")
         s = stream if stream is not None else torch.cuda.current_stream(vis.device)
+        self._device = vis.device                         # the plan's flag buffer lives on this device
         _check(self._lib.rfi_process_chunk(self._h, vis.data_ptr(), avg.data_ptr(), weight.data_ptr(),
                                            stats.data_ptr() if stats is not None else None, s.cuda_stream),
                "rfi_process_chunk")
@@ -221,7 +225,7 @@ class RfiPlan:
         assert n.value == shape[0] * shape[1] * shape[2] * shape[3]
         iface = {"shape": (n.value,), "typestr": "<i4", "data": (ptr.value, False), "version": 2}
         holder = type("_FlagView", (), {"__cuda_array_interface__": iface})()
-        return torch.as_tensor(holder, device="cuda").view(shape)
+        return torch.as_tensor(holder, device=getattr(self, "_device", "cuda")).view(shape)
 
     def confusion_counts(self, truth_words: torch.Tensor, stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
         """rfi_confusion_counts: truth_words = pack_flags(bool truth) on the device; returns int64 [K, 4] on the device."""
@@ -272,6 +276,20 @@ class RfiPlan:
             self.destroy()
         except Exception:
             pass
+
+
+def probe_read_bandwidth(buf: torch.Tensor, repeats: int = 10) -> float:
+    """rfi_probe_read_bandwidth: read-only streaming GB/s of buf's device (diagnostics; the denominator that suits a
+    one-touch read stream).  buf: contiguous CUDA tensor, 32-byte aligned."""
+    if not (buf.is_cuda and buf.is_contiguous()):
+        raise ValueError("buf must be a contiguous CUDA tensor")
+    lib = load_library()
+    ms = ctypes.c_float()
+    nbytes = buf.numel() * buf.element_size()
+    with torch.cuda.device(buf.device):
+        _check(lib.rfi_probe_read_bandwidth(buf.data_ptr(), nbytes, repeats, ctypes.byref(ms),
+                                            torch.cuda.current_stream(buf.device).cuda_stream), "rfi_probe_read_bandwidth")
+    return (nbytes // 32 * 32) / (ms.value * 1e-3) / 1e9
 
 
 def unpack_flags(flags: torch.Tensor, n_chan: int) -> torch.Tensor:

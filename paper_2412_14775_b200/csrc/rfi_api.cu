@@ -21,16 +21,16 @@ using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t
                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
 EncodeTiledFn get_encode_fn() {
-    static EncodeTiledFn fn = nullptr;
-    static bool tried = false;
-    if (!tried) {
-        tried = true;
+    // function-local static: initialised exactly once, thread-safe (plans of different threads are independent)
+    static const EncodeTiledFn fn = []() -> EncodeTiledFn {
         void* p = nullptr;
         cudaDriverEntryPointQueryResult qres;
         if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
             qres == cudaDriverEntryPointSuccess)
-            fn = reinterpret_cast<EncodeTiledFn>(p);
-    }
+            return reinterpret_cast<EncodeTiledFn>(p);
+        cudaGetLastError();
+        return nullptr;
+    }();
     return fn;
 }
 
@@ -70,6 +70,7 @@ struct rfi_plan {
     std::vector<MapEntry> maps;
     // host path
     void* d_stage[2] = {nullptr, nullptr};
+    size_t d_stage_cap[2] = {0, 0};
     cudaStream_t streams[2] = {nullptr, nullptr};
     cudaEvent_t ev_copied[2] = {nullptr, nullptr};
     cudaEvent_t ev_done[2] = {nullptr, nullptr};
@@ -89,7 +90,17 @@ struct rfi_plan {
 namespace {
 
 int ensure_device(rfi_plan* p) {
-    if (p->dev_ready) return RFI_OK;
+    if (p->dev_ready) {
+        // a plan is bound to the device that was current at its first process call (its flag buffer, class table and
+        // staging buffers live there): refuse to run with another device current instead of faulting later
+        int cur = -1;
+        RFI_CUDA(cudaGetDevice(&cur));
+        if (cur != p->device) {
+            snprintf(g_cuda_err, sizeof(g_cuda_err), "plan is bound to CUDA device %d but device %d is current", p->device, cur);
+            return RFI_EINVAL;
+        }
+        return RFI_OK;
+    }
     int count = 0;
     if (cudaGetDeviceCount(&count) != cudaSuccess || count == 0) {
         cudaGetLastError();
@@ -120,9 +131,12 @@ rfi::Thr to_device_thr(const rfi_thresholds& t, int W) {
     return r;
 }
 
-int get_tensor_map(rfi_plan* p, const void* vis, int rows, int R, const CUtensorMap** out) {
+// The map is returned BY VALUE (it is consumed as a __grid_constant__ kernel parameter): no pointer into the cache
+// outlives an eviction.  Key: everything the encoding depends on that can change during a plan's life (the shard and
+// the layout clear the cache).
+int get_tensor_map(rfi_plan* p, const void* vis, int rows, int R, CUtensorMap* out) {
     for (auto& e : p->maps)
-        if (e.ptr == vis && e.rows == rows && e.R == R) { *out = &e.map; return RFI_OK; }
+        if (e.ptr == vis && e.rows == rows && e.R == R) { *out = e.map; return RFI_OK; }
     EncodeTiledFn enc = get_encode_fn();
     if (!enc) {
         snprintf(g_cuda_err, sizeof(g_cuda_err), "cuTensorMapEncodeTiled entry point not found");
@@ -168,7 +182,7 @@ int get_tensor_map(rfi_plan* p, const void* vis, int rows, int R, const CUtensor
     }
     if (p->maps.size() >= 16) p->maps.erase(p->maps.begin());
     p->maps.push_back(e);
-    *out = &p->maps.back().map;
+    *out = e.map;
     return RFI_OK;
 }
 
@@ -251,8 +265,9 @@ int enqueue_slab(rfi_plan* p, const void* d_vis_slab, int o_first, int n_out_sla
             snprintf(g_cuda_err, sizeof(g_cuda_err), "cell-major layout needs window_M %% %d == 0 and device buffers", R);
             return RFI_EINVAL;
         }
-        const CUtensorMap* map = nullptr;
-        int rc = get_tensor_map(p, kp.vis, p->n_time, -1, &map);
+        CUtensorMap map_v;
+        const CUtensorMap* map = &map_v;
+        int rc = get_tensor_map(p, kp.vis, p->n_time, -1, &map_v);
         if (rc != RFI_OK) return rc;
         if (p->K == 1) {
             p->last_variant = RFI_VARIANT_TMA;
@@ -282,10 +297,11 @@ int enqueue_slab(rfi_plan* p, const void* d_vis_slab, int o_first, int n_out_sla
         // same block length as the single-set direct kernel whenever that one uses R <= 4 (fp32) / 8 (fp16): then
         // K sets equal K single-set runs bit for bit
         const int R = pick_rows(p->M, fp16, fp16 ? 8 : 4);
-        const CUtensorMap* map = nullptr;
+        CUtensorMap map_v;
+        const CUtensorMap* map = &map_v;
         const bool use_tma = batched_tma_supported(fp16, kp, R) && tma_allowed(p);
         if (use_tma) {
-            const int rc = get_tensor_map(p, kp.vis, n_out_slab * p->n_int, R, &map);
+            const int rc = get_tensor_map(p, kp.vis, n_out_slab * p->n_int, R, &map_v);
             if (rc != RFI_OK) return rc;
         }
         for (int k0 = 0; k0 < p->K; k0 += rfi::kMaxBatch) {
@@ -307,16 +323,21 @@ int enqueue_slab(rfi_plan* p, const void* d_vis_slab, int o_first, int n_out_sla
     int variant = p->variant;
     // measured on B200 (profiles/): the register-staged direct kernel is the faster one for both storage types
     if (variant == RFI_VARIANT_AUTO) variant = RFI_VARIANT_DIRECT;
-    if (variant == RFI_VARIANT_TMA && !tma_allowed(p)) return RFI_EINVAL;
+    if (variant == RFI_VARIANT_TMA && !tma_allowed(p)) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err),
+                 "RFI_VARIANT_TMA with RFI_FP32 storage needs n_baselines * n_chan %% 4 == 0 (128-byte tensor-map rows); "
+                 "use RFI_VARIANT_AUTO or RFI_VARIANT_DIRECT for %zu cells", p->n_cells());
+        return RFI_EINVAL;
+    }
     p->last_variant = variant;
     int rc;
     if (variant == RFI_VARIANT_TMA) {
         const int rows = n_out_slab * p->n_int;
         const int R = tma_rows(p->M);
-        const CUtensorMap* map = nullptr;
-        rc = get_tensor_map(p, kp.vis, rows, R, &map);
+        CUtensorMap map_v;
+        rc = get_tensor_map(p, kp.vis, rows, R, &map_v);
         if (rc != RFI_OK) return rc;
-        rc = launch_tma(fp16, kp, map, R, p->sm_count, p->smem_optin, st);
+        rc = launch_tma(fp16, kp, &map_v, R, p->sm_count, p->smem_optin, st);
     } else {
         rc = launch_direct(fp16, kp, st);
     }
@@ -450,6 +471,7 @@ int rfi_plan_set_variant(rfi_plan* p, int variant) {
 }
 
 int rfi_process_chunk(rfi_plan* p, const void* d_vis, void* d_avg, void* d_weight, void* d_stats, void* cuda_stream) {
+    g_cuda_err[0] = 0;                        // rfi_last_cuda_error() describes THIS call if it fails
     if (!p) return RFI_EINVAL;
     if (p->K < 1) return RFI_ESTATE;
     if (!d_vis || !d_avg || !d_weight) return RFI_EINVAL;
@@ -486,6 +508,7 @@ int rfi_confusion_counts(rfi_plan* p, const uint32_t* d_truth, uint64_t* d_count
 
 int rfi_process_chunk_host(rfi_plan* p, const void* h_vis, void* h_avg, void* h_weight, void* h_flags,
                            void* h_stats) {
+    g_cuda_err[0] = 0;
     if (!p) return RFI_EINVAL;
     if (p->K < 1) return RFI_ESTATE;
     if (!h_vis || !h_avg || !h_weight || !h_flags) return RFI_EINVAL;
@@ -497,9 +520,6 @@ int rfi_process_chunk_host(rfi_plan* p, const void* h_vis, void* h_avg, void* h_
         if (!p->streams[i]) RFI_CUDA(cudaStreamCreateWithFlags(&p->streams[i], cudaStreamNonBlocking));
         if (!p->ev_copied[i]) RFI_CUDA(cudaEventCreateWithFlags(&p->ev_copied[i], cudaEventDisableTiming));
         if (!p->ev_done[i]) RFI_CUDA(cudaEventCreateWithFlags(&p->ev_done[i], cudaEventDisableTiming));
-        if (!p->d_stage[i]) {
-            if (cudaMalloc(&p->d_stage[i], slab_bytes) != cudaSuccess) { cudaGetLastError(); return RFI_ENOMEM; }
-        }
     }
     auto grow = [](auto*& ptr, size_t& cap, size_t need) -> int {
         if (need <= cap) return RFI_OK;
@@ -514,29 +534,42 @@ int rfi_process_chunk_host(rfi_plan* p, const void* h_vis, void* h_avg, void* h_
     if ((rc = grow(p->d_avg, p->d_avg_cap, rfi_avg_bytes(p))) != RFI_OK) return rc;
     if ((rc = grow(p->d_weight, p->d_weight_cap, rfi_weight_bytes(p))) != RFI_OK) return rc;
     if (h_stats && (rc = grow(p->d_stats, p->d_stats_cap, rfi_stats_bytes(p))) != RFI_OK) return rc;
+    // the staging slabs hold one integration of the CURRENT shape: rfi_plan_set_integration / _set_baseline_shard
+    // can enlarge it between calls (no work of a previous call is in flight here: every host call synchronises)
+    for (int i = 0; i < 2; ++i)
+        if ((rc = grow(p->d_stage[i], p->d_stage_cap[i], slab_bytes)) != RFI_OK) return rc;
 
     cudaStream_t copy_st = p->streams[0], comp_st = p->streams[1];
     rc = prepare(p, comp_st);
     if (rc != RFI_OK) return rc;
     const int n_out = p->n_out();
     const uint8_t* src = static_cast<const uint8_t*>(h_vis);
-    for (int o = 0; o < n_out; ++o) {
-        const int b = o & 1;
-        // the staging buffer is free once the kernel that read it (slab o-2) has finished
-        if (o >= 2) RFI_CUDA(cudaStreamWaitEvent(copy_st, p->ev_done[b], 0));
-        RFI_CUDA(cudaMemcpyAsync(p->d_stage[b], src + (size_t)o * slab_bytes, slab_bytes, cudaMemcpyHostToDevice, copy_st));
-        RFI_CUDA(cudaEventRecord(p->ev_copied[b], copy_st));
-        RFI_CUDA(cudaStreamWaitEvent(comp_st, p->ev_copied[b], 0));
-        rc = enqueue_slab(p, p->d_stage[b], o, 1, p->d_avg, p->d_weight, h_stats ? p->d_stats : nullptr, comp_st);
-        if (rc != RFI_OK) return rc;
-        RFI_CUDA(cudaEventRecord(p->ev_done[b], comp_st));
-    }
-    RFI_CUDA(cudaMemcpyAsync(h_avg, p->d_avg, rfi_avg_bytes(p), cudaMemcpyDeviceToHost, comp_st));
-    RFI_CUDA(cudaMemcpyAsync(h_weight, p->d_weight, rfi_weight_bytes(p), cudaMemcpyDeviceToHost, comp_st));
-    RFI_CUDA(cudaMemcpyAsync(h_flags, p->d_flags, rfi_flags_bytes(p), cudaMemcpyDeviceToHost, comp_st));
-    if (h_stats) RFI_CUDA(cudaMemcpyAsync(h_stats, p->d_stats, rfi_stats_bytes(p), cudaMemcpyDeviceToHost, comp_st));
-    RFI_CUDA(cudaStreamSynchronize(comp_st));
-    RFI_CUDA(cudaStreamSynchronize(copy_st));
+    // Every exit path below drains both internal streams first: no copy from (or to) the caller's host buffers is
+    // left in flight after the call returns, error or not.
+    auto pipeline = [&]() -> int {
+        for (int o = 0; o < n_out; ++o) {
+            const int b = o & 1;
+            // the staging buffer is free once the kernel that read it (slab o-2) has finished
+            if (o >= 2) RFI_CUDA(cudaStreamWaitEvent(copy_st, p->ev_done[b], 0));
+            RFI_CUDA(cudaMemcpyAsync(p->d_stage[b], src + (size_t)o * slab_bytes, slab_bytes, cudaMemcpyHostToDevice, copy_st));
+            RFI_CUDA(cudaEventRecord(p->ev_copied[b], copy_st));
+            RFI_CUDA(cudaStreamWaitEvent(comp_st, p->ev_copied[b], 0));
+            const int rc2 = enqueue_slab(p, p->d_stage[b], o, 1, p->d_avg, p->d_weight, h_stats ? p->d_stats : nullptr, comp_st);
+            if (rc2 != RFI_OK) return rc2;
+            RFI_CUDA(cudaEventRecord(p->ev_done[b], comp_st));
+        }
+        RFI_CUDA(cudaMemcpyAsync(h_avg, p->d_avg, rfi_avg_bytes(p), cudaMemcpyDeviceToHost, comp_st));
+        RFI_CUDA(cudaMemcpyAsync(h_weight, p->d_weight, rfi_weight_bytes(p), cudaMemcpyDeviceToHost, comp_st));
+        RFI_CUDA(cudaMemcpyAsync(h_flags, p->d_flags, rfi_flags_bytes(p), cudaMemcpyDeviceToHost, comp_st));
+        if (h_stats) RFI_CUDA(cudaMemcpyAsync(h_stats, p->d_stats, rfi_stats_bytes(p), cudaMemcpyDeviceToHost, comp_st));
+        return RFI_OK;
+    };
+    rc = pipeline();
+    const cudaError_t e1 = cudaStreamSynchronize(copy_st);
+    const cudaError_t e2 = cudaStreamSynchronize(comp_st);
+    if (rc != RFI_OK) return rc;
+    RFI_CUDA(e1);
+    RFI_CUDA(e2);
     p->have_result = true;
     return RFI_OK;
 }

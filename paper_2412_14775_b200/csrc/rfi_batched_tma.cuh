@@ -90,7 +90,9 @@ rfi_batched_tma_kernel(const __grid_constant__ CUtensorMap tmap, const KParams p
     const int warp = threadIdx.x >> 5;
     const uint32_t ring = smem_base + (uint32_t)warp * stages * STAGE_BYTES;
     const uint32_t rec_base = smem_base + (uint32_t)NW * stages * STAGE_BYTES;          // [2][NW][32 lanes][48 B]
-    const uint32_t bars = rec_base + 2u * NW * 32u * kRecBytes + (uint32_t)warp * stages * 8;
+    // per warp: `stages` "full" barriers followed by `stages` "empty" barriers (consumer -> producer hand-off)
+    const uint32_t bars = rec_base + 2u * NW * 32u * kRecBytes + (uint32_t)warp * stages * 16;
+    const uint32_t ebars = bars + (uint32_t)stages * 8;
 
     const int n_tiles = (p.n_cells + 31) >> 5;                // FULLWORD (n_chan % 32 == 0): whole tiles only; else the
                                                               // last tile is ragged (TMA zero-fills, invalid lanes are masked)
@@ -106,7 +108,7 @@ rfi_batched_tma_kernel(const __grid_constant__ CUtensorMap tmap, const KParams p
     const size_t flag_set_stride = (size_t)p.n_win_total * flag_words_per_win;
 
     if (lane == 0) {
-        for (int s = 0; s < stages; ++s) mbar_init(bars + 8 * s, 1);
+        for (int s = 0; s < stages; ++s) { mbar_init(bars + 8 * s, 1); mbar_init(ebars + 8 * s, 32); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
@@ -205,11 +207,14 @@ rfi_batched_tma_kernel(const __grid_constant__ CUtensorMap tmap, const KParams p
                             lds_raw(sbase + r * ROW_BYTES + off0, sbase + r * ROW_BYTES + off1, buf[r]);
                         }
                     }
-#pragma unroll
-                    for (int r = 0; r < R; ++r) loads_done(buf[r]);
-                    __syncwarp();                              // all lanes hold the stage in registers
-                    if (lane == 0 && it + stages < total) { fence_proxy_async(); pr_issue(); }
                     accumulate_block<R, FP16>(w, buf, b);
+                    // stage hand-off (rfi_common.cuh): 32 arrivals after consumption, then the producer's refill
+                    mbar_arrive(ebars + 8 * stage);
+                    if (lane == 0 && it + stages < total) {
+                        mbar_wait(ebars + 8 * stage, parity);
+                        fence_proxy_async();
+                        pr_issue();
+                    }
                     ++it;
                     if (++stage == stages) { stage = 0; parity ^= 1u; }
                 }

@@ -119,11 +119,14 @@ __device__ __forceinline__ void lds_raw(uint32_t a0, uint32_t, Raw<true>& r) {
     asm volatile("ld.shared.v4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(r.p[0]), "=r"(r.p[1]), "=r"(r.p[2]), "=r"(r.p[3]) : "r"(a0));
 }
 
-// Stage reuse (read by the generic proxy, then overwritten by the async proxy): make the warp's shared-memory loads
-// of a stage complete -- a register dependency on the last load of every row -- and order them before the TMA
-// refill with a proxy fence.  The data is needed by the very next instructions anyway, so this costs nothing.
-__device__ __forceinline__ void loads_done(const Raw<false>& r) { asm volatile("" ::"l"(r.p[3]) : "memory"); }
-__device__ __forceinline__ void loads_done(const Raw<true>& r) { asm volatile("" ::"r"(r.p[3]) : "memory"); }
+// Stage reuse (a stage is read by the generic proxy, then overwritten by the async proxy).  The hand-off is an
+// explicit consumer -> producer barrier: every lane arrives on the stage's "empty" mbarrier (count 32) AFTER it has
+// consumed the stage (mbarrier.arrive has release semantics: the lane's shared-memory reads are performed before the
+// arrival becomes visible), the producer lane waits on that barrier (acquire), orders the generic-proxy reads before
+// the async-proxy write with fence.proxy.async, and only then issues the TMA refill.
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.release.cta.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 // Widen one sample to four fp32 (re,im) pairs: xx, xy, yx, yy (row-major Eq.(1)).

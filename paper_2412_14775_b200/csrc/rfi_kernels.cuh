@@ -142,7 +142,9 @@ __global__ void __launch_bounds__(512, 1) rfi_tma_kernel(const __grid_constant__
     const int warp = threadIdx.x >> 5;
     const int nwarps = blockDim.x >> 5;
     const uint32_t ring = smem_base + (uint32_t)warp * stages * STAGE_BYTES;
-    const uint32_t bars = smem_base + (uint32_t)nwarps * stages * STAGE_BYTES + (uint32_t)warp * stages * 8;
+    // per warp: `stages` "full" barriers (count 1 + TMA bytes) followed by `stages` "empty" barriers (count 32)
+    const uint32_t bars = smem_base + (uint32_t)nwarps * stages * STAGE_BYTES + (uint32_t)warp * stages * 16;
+    const uint32_t ebars = bars + (uint32_t)stages * 8;
 
     const int n_tiles = (p.n_cells + 31) >> 5;
     const int n_units = n_tiles * p.n_out_slab;
@@ -156,7 +158,7 @@ __global__ void __launch_bounds__(512, 1) rfi_tma_kernel(const __grid_constant__
     const float inv_M = p.inv_W;                             // 1/W, W = T*F
 
     if (lane == 0) {
-        for (int s = 0; s < stages; ++s) mbar_init(bars + 8 * s, 1);
+        for (int s = 0; s < stages; ++s) { mbar_init(bars + 8 * s, 1); mbar_init(ebars + 8 * s, 32); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
@@ -228,11 +230,15 @@ __global__ void __launch_bounds__(512, 1) rfi_tma_kernel(const __grid_constant__
                         lds_raw(sbase + r * ROW_BYTES + off0, sbase + r * ROW_BYTES + off1, buf[r]);
                     }
                 }
-#pragma unroll
-                for (int r = 0; r < R; ++r) loads_done(buf[r]);
-                __syncwarp();                                  // all lanes have read the stage into registers
-                if (lane == 0 && it + stages < total) { fence_proxy_async(); pr_issue(); }
                 accumulate_block<R, FP16>(w, buf, b);
+                // hand the stage back: every lane arrives after consuming it, the producer lane waits for all 32
+                // arrivals (same phase parity as the fill it just consumed) before the async-proxy refill
+                mbar_arrive(ebars + 8 * stage);
+                if (lane == 0 && it + stages < total) {
+                    mbar_wait(ebars + 8 * stage, parity);
+                    fence_proxy_async();
+                    pr_issue();
+                }
                 ++it;
                 if (++stage == stages) { stage = 0; parity ^= 1u; }
             }

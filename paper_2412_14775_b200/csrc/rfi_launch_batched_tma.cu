@@ -15,9 +15,9 @@ int launch_rs(const rfi::KParams& kp, const rfi::BatchThr& bt, const CUtensorMap
     const int budget = smem_optin - 1024 - rec_bytes - 256;
     int stages = env_int("RFI_BT_STAGES", 0);
     if (stages <= 0) stages = 8;
-    while (stages > 1 && NW * stages * (stage_bytes + 8) > budget) --stages;
-    if (NW * stages * (stage_bytes + 8) > budget) return RFI_EINVAL;
-    const size_t smem = (size_t)NW * stages * (stage_bytes + 8) + rec_bytes + 1024;
+    while (stages > 1 && NW * stages * (stage_bytes + 16) > budget) --stages;
+    if (NW * stages * (stage_bytes + 16) > budget) return RFI_EINVAL;
+    const size_t smem = (size_t)NW * stages * (stage_bytes + 16) + rec_bytes + 1024;
     const int n_tiles = (kp.n_cells + 31) / 32;
     const long n_units = (long)n_tiles * kp.n_out_slab;
     long grid = n_units < sm_count ? n_units : sm_count;

@@ -15,12 +15,12 @@ int launch_r(const rfi::KParams& kp, const CUtensorMap* map, int sm_count, int s
     if (warps > 16) warps = 16;
     const int budget = smem_optin - 1024 - 256;
     if (stages <= 0) {
-        stages = budget / (warps * (stage_bytes + 8));
+        stages = budget / (warps * (stage_bytes + 16));
         if (stages > 6) stages = 6;
     }
-    while (stages > 1 && warps * stages * (stage_bytes + 8) > budget) --stages;
-    while (warps > 1 && warps * stages * (stage_bytes + 8) > budget) --warps;
-    const size_t smem = (size_t)warps * stages * (stage_bytes + 8) + 1024;
+    while (stages > 1 && warps * stages * (stage_bytes + 16) > budget) --stages;
+    while (warps > 1 && warps * stages * (stage_bytes + 16) > budget) --warps;
+    const size_t smem = (size_t)warps * stages * (stage_bytes + 16) + 1024;
     const int n_tiles = (kp.n_cells + 31) / 32;
     const long n_units = (long)n_tiles * kp.n_out_slab;
     long grid = (n_units + warps - 1) / warps;

@@ -23,6 +23,33 @@ def shard_baselines(n_baselines: int, world_size: int, rank: int) -> Tuple[int, 
     return first, q + (1 if rank < r else 0)
 
 
+def rank_work(n_baselines: int, world_size: int, rank: int, scaling: str = "weak", base_seed: int = 1234) -> dict:
+    """What `rank` processes in bench.py --gpus N.
+    weak:   every rank owns its own subband chunk (all baselines, seed base+rank) -- per-GPU work fixed.
+    strong: ONE chunk (seed base, the same on every rank) partitioned by baseline -- total work fixed; the rank's plan
+            is restricted with rfi_plan_set_baseline_shard(b_first, b_count).  world_size 1 is never sharded."""
+    if scaling not in ("weak", "strong"):
+        raise ValueError("scaling must be 'weak' or 'strong'")
+    if scaling == "strong" and world_size > 1:
+        b0, bc = shard_baselines(n_baselines, world_size, rank)
+        if bc < 1:
+            raise ValueError("more ranks than baselines")
+        return {"sharded": True, "b_first": b0, "b_count": bc, "seed": base_seed}
+    if not (0 <= rank < world_size):
+        raise ValueError("bad rank / world_size")
+    return {"sharded": False, "b_first": 0, "b_count": n_baselines, "seed": base_seed + rank}
+
+
+def sum_scalar_over_ranks(value, device=None, group=None) -> float:
+    """SUM all-reduce of a scalar (samples or bytes processed by each rank)."""
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()):
+        return float(value)
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.SUM, group=group)
+    return float(t.item())
+
+
 def max_over_ranks(value: float, device=None, group=None) -> float:
     """MAX all-reduce of a scalar (e.g. milliseconds measured with CUDA events on each rank)."""
     import torch.distributed as dist

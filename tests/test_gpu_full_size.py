@@ -7,7 +7,7 @@ import torch
 
 import paper_2412_14775_b200 as rfi
 from paper_2412_14775_b200 import synth
-from tests.parity_util import compare
+from tests.parity_util import compare, fp16_vs_fp32_original
 
 pytestmark = pytest.mark.gpu
 
@@ -22,19 +22,30 @@ def _sample_cells(w, truth, n_clean, n_rfi, seed):
     return pick.sort().values
 
 
-def _run_full(name, K, n_clean=768, n_rfi=256):
+def _run_full(name, K, n_clean=768, n_rfi=256, layout="time_major", vs_fp32_original=False):
     w = synth.WORKLOADS[name]
-    need = w.input_bytes * 1.15 + 6e9
+    need = w.input_bytes * (1.15 + (1.0 if layout == "cell_major" else 0.0) + (2.0 if vs_fp32_original else 0.0)) + 6e9
     if torch.cuda.mem_get_info()[0] < need:
         pytest.skip("not enough free device memory for the full-size chunk")
     dev = torch.device("cuda")
-    vis, truth = synth.make_chunk(w, seed=1234, device=dev)
+    sub32 = None
+    if vs_fp32_original:
+        # the same seeded chunk BEFORE rounding to half (make_chunk rounds as its last step)
+        vis32, truth = synth.make_chunk(w.scaled(fp16=False), seed=1234, device=dev)
+        vis = vis32.to(torch.float16)
+    else:
+        vis, truth = synth.make_chunk(w, seed=1234, device=dev)
     thr = synth.default_thresholds(w.window_M) if K == 1 else synth.sweep_thresholds(w.window_M, K)
     plan = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M,
                        rfi.RFI_FP16 if w.fp16 else rfi.RFI_FP32, n_int=w.n_int)
     plan.set_thresholds(thr)
     avg, weight, stats = plan.alloc_outputs(stats=True)
-    plan.process_chunk(vis, avg, weight, stats)                 # auto variant: what bench.py times
+    if layout == "cell_major":
+        plan.set_layout("cell_major")
+        d_in = vis.permute(1, 2, 0, 3, 4).contiguous()          # vis[b][c][t][pol][re,im]
+    else:
+        d_in = vis
+    plan.process_chunk(d_in, avg, weight, stats)                # auto variant: what bench.py times
     torch.cuda.synchronize()
     assert plan.launch_count == 1
     flags = rfi.unpack_flags(plan.get_flags(), w.n_chan).reshape(K, plan.n_win, plan.n_cells)
@@ -48,6 +59,9 @@ def _run_full(name, K, n_clean=768, n_rfi=256):
     # sampled cells against the oracle
     idx = _sample_cells(w, truth.reshape(plan.n_win, plan.n_cells), n_clean, n_rfi, seed=3).to(dev)
     sub = vis.reshape(w.n_time, plan.n_cells, 4, 2)[:, idx].cpu().numpy()
+    if vs_fp32_original:
+        sub32 = vis32.reshape(w.n_time, plan.n_cells, 4, 2)[:, idx].cpu().numpy()
+        del vis32
     out = {
         "avg": avg.reshape(K, plan.n_out, plan.n_cells, 4, 2)[:, :, idx].cpu().numpy().view(np.complex64).reshape(K, plan.n_out, -1, 4),
         "weight": wt[:, :, idx].cpu().numpy(),
@@ -56,9 +70,11 @@ def _run_full(name, K, n_clean=768, n_rfi=256):
     }
     used = plan.last_variant
     plan.destroy()
-    del vis, avg, weight, stats
+    del vis, d_in, avg, weight, stats
     torch.cuda.empty_cache()
     rep = compare(sub, w.window_M, w.n_int, thr, out, tol=2e-3 if w.fp16 else 1e-5, fp16=w.fp16)
+    if sub32 is not None:
+        rep.update(fp16_vs_fp32_original(sub32, w.window_M, w.n_int, thr, out))
     return rep, used
 
 
@@ -68,13 +84,32 @@ def test_lofar_fp32_full_size():
 
 
 def test_lofar_fp16_full_size():
-    rep, used = _run_full("lofar_fp16", 1)
+    """configs[2]: statistics against the oracle on the same fp16-rounded values (2e-3), and -- SURVEY 8(c)-T,
+    PAPER.md:251,269 -- flag agreement >= 99.9 % against the oracle on the ORIGINAL fp32 values."""
+    rep, used = _run_full("lofar_fp16", 1, vs_fp32_original=True)
+    print({k: rep[k] for k in ("flag_agreement", "flag_agreement_vs_fp32_original", "quantisation_dtau_max",
+                               "quantisation_dr_max", "outputs_skipped", "outputs_total")})
     assert rep["flag_agreement"] >= 0.999
+    assert rep["flag_agreement_vs_fp32_original"] >= 0.999
 
 
 def test_sweep_K64_full_size():
     rep, used = _run_full("sweep", 64, n_clean=192, n_rfi=64)
     assert used == "batched" and rep["K"] == 64 and rep["flag_mismatch_unexplained"] == 0
+
+
+def test_large_K64_full_size():
+    """configs[3] shape with the K = 64 sweep (DESIGN.md section 7 row "large K=64")."""
+    rep, used = _run_full("large", 64, n_clean=96, n_rfi=96)
+    assert used == "batched" and rep["K"] == 64 and rep["flag_mismatch_unexplained"] == 0
+
+
+@pytest.mark.parametrize("name,K", [("lofar", 1), ("lofar_fp16", 1), ("sweep", 64)])
+def test_cell_major_full_size(name, K):
+    """Cell-major input vis[b][c][t][pol] at the sizes bench.py times."""
+    rep, used = _run_full(name, K, n_clean=192, n_rfi=64, layout="cell_major")
+    assert used == ("tma" if K == 1 else "batched")
+    assert rep["flag_agreement"] >= 0.999 if synth.WORKLOADS[name].fp16 else rep["flag_mismatch_unexplained"] == 0
 
 
 def test_large_array_full_size():

@@ -8,13 +8,13 @@ import torch
 
 import paper_2412_14775_b200 as rfi
 from paper_2412_14775_b200 import synth
-from tests.parity_util import compare, gpu_outputs_to_numpy
+from tests.parity_util import compare, fp16_vs_fp32_original, gpu_outputs_to_numpy
 
 pytestmark = pytest.mark.gpu
 INF = float("inf")
 
 
-def run_gpu(w, vis, thresholds, variant="auto", stats=True):
+def run_gpu(w, vis, thresholds, variant="auto", stats=True, layout="time_major"):
     plan = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M,
                        rfi.RFI_FP16 if w.fp16 else rfi.RFI_FP32, n_int=w.n_int)
     if w.window_F > 1:
@@ -25,7 +25,11 @@ def run_gpu(w, vis, thresholds, variant="auto", stats=True):
     avg.fill_(float("nan")); weight.fill_(-1)
     if st is not None:
         st.fill_(float("nan"))
-    plan.process_chunk(vis.cuda(), avg, weight, st)
+    d_vis = vis.cuda()
+    if layout == "cell_major":                           # vis[b][c][t][pol] behind the transposing tensor map
+        plan.set_layout("cell_major")
+        d_vis = d_vis.permute(1, 2, 0, 3, 4).contiguous()
+    plan.process_chunk(d_vis, avg, weight, st)
     torch.cuda.synchronize()
     flags = rfi.unpack_flags(plan.get_flags(), w.n_chan)
     out = gpu_outputs_to_numpy(plan, avg, weight, st, flags)
@@ -35,11 +39,11 @@ def run_gpu(w, vis, thresholds, variant="auto", stats=True):
     return out, used
 
 
-def check(w, thresholds, variant, seed=1234, tol=None, mutate=None):
+def check(w, thresholds, variant, seed=1234, tol=None, mutate=None, layout="time_major"):
     vis, truth = synth.make_chunk(w, seed=seed, device="cpu")
     if mutate is not None:
         mutate(vis)
-    out, used = run_gpu(w, vis, thresholds, variant)
+    out, used = run_gpu(w, vis, thresholds, variant, layout=layout)
     if variant != "auto":
         assert used == variant
     v = vis.numpy().reshape(w.n_time, w.n_cells, 4, 2)
@@ -114,6 +118,14 @@ def test_fp16_storage(variant):
     # and the fp32-accumulate path on fp16 data is in fact as tight as the fp32 one
     vis, _ = synth.make_chunk(w, seed=1234)
     compare(vis.numpy().reshape(w.n_time, w.n_cells, 4, 2), 16, 256, synth.default_thresholds(16), out, tol=1e-5)
+    # against the oracle on the ORIGINAL fp32 values (the same seeded chunk before
+    # it is rounded to half) the flags must agree to >= 99.9 %; the statistic shifts are reported
+    vis32, _ = synth.make_chunk(w.scaled(fp16=False), seed=1234)
+    assert torch.equal(vis32.to(torch.float16), vis)
+    q = fp16_vs_fp32_original(vis32.numpy().reshape(w.n_time, w.n_cells, 4, 2), 16, 256, synth.default_thresholds(16), out)
+    print(f"fp16 storage vs fp32 originals [{variant}]: {q}; outputs skipped in the fp16 comparison: "
+          f"{rep['outputs_skipped']} of {rep['outputs_total']}")
+    assert q["flag_agreement_vs_fp32_original"] >= 0.999
 
 
 @pytest.mark.parametrize("variant", ["direct", "tma"])
@@ -141,6 +153,63 @@ def test_degenerate_inputs(variant):
     # detectors disabled: only the non-finite windows are flagged
     rep2, out2, _ = check(w, [[1.0, -INF, INF, INF]], variant, mutate=mutate)
     assert out2["flags"].sum() == 2
+
+
+# Reading G6 (non-finite input: the window is flagged by every set and contributes nothing) on every kernel family
+# that has its own code for it: the batched TMA kernel zeroes non-finite window sums before its fma-masked add
+# (whole-word and per-word flag stores), the register-staged batched kernel predicates its adds, fp16 storage widens
+# half NaN / Inf, the cell-major kernels read through the transposing map.  (name, n_stations, autos, n_chan, fp16, K, layout)
+_G6_CASES = [
+    ("batched_tma_fullword_K5", 4, True, 32, False, 5, "time_major"),
+    ("batched_tma_fullword_K64", 4, True, 32, False, 64, "time_major"),
+    ("batched_tma_perword_K5", 4, True, 16, False, 5, "time_major"),
+    ("batched_register_staged_ragged_K5", 3, False, 13, False, 5, "time_major"),     # 39 cells: n_cells % 4 != 0
+    ("batched_register_staged_ragged_K64", 3, False, 13, False, 64, "time_major"),
+    ("fp16_direct_K1", 4, True, 16, True, 1, "time_major"),
+    ("fp16_batched_K5", 4, True, 32, True, 5, "time_major"),
+    ("fp16_batched_K64", 4, True, 32, True, 64, "time_major"),
+    ("cell_major_K1", 4, True, 16, False, 1, "cell_major"),
+    ("cell_major_K5", 4, True, 32, False, 5, "cell_major"),
+    ("cell_major_fp16_K1", 4, True, 16, True, 1, "cell_major"),
+    ("cell_major_fp16_K17", 4, True, 32, True, 17, "cell_major"),
+]
+
+
+@pytest.mark.parametrize("name,n_st,autos,n_chan,fp16,K,layout", _G6_CASES, ids=[c[0] for c in _G6_CASES])
+def test_non_finite_and_degenerate_inputs_every_kernel_family(name, n_st, autos, n_chan, fp16, K, layout):
+    w = synth.Workload(name, n_st, autos, n_chan, 512, 16, 128, fp16=fp16, burst_cell_frac=0.2)
+    nc = w.n_cells
+
+    def mutate(vis):
+        v = vis.view(w.n_time, nc, 4, 2)
+        v[:, 5 % nc] = 0.0                                # all-zero cell
+        v[40:48, 7 % nc] = 0.0                            # zero samples inside a window
+        v[17, 9 % nc, 2, 1] = float("nan")
+        v[100, 11 % nc, 0, 0] = float("inf")
+        v[200, 12 % nc, 3, 1] = float("-inf")
+        v[300:303, 13 % nc] = float("nan")                # a run of NaN samples across all pols
+        v[317, nc - 1, 1, 0] = float("nan")               # last cell of the last (possibly ragged) tile
+        if fp16:
+            v[:, 20 % nc] *= 1e-3                         # subnormal halves (|x| < 6.1e-5)
+            v[64:80, 21 % nc, 0, 0] = 65504.0             # largest finite half
+            v[80:96, 21 % nc, 3, 0] = -65504.0
+            v[96, 22 % nc, 0, 0] = 65504.0                # one maximal sample among noise
+        else:
+            v[:, 20 % nc] *= 1e-12
+            v[:, 21 % nc] *= 1e12
+
+    bad = sorted({(17 // 16, 9 % nc), (100 // 16, 11 % nc), (200 // 16, 12 % nc), (300 // 16, 13 % nc), (317 // 16, nc - 1)})
+    thr = synth.sweep_thresholds(16, K, seed=3) if K > 1 else [[1.0, 0.1, 0.62, 0.52]]
+    rep, out, _ = check(w, thr, "auto", mutate=mutate, layout=layout)
+    assert rep["K"] == K
+    for k in range(K):
+        for (wi, c) in bad:
+            assert out["flags"][k][wi, c], f"set {k}: non-finite window ({wi}, cell {c}) not flagged"
+    assert np.isfinite(out["avg"]).all()                  # a non-finite window contributes nothing to any average
+    assert (out["weight"][:, :, 5 % nc] == 0).all()       # all-zero cell: tau = -c is below every s_low -> all flagged
+    # detectors disabled (thresholds at infinity): ONLY the non-finite windows are flagged, in every set
+    rep2, out2, _ = check(w, [[1.0, -INF, INF, INF]] * K, "auto", mutate=mutate, layout=layout)
+    assert out2["flags"].sum() == K * len(bad)
 
 
 @pytest.mark.parametrize("variant", ["direct", "tma"])
@@ -173,6 +242,45 @@ def test_host_path_equals_device_path():
     plan.destroy()
     for key in ("avg", "weight", "flags", "tau", "r_re", "r_im"):
         np.testing.assert_array_equal(out_dev[key], out_host[key])
+
+
+def test_host_path_staging_regrows_with_the_slab(K=1):
+    """VERDICT r01 / ADVICE: the host path's staging slabs hold one integration of the CURRENT shape.  A host call at
+    n_int = 256, then rfi_plan_set_integration(1024) (4x larger slab), then a shard that grows from 2 baselines to all:
+    every host call must equal the device path bit for bit (before the fix the second call copied past the slab)."""
+    w = synth.WORKLOADS["lofar"].scaled(n_stations=5, n_time=1024, n_int=256, burst_cell_frac=0.1)
+    vis, _ = synth.make_chunk(w, seed=21)
+    thr = synth.default_thresholds(16)
+    plan = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M, n_int=256)
+    plan.set_thresholds(thr)
+    plan.set_baseline_shard(0, 2)                         # smallest slab first: 2 baselines x 256 samples
+    shapes = [(0, 2, 256), (0, 2, 1024), (0, w.n_baselines, 1024), (3, 7, 512), (0, w.n_baselines, 256)]
+    for b0, bc, n_int in shapes:
+        plan.set_baseline_shard(b0, bc)
+        plan.set_integration(n_int)
+        sub = vis[:, b0:b0 + bc].contiguous()
+        ws = synth.Workload("host_regrow", w.n_stations, True, w.n_chan, w.n_time, w.window_M, n_int)
+        avg, weight, flags, stats = plan.process_chunk_host(sub.pin_memory(), want_stats=True)
+        host = gpu_outputs_to_numpy(plan, avg, weight, stats, rfi.unpack_flags(flags, w.n_chan))
+        d_avg, d_weight, d_stats = plan.alloc_outputs(stats=True)
+        plan.process_chunk(sub.cuda(), d_avg, d_weight, d_stats)
+        torch.cuda.synchronize()
+        dev = gpu_outputs_to_numpy(plan, d_avg, d_weight, d_stats, rfi.unpack_flags(plan.get_flags(), w.n_chan))
+        for key in ("avg", "weight", "flags", "tau", "r_re", "r_im"):
+            np.testing.assert_array_equal(host[key], dev[key], err_msg=f"{key} at shard ({b0},{bc}), n_int {n_int}")
+        compare(sub.numpy().reshape(w.n_time, bc * w.n_chan, 4, 2), 16, n_int, thr, host)
+    plan.destroy()
+
+
+def test_tma_variant_rejection_has_a_message():
+    plan = rfi.RfiPlan(3, 3, 13, 128, 16)
+    plan.set_thresholds(synth.default_thresholds(16)); plan.set_variant("tma")
+    avg, weight, _ = plan.alloc_outputs()
+    vis = torch.zeros(128, 3, 13, 4, 2, device="cuda")
+    with pytest.raises(rfi.RfiError) as e:
+        plan.process_chunk(vis, avg, weight)
+    assert e.value.code == -1 and "% 4" in rfi.load_library().rfi_last_cuda_error().decode()
+    plan.destroy()
 
 
 @pytest.mark.parametrize("K", [1, 5])

@@ -23,6 +23,23 @@ def test_shard_baselines_is_a_contiguous_balanced_partition(n, world):
         sharding.shard_baselines(n, world, world)
 
 
+def test_rank_work_weak_and_strong():
+    """bench.py --gpus N --scaling weak|strong: what each rank processes."""
+    for world in (1, 2, 4, 8):
+        weak = [sharding.rank_work(1176, world, r, "weak") for r in range(world)]
+        assert all(not x["sharded"] and x["b_count"] == 1176 for x in weak)
+        assert [x["seed"] for x in weak] == [1234 + r for r in range(world)]           # one subband chunk per rank
+        strong = [sharding.rank_work(1176, world, r, "strong") for r in range(world)]
+        assert sum(x["b_count"] for x in strong) == 1176                                # ONE chunk, partitioned
+        assert all(x["seed"] == 1234 for x in strong)
+        assert all(x["sharded"] == (world > 1) for x in strong)
+        assert [x["b_first"] for x in strong] == [sharding.shard_baselines(1176, world, r)[0] for r in range(world)]
+    with pytest.raises(ValueError):
+        sharding.rank_work(3, 8, 7, "strong")                                           # more ranks than baselines
+    with pytest.raises(ValueError):
+        sharding.rank_work(10, 2, 0, "diagonal")
+
+
 def test_confusion_counts_by_hand():
     flags = torch.tensor([[[1, 0, 1], [0, 0, 1]], [[0, 0, 0], [1, 1, 1]]]).bool()      # [K=2, W=2, cells=3]
     truth = torch.tensor([[1, 0, 0], [0, 0, 1]]).bool()
@@ -54,6 +71,12 @@ def _worker(rank, world, port, n_baselines, n_chan, n_win, K, out_dir):
         # device-time bookkeeping: MAX over ranks
         t = sharding.max_over_ranks(1.0 + rank)
         assert t == float(world)
+        # bench.py --scaling strong: the ranks' shards add up to the one chunk; weak: N chunks
+        ws = sharding.rank_work(n_baselines, world, rank, "strong")
+        assert (ws["b_first"], ws["b_count"]) == (b0, bc)
+        assert sharding.sum_scalar_over_ranks(ws["b_count"] * n_chan) == n_baselines * n_chan
+        ww = sharding.rank_work(n_baselines, world, rank, "weak")
+        assert sharding.sum_scalar_over_ranks(ww["b_count"] * n_chan) == world * n_baselines * n_chan
         dist.barrier()
         np.save(os.path.join(out_dir, f"ok{rank}.npy"), np.array([b0, bc]))
     finally:
