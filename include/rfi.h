@@ -193,6 +193,62 @@ int rfi_process_chunk_host(rfi_plan *plan, const void *h_vis, void *h_avg, void 
 
 int rfi_plan_destroy(rfi_plan *plan);
 
+/* ---------------------------------------------------------------------------------------------------------------
+ * Section-4.2 simulator: seeded synthetic blocks with injected RFI at a set
+ * interference-to-noise ratio, generated on the device.  One realisation = one simulated baseline = n_time x n_chan
+ * time-frequency samples (the paper: 2000 x 512, "about 1 s of data with about 200 kHz bandwidth");
+ * realisations sit on the baseline axis: d_vis is vis[n_time][n_real][n_chan][4][re,im] float, i.e. a chunk for a
+ * plan with n_baselines = n_real.  Per realisation (readings S1-S9 in DESIGN.md section 2):
+ *   noise     a * e_p e_q^H + sky: e_p, e_q ~ CN(0, I_2) station voltages per sample ("the conjugate product of the
+ *             two voltages"), sky ~ CN(0,1) per correlation, a = 100 U(0,1) constant over the block
+ *   sources   n_sources (200): (u,v,w) = 300 N(0,1); (l,m) ~ U(-0.5,0.5), n = sqrt(1-l^2-m^2); flux ~ U(1,10);
+ *             coherence flux * exp(j 2 pi f (ul+vm+w(n-1))/c), f_k = 120 MHz + k * 200 kHz / n_chan; unpolarised
+ *             (xx = yy = half the coherence, Eq.(2) has no 1/2), constant in time
+ *   RFI       n_broadband footprints [t0,t1) x [c0,c1) (sorted uniform edges) filled with ones; n_narrowband: one
+ *             channel, all times, exp(j 2 pi t / P), P = max(120 U(0,1), 2) samples; n_narrowdur: one time sample,
+ *             all channels, exp(j 2 pi c / P), P = max(1024 U(0,1), 2); each scaled by J/||J||, J = 4 draws of
+ *             CN(0,1) = (xx,xy,yx,yy); draws whose coherency J J^H (J as a 2x2 matrix) is more than 90 % polarised
+ *             are redrawn (<= 16 times); polarized = 0: J = (1,0,0,1)/sqrt(2) (Fig. 3(b))
+ *   mixing    data = celestial + g * rfi, g^2 = inr * P_celestial / P_rfi, P = total power over the block and the
+ *             four correlations; inr = 0 adds nothing
+ * d_truth (nullable): the window-level ground truth for rfi_confusion_counts, bit-packed like one
+ * set of the flag mask, [n_time/window_T][n_real][ceil(n_chan/32)]: bit c is set where the window_T x window_F
+ * footprint containing channel c holds an RFI point (needs window_T | n_time, window_F | n_chan).
+ * d_table / d_sources (nullable, diagnostics and tests): the per-realisation parameter table and the source coherence
+ * double[n_real][n_chan][re,im]; when NULL, work buffers are allocated internally and the call synchronises the stream,
+ * otherwise it only enqueues work.  Random numbers: Philox-4x32-10 keyed by `seed`, counter (index, 0, stream,
+ * realisation) -- every value is a pure function of its coordinates (the draw table is in oracle/sim42_oracle.py and
+ * csrc/rfi_sim42.cu).  The Gaussian transform of the noise runs in fp32, parameters and RFI phases in fp64.
+ * RFI_EINVAL (with rfi_last_cuda_error text) for sizes < 1, n_real > 65535, n_sources > 4096, more than
+ * RFI_SIM42_MAX_COMPONENTS RFI components, a negative or non-finite inr, a misaligned d_vis. */
+#define RFI_SIM42_MAX_COMPONENTS 16
+typedef struct {
+    int n_time, n_chan, n_real;                    /* block size and number of realisations */
+    int n_sources;                                 /* 200 in the paper */
+    int n_broadband, n_narrowband, n_narrowdur;    /* 5, 1, 1: "five broadband ... and two narrowband" (Fig. 2) */
+    int polarized;                                 /* 1: random J with the 90 % cut; 0: unpolarised RFI */
+    float inr;                                     /* interference-to-noise ratio (total power ratio) */
+    int window_T, window_F;                        /* footprint of the truth mask */
+    uint64_t seed;
+} rfi_sim42_config;
+typedef struct {
+    int kind;                                      /* 0 broadband, 1 narrowband (one channel), 2 narrow duration (one sample) */
+    int t0, t1, c0, c1;                            /* support [t0,t1) x [c0,c1) */
+    int tries;                                     /* J draws used (0 when unpolarised) */
+    double period;                                 /* samples; 0 for broadband */
+    double J[8];                                   /* J / ||J||: xx, xy, yx, yy as (re, im) */
+} rfi_sim42_component;
+typedef struct {
+    double a, u, v, w;                             /* receiver-noise scale; baseline coordinates (m) */
+    double p_cel, p_rfi, gain;                     /* total powers and g of the mixing step */
+    int n_comp, reserved;
+    rfi_sim42_component comp[RFI_SIM42_MAX_COMPONENTS];
+} rfi_sim42_realisation;
+int rfi_sim42_generate(const rfi_sim42_config *cfg, void *d_vis, uint32_t *d_truth,
+                       rfi_sim42_realisation *d_table, double *d_sources, void *cuda_stream);
+size_t rfi_sim42_vis_bytes(const rfi_sim42_config *cfg);      /* n_time * n_real * n_chan * 32 */
+size_t rfi_sim42_truth_bytes(const rfi_sim42_config *cfg);    /* (n_time/window_T) * n_real * ceil(n_chan/32) * 4 */
+
 /* Diagnostics (not part of the method): read-only streaming bandwidth of the current device.  Reads `bytes` (>= 32,
  * a multiple of 32 is used) of the 32-byte aligned device buffer d_buf once per launch with the 256-bit streaming
  * load of the direct kernel, `repeats` timed launches after two warm-up launches, CUDA events on the stream;

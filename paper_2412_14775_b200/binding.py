@@ -25,7 +25,7 @@ EXPORTS = [
     "rfi_plan_set_variant", "rfi_process_chunk", "rfi_get_flags", "rfi_confusion_counts", "rfi_process_chunk_host", "rfi_plan_destroy",
     "rfi_strerror", "rfi_last_cuda_error", "rfi_flags_bytes", "rfi_avg_bytes", "rfi_weight_bytes",
     "rfi_stats_bytes", "rfi_vis_bytes", "rfi_plan_launch_count", "rfi_plan_last_variant", "rfi_version",
-    "rfi_probe_read_bandwidth",
+    "rfi_probe_read_bandwidth", "rfi_sim42_generate", "rfi_sim42_vis_bytes", "rfi_sim42_truth_bytes",
 ]
 
 
@@ -34,12 +34,34 @@ class RfiThresholds(ctypes.Structure):
                 ("gamma", ctypes.c_float)]
 
 
+SIM42_MAX_COMPONENTS = 16
+
+
+class Sim42Config(ctypes.Structure):
+    """rfi_sim42_config (include/rfi.h): the section-4.2 simulator of the paper."""
+    _fields_ = [("n_time", ctypes.c_int), ("n_chan", ctypes.c_int), ("n_real", ctypes.c_int), ("n_sources", ctypes.c_int),
+                ("n_broadband", ctypes.c_int), ("n_narrowband", ctypes.c_int), ("n_narrowdur", ctypes.c_int),
+                ("polarized", ctypes.c_int), ("inr", ctypes.c_float), ("window_T", ctypes.c_int), ("window_F", ctypes.c_int),
+                ("seed", ctypes.c_uint64)]
+
+
+class Sim42Component(ctypes.Structure):
+    _fields_ = [("kind", ctypes.c_int), ("t0", ctypes.c_int), ("t1", ctypes.c_int), ("c0", ctypes.c_int), ("c1", ctypes.c_int),
+                ("tries", ctypes.c_int), ("period", ctypes.c_double), ("J", ctypes.c_double * 8)]
+
+
+class Sim42Realisation(ctypes.Structure):
+    _fields_ = [("a", ctypes.c_double), ("u", ctypes.c_double), ("v", ctypes.c_double), ("w", ctypes.c_double),
+                ("p_cel", ctypes.c_double), ("p_rfi", ctypes.c_double), ("gain", ctypes.c_double),
+                ("n_comp", ctypes.c_int), ("reserved", ctypes.c_int), ("comp", Sim42Component * SIM42_MAX_COMPONENTS)]
+
+
 class RfiError(RuntimeError):
     def __init__(self, code: int, where: str):
         lib = load_library()
         msg = lib.rfi_strerror(code).decode()
         cuda = lib.rfi_last_cuda_error().decode()
-        super().__init__(f"{where}: {msg} ({code})" + (f" [{cuda}]" if cuda and where.startswith("rfi_process") else ""))
+        super().__init__(f"{where}: {msg} ({code})" + (f" [{cuda}]" if cuda and where.startswith(("rfi_process", "rfi_sim42", "rfi_probe")) else ""))
         self.code = code
 
 
@@ -81,6 +103,11 @@ def load_library(build_if_missing: bool = True):
     lib.rfi_plan_destroy.argtypes = [vp]
     lib.rfi_probe_read_bandwidth.argtypes = [vp, sz, ci, ctypes.POINTER(ctypes.c_float), vp]
     lib.rfi_probe_read_bandwidth.restype = ci
+    lib.rfi_sim42_generate.argtypes = [ctypes.POINTER(Sim42Config), vp, vp, vp, vp, vp]
+    lib.rfi_sim42_generate.restype = ci
+    for name in ("rfi_sim42_vis_bytes", "rfi_sim42_truth_bytes"):
+        getattr(lib, name).argtypes = [ctypes.POINTER(Sim42Config)]
+        getattr(lib, name).restype = sz
     for name in ("rfi_plan_create", "rfi_plan_set_integration", "rfi_plan_set_baseline_shard",
                  "rfi_plan_set_window_freq", "rfi_plan_set_arithmetic", "rfi_set_thresholds", "rfi_plan_set_variant",
                  "rfi_process_chunk", "rfi_get_flags", "rfi_confusion_counts", "rfi_process_chunk_host", "rfi_plan_destroy",
@@ -276,6 +303,36 @@ class RfiPlan:
             self.destroy()
         except Exception:
             pass
+
+
+def sim42_generate(n_real: int, inr: float, seed: int = 1, n_time: int = 2000, n_chan: int = 512, n_sources: int = 200,
+                   n_broadband: int = 5, n_narrowband: int = 1, n_narrowdur: int = 1, polarized: bool = True,
+                   window_T: int = 10, window_F: int = 2, device="cuda", out: Optional[torch.Tensor] = None,
+                   diagnostics: bool = False):
+    """rfi_sim42_generate: the paper's section-4.2 simulator on the device.
+    Returns (vis [n_time, n_real, n_chan, 4, 2] float32, truth_words [n_time/window_T, n_real, ceil(n_chan/32)] int32)
+    and, with diagnostics=True, also the parameter table (list of Sim42Realisation) and the source coherence
+    [n_real, n_chan, 2] float64.  Argument marshalling only: every number is drawn and computed by the CUDA kernels."""
+    lib = load_library()
+    cfg = Sim42Config(n_time, n_chan, n_real, n_sources, n_broadband, n_narrowband, n_narrowdur, 1 if polarized else 0,
+                      float(inr), window_T, window_F, seed)
+    dev = torch.device(device)
+    vis = out if out is not None else torch.empty(n_time, n_real, n_chan, 4, 2, dtype=torch.float32, device=dev)
+    if not (vis.is_cuda and vis.is_contiguous() and vis.numel() * 4 == lib.rfi_sim42_vis_bytes(ctypes.byref(cfg))):
+        raise ValueError("out must be a contiguous CUDA float32 tensor of n_time * n_real * n_chan * 8 elements")
+    truth = torch.empty(n_time // window_T, n_real, (n_chan + 31) // 32, dtype=torch.int32, device=vis.device)
+    table = torch.empty(n_real * ctypes.sizeof(Sim42Realisation), dtype=torch.uint8, device=vis.device) if diagnostics else None
+    src = torch.empty(n_real, n_chan, 2, dtype=torch.float64, device=vis.device) if diagnostics else None
+    with torch.cuda.device(vis.device):
+        _check(lib.rfi_sim42_generate(ctypes.byref(cfg), vis.data_ptr(), truth.data_ptr(),
+                                      table.data_ptr() if diagnostics else None, src.data_ptr() if diagnostics else None,
+                                      torch.cuda.current_stream(vis.device).cuda_stream), "rfi_sim42_generate")
+    if not diagnostics:
+        return vis, truth
+    raw = table.cpu().numpy().tobytes()
+    n = ctypes.sizeof(Sim42Realisation)
+    tab = [Sim42Realisation.from_buffer_copy(raw[i * n:(i + 1) * n]) for i in range(n_real)]
+    return vis, truth, tab, src
 
 
 def probe_read_bandwidth(buf: torch.Tensor, repeats: int = 10) -> float:

@@ -19,7 +19,7 @@ ROOT = os.path.dirname(HERE)
 LIB = os.path.join(CSRC, "librfi.so")
 OBJ_DIR = os.path.join(CSRC, "build")
 SOURCES = [os.path.join(CSRC, f) for f in
-           ("rfi_api.cu", "rfi_launch_direct.cu", "rfi_launch_tma.cu", "rfi_launch_batched.cu", "rfi_launch_batched_tma.cu", "rfi_launch_tables.cu", "rfi_confusion.cu", "rfi_probe.cu")]
+           ("rfi_api.cu", "rfi_launch_direct.cu", "rfi_launch_tma.cu", "rfi_launch_batched.cu", "rfi_launch_batched_tma.cu", "rfi_launch_tables.cu", "rfi_confusion.cu", "rfi_probe.cu", "rfi_sim42.cu")]
 DEPS = SOURCES + sorted(glob.glob(os.path.join(CSRC, "*.cuh"))) + [
     os.path.join(CSRC, "rfi_internal.h"), os.path.join(ROOT, "include", "rfi.h")]
 
