@@ -148,7 +148,7 @@ def run_reference(args):
     import numpy as np
     from oracle import rfi_oracle as orc
     from paper_2412_14775_b200 import synth
-    w = synth.WORKLOADS[args.workload]
+    w = synth.WORKLOADS.get(args.workload, synth.WORKLOADS["lofar"])      # sim42 etc.: the reference arm times the lofar recipe
     thr = synth.default_thresholds(w.window_M)
     cores = orc.max_threads()
     # bounded sample: few stations of the same recipe, all time samples; sized so K+W steps end within minutes
@@ -294,6 +294,105 @@ def measure_config(name, K, dev, steps, warmup, peak, read_probe_gbs, vis=None, 
         del vis, truth
     torch.cuda.empty_cache()
     return rec
+
+
+def run_sim42(args):
+    """--workload sim42: the paper's 400-run FA/MD-vs-INR experiment (Fig. 3) on the device.
+    406 realisations (29 stations, cross baselines: the nearest triangular number above 400) of the 2000 x 512 block are
+    generated by rfi_sim42_generate at each INR, flagged with 10 x 2 footprints by ONE K-set launch whose sets are
+    {SK only, DS only, BOTH} x a ladder of design false-alarm rates (thresholds = empirical null quantiles on RFI-free
+    realisations of another seed), and scored by rfi_confusion_counts.  The timed step is the K-set flag+average pass."""
+    import torch
+    import paper_2412_14775_b200 as rfi
+    from paper_2412_14775_b200 import sharding
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    if int(os.environ.get("WORLD_SIZE", "1")) > 1:
+        raise RuntimeError("--workload sim42 is a single-GPU experiment")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    INF = float("inf")
+    R, T, C, wT, wF = 406, 2000, 512, 10, 2
+    fa_ladder = [0.001, 0.002, 0.005, 0.01, 0.02, 0.05, 0.1][: max(1, min(7, (max(args.K, 3)) // 3))] if args.K < 21 else \
+                [0.0005, 0.001, 0.002, 0.003, 0.005, 0.0075, 0.01, 0.015, 0.02, 0.03, 0.04, 0.05, 0.06, 0.075, 0.1, 0.125, 0.15, 0.2, 0.25, 0.3, 0.4]
+    plan = rfi.RfiPlan(29, R, C, T, wT, n_int=T)
+    plan.set_window_freq(wF)
+    vis = torch.empty(T, R, C, 4, 2, dtype=torch.float32, device=dev)
+    t0 = time.perf_counter()
+    rfi.sim42_generate(R, 0.0, seed=4242, out=vis)
+    torch.cuda.synchronize()
+    # null quantiles of the two statistics on RFI-free realisations (PAPER.md:229: thresholds from a design false-alarm rate)
+    plan.set_thresholds([[1.0, -INF, INF, INF]])
+    avg, weight, stats = plan.alloc_outputs(device=dev, stats=True)
+    plan.process_chunk(vis, avg, weight, stats)
+    s = stats.reshape(3, plan.n_win, R, C)[:, :, :, ::wF]
+    g = torch.Generator(device=dev).manual_seed(1)
+    idx = torch.randint(0, s[0].numel(), (4_000_000,), generator=g, device=dev)
+    tau, rmax = s[0].flatten()[idx], torch.maximum(s[1], s[2]).flatten()[idx]
+    sets, labels = [], []
+    for fa in fa_ladder:
+        lo, hi = float(torch.quantile(tau, fa / 2)), float(torch.quantile(tau, 1 - fa / 2))
+        gm = float(torch.quantile(rmax, 1 - fa))
+        sets += [[1.0, lo, hi, INF], [1.0, -INF, INF, gm], [1.0, lo, hi, gm]]
+        labels += [("sk", fa), ("ds", fa), ("both", fa)]
+    del avg, weight, stats, s, tau, rmax
+    plan.set_thresholds(sets)
+    K = len(sets)
+    avg, weight, _ = plan.alloc_outputs(device=dev)
+    inrs = [0.01, 0.1, 1.0, 10.0, 100.0, 1000.0]
+    curves, gen_ms, kernel_ms = {}, [], []
+    sampler = ClockSampler(0)
+    sampler.start()
+    for polarized in (True, False):
+        for inr in inrs:
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            _, truth = rfi.sim42_generate(R, inr, seed=777, polarized=polarized, out=vis)
+            b.record()
+            for _ in range(args.warmup if not kernel_ms else 0):
+                plan.process_chunk(vis, avg, weight)
+            evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(max(2, args.steps // 4))]
+            for x, y in evs:
+                x.record(); plan.process_chunk(vis, avg, weight); y.record()
+            counts = plan.confusion_counts(truth).cpu().double()
+            torch.cuda.synchronize()
+            gen_ms.append(a.elapsed_time(b)); kernel_ms += [x.elapsed_time(y) for x, y in evs]
+            fa_m, md_m = (counts[:, 0] / counts[:, 1].clamp(min=1)).tolist(), (counts[:, 2] / counts[:, 3].clamp(min=1)).tolist()
+            for k, (det, fa) in enumerate(labels):
+                curves.setdefault(("polarised" if polarized else "unpolarised"), {}).setdefault(f"design_fa_{fa}", {}) \
+                      .setdefault(det, []).append({"inr": inr, "false_alarm": round(fa_m[k], 5), "missed_detection": round(md_m[k], 5)})
+    clocks = sampler.stop()
+    peak, peak_src = load_peaks()
+    out_bytes = avg.numel() * 4 + weight.numel() * 4 + K * plan.n_win * R * plan.wpb * 4
+    algo = vis.numel() * 4 + out_bytes
+    k_med = statistics.median(kernel_ms)
+    samples = T * R * C
+    keep = [f"design_fa_{f}" for f in (0.01, 0.05) if f in fa_ladder] or [f"design_fa_{fa_ladder[0]}"]
+    line = {
+        "metric": METRIC, "value": samples / (k_med * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": len(kernel_ms), "warmup": args.warmup,
+        "ms_per_step": statistics.mean(kernel_ms), "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic: the paper's section-4.2 simulator (PAPER.md:219-237) generated on the device, seeded",
+        "config": {"workload": "sim42: SURVEY 8(f) NEXT-4, the FA/MD-vs-INR experiment of PAPER.md:235-237 (not a BASELINE.json config)",
+                   "n_realisations": R, "n_time": T, "n_chan": C, "window": f"{wT} x {wF}", "K": K, "variant": plan.last_variant,
+                   "sets": "{SK only, DS only, BOTH} x design false-alarm ladder " + str(fa_ladder),
+                   "input_bytes": vis.numel() * 4, "l2": "input (13.3 GB) is far larger than the 126 MB L2: no flush needed"},
+        "roofline": {"bound": "hbm", "achieved": algo / (k_med * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                     "frac": algo / (k_med * 1e-3) / 1e9 / peak, "traffic": None, "peak_source": peak_src,
+                     "kernel": "rfi_batched_tma_kernel", "kernel_ms_best": min(kernel_ms), "kernel_ms_median": k_med,
+                     "frac_of_nominal_8TBs": algo / (k_med * 1e-3) / 1e9 / 8000.0, "algorithmic_bytes_per_launch": algo},
+        "cpu_baseline": None, "e2e": None, "gpu_launches": int(plan.launch_count), "clocks": clocks,
+        "sim42": {"generator_ms_median": statistics.median(gen_ms), "generator_gbytes_per_s": vis.numel() * 4 / (statistics.median(gen_ms) * 1e-3) / 1e9,
+                  "paper_fig2_context": "INR 100, 10 x 2: SK 0.01/0.89, DS 0.01/0.06, BOTH 0.01/0.05 (FA/MD, PAPER.md:233)",
+                  "curves": {pol: {k: v for k, v in c.items() if k in keep} for pol, c in curves.items()},
+                  "roc_at_inr_100": {pol: {det: [{"design_fa": fa, **next(p for p in c[f"design_fa_{fa}"][det] if p["inr"] == 100.0)} for fa in fa_ladder]
+                                           for det in ("sk", "ds", "both")} for pol, c in curves.items()}},
+    }
+    for v in line["sim42"]["roc_at_inr_100"].values():
+        for pts in v.values():
+            for p in pts:
+                p.pop("inr", None)
+    print(json.dumps(line))
+    plan.destroy()
 
 
 def run_ours(args):
@@ -574,6 +673,10 @@ def main():
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         run_reference(args)
+    elif args.workload == "sim42":
+        if args.K <= 1:
+            args.K = 64
+        run_sim42(args)
     else:
         run_ours(args)
 

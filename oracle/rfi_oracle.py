@@ -70,6 +70,13 @@ def _load():
         lib.oracle_tables_process.restype = ctypes.c_int
         lib.oracle_tables_to_half.argtypes = [cf]
         lib.oracle_tables_to_half.restype = cf
+        lib.oracle_rl_record_doubles.argtypes = []
+        lib.oracle_rl_record_doubles.restype = ctypes.c_int
+        lib.oracle_rl_cost.argtypes = [cu, ctypes.c_int, c_dp, c_dp]
+        lib.oracle_rl_cost.restype = None
+        lib.oracle_rl_evaluate.argtypes = [ctypes.c_void_p, ctypes.c_int64, ctypes.c_int, cu, cf, cf, cf, cf, ctypes.c_double,
+                                           c_dp, ctypes.c_int]
+        lib.oracle_rl_evaluate.restype = ctypes.c_int
         lib.oracle_rfi_max_threads.argtypes = []
         lib.oracle_rfi_max_threads.restype = ctypes.c_int
         _lib = lib
@@ -207,3 +214,29 @@ def tables_process(vis, M: int, n_int: int, threshold, mask: int, n_threads: int
     if rc != 0:
         raise ValueError("oracle_tables_process: invalid arguments")
     return OracleResult(tau[None], r_re, r_im, flags[None], avg.view(np.complex128).reshape(1, n_out, n_cells, 4), weight[None])
+
+
+RL_FIELDS = {"features": slice(0, 10), "bits": slice(10, 24), "errors": slice(24, 45), "op_cost": 45, "conversions": 46,
+             "overflow": 47, "underflow": 48, "matches": 49, "reward": 50, "flags": 51}
+
+
+def rl_cost(mask: int, W: int):
+    """(operation cost, type conversions) of a precision mask for window size W (readings T10, T12)."""
+    c, v = ctypes.c_double(), ctypes.c_double()
+    _load().oracle_rl_cost(int(mask), int(W), ctypes.byref(c), ctypes.byref(v))
+    return c.value, v.value
+
+
+def rl_evaluate(windows, mask: int, threshold, rho: float = 3.0, n_threads: int = 0):
+    """The RL environment of PAPER.md:149-172 on windows float32 [n, W, 4, 2]: returns float64 [n, 52] records
+    (layout RL_FIELDS; readings T10-T15 in oracle/rfi_oracle_tables.cpp)."""
+    a = np.ascontiguousarray(windows, np.float32)
+    assert a.ndim == 4 and a.shape[2:] == (4, 2), a.shape
+    n, W = a.shape[0], a.shape[1]
+    rec = _load().oracle_rl_record_doubles()
+    out = np.empty((n, rec), np.float64)
+    d, lo, hi, g = [float(np.float32(x)) for x in threshold]
+    rc = _load().oracle_rl_evaluate(a.ctypes.data, n, W, int(mask), d, lo, hi, g, float(rho), _dp(out), int(n_threads))
+    if rc != 0:
+        raise ValueError("oracle_rl_evaluate: invalid arguments")
+    return out
