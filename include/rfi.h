@@ -194,6 +194,36 @@ int rfi_process_chunk_host(rfi_plan *plan, const void *h_vis, void *h_avg, void 
 int rfi_plan_destroy(rfi_plan *plan);
 
 /* ---------------------------------------------------------------------------------------------------------------
+ * The reinforcement-learning environment of section 3: one launch evaluates
+ * n_windows windows against ONE 14-bit precision mask (bit g-1: Table 1 group g in half; bit 7+g-1: Table 2 group g)
+ * so that an external soft-actor-critic loop (host side, out of scope) gets state, cost and reward for its batch.
+ *   d_windows  [n_windows][W][4 pols][re,im] float: each window's W = T x F samples contiguous (the
+ *              tables do not use the order of the samples beyond the order of their sums)
+ *   d_out      [n_windows][RFI_RL_RECORD_DOUBLES] double:
+ *              [0..9]   data features: log(sum_i part(X_i)^p)/W for (I,2), (I,4), (Q,2), (U,2), (V,2), real parts then
+ *                       imaginary parts, natural log, on the single-precision Stokes parameters
+ *              [10..23] the 14 precision bits
+ *              [24..44] the 21 errors: per group, mean over the group's outputs of |value in the chosen precisions -
+ *                       value with every operation in double| (+inf if not finite): Table 1 groups 1-7, Table 2 on the
+ *                       real parts groups 1-7, Table 2 on the imaginary parts groups 1-7 (group 7 of Table 2: the flag)
+ *              [45]     operation cost: cost column x C, C = 1 single / 0.6 half: Table 1 as printed
+ *                       (3W, W, W, W, 1, 1, 1+2), Table 2 groups 1-7 = 3W, W, 3W, 3W, 3, 4, 1, counted twice
+ *              [46]     type conversions (0.3 each): elements carried over data-flow edges whose ends differ in format
+ *              [47],[48] overflow / underflow events (exact result finite but rounded not; exact non-zero but rounded
+ *                       below the smallest normal number of the format)
+ *              [49]     how many of the three flags (SK, DS real, DS imaginary) equal the double-precision flags
+ *              [50]     reward = reward_per_match * [49] - [45] - 0.3 * [46] - 20 * ([47] + [48] > 0)     (
+ *                       the printed reward constant is garbled, hence the argument)
+ *              [51]     flags: mixed-precision (bit 0 SK, 1 DS real, 2 DS imaginary) + 8 * double-precision flags
+ * Thresholds (d, s_low, s_high, gamma) are read from host memory.  Every operation is an IEEE round-to-nearest
+ * operation of its group's format; eps = machine epsilon of the format (2^-52 for the ground truth); results equal the
+ * step-by-step CPU restatement (bit for bit except the libm-dependent logarithms of the features).  Asynchronous on the
+ * stream.  RFI_EINVAL for NULL / misaligned pointers, W < 2, mask bits above 13, d <= 0. */
+#define RFI_RL_RECORD_DOUBLES 52
+int rfi_rl_evaluate(const float *d_windows, int64_t n_windows, int W, uint32_t mask14,
+                    const rfi_thresholds *h_thr, double reward_per_match, double *d_out, void *cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------------------------
  * Section-4.2 simulator: seeded synthetic blocks with injected RFI at a set
  * interference-to-noise ratio, generated on the device.  One realisation = one simulated baseline = n_time x n_chan
  * time-frequency samples (the paper: 2000 x 512, "about 1 s of data with about 200 kHz bandwidth");

@@ -26,6 +26,7 @@ EXPORTS = [
     "rfi_strerror", "rfi_last_cuda_error", "rfi_flags_bytes", "rfi_avg_bytes", "rfi_weight_bytes",
     "rfi_stats_bytes", "rfi_vis_bytes", "rfi_plan_launch_count", "rfi_plan_last_variant", "rfi_version",
     "rfi_probe_read_bandwidth", "rfi_sim42_generate", "rfi_sim42_vis_bytes", "rfi_sim42_truth_bytes",
+    "rfi_rl_evaluate",
 ]
 
 
@@ -61,7 +62,7 @@ class RfiError(RuntimeError):
         lib = load_library()
         msg = lib.rfi_strerror(code).decode()
         cuda = lib.rfi_last_cuda_error().decode()
-        super().__init__(f"{where}: {msg} ({code})" + (f" [{cuda}]" if cuda and where.startswith(("rfi_process", "rfi_sim42", "rfi_probe")) else ""))
+        super().__init__(f"{where}: {msg} ({code})" + (f" [{cuda}]" if cuda and where.startswith(("rfi_process", "rfi_sim42", "rfi_probe", "rfi_rl")) else ""))
         self.code = code
 
 
@@ -103,6 +104,8 @@ def load_library(build_if_missing: bool = True):
     lib.rfi_plan_destroy.argtypes = [vp]
     lib.rfi_probe_read_bandwidth.argtypes = [vp, sz, ci, ctypes.POINTER(ctypes.c_float), vp]
     lib.rfi_probe_read_bandwidth.restype = ci
+    lib.rfi_rl_evaluate.argtypes = [vp, ctypes.c_int64, ci, ctypes.c_uint32, ctypes.POINTER(RfiThresholds), ctypes.c_double, vp, vp]
+    lib.rfi_rl_evaluate.restype = ci
     lib.rfi_sim42_generate.argtypes = [ctypes.POINTER(Sim42Config), vp, vp, vp, vp, vp]
     lib.rfi_sim42_generate.restype = ci
     for name in ("rfi_sim42_vis_bytes", "rfi_sim42_truth_bytes"):
@@ -303,6 +306,28 @@ class RfiPlan:
             self.destroy()
         except Exception:
             pass
+
+
+RL_RECORD_DOUBLES = 52
+RL_FIELDS = {"features": slice(0, 10), "bits": slice(10, 24), "errors": slice(24, 45), "op_cost": 45, "conversions": 46,
+             "overflow": 47, "underflow": 48, "matches": 49, "reward": 50, "flags": 51}
+
+
+def rl_evaluate(windows: torch.Tensor, mask14: int, threshold, reward_per_match: float = 3.0,
+                out: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """rfi_rl_evaluate: the RL environment of PAPER.md:149-172 for a batch of windows and one precision mask.
+    windows: contiguous CUDA float32 [n, W, 4, 2]; returns float64 [n, 52] (layout RL_FIELDS / include/rfi.h)."""
+    if not (windows.is_cuda and windows.is_contiguous() and windows.dtype == torch.float32 and windows.dim() == 4
+            and tuple(windows.shape[2:]) == (4, 2)):
+        raise ValueError("windows must be a contiguous CUDA float32 tensor [n, W, 4, 2]")
+    n, W = windows.shape[0], windows.shape[1]
+    rec = out if out is not None else torch.empty(n, RL_RECORD_DOUBLES, dtype=torch.float64, device=windows.device)
+    thr = RfiThresholds(*map(float, threshold))
+    with torch.cuda.device(windows.device):
+        _check(load_library().rfi_rl_evaluate(windows.data_ptr(), n, W, int(mask14), ctypes.byref(thr), float(reward_per_match),
+                                              rec.data_ptr(), torch.cuda.current_stream(windows.device).cuda_stream),
+               "rfi_rl_evaluate")
+    return rec
 
 
 def sim42_generate(n_real: int, inr: float, seed: int = 1, n_time: int = 2000, n_chan: int = 512, n_sources: int = 200,

@@ -19,9 +19,13 @@ ROOT = os.path.dirname(HERE)
 LIB = os.path.join(CSRC, "librfi.so")
 OBJ_DIR = os.path.join(CSRC, "build")
 SOURCES = [os.path.join(CSRC, f) for f in
-           ("rfi_api.cu", "rfi_launch_direct.cu", "rfi_launch_tma.cu", "rfi_launch_batched.cu", "rfi_launch_batched_tma.cu", "rfi_launch_tables.cu", "rfi_confusion.cu", "rfi_probe.cu", "rfi_sim42.cu")]
-DEPS = SOURCES + sorted(glob.glob(os.path.join(CSRC, "*.cuh"))) + [
+           ("rfi_api.cu", "rfi_launch_direct.cu", "rfi_launch_tma.cu", "rfi_launch_batched.cu", "rfi_launch_batched_tma.cu", "rfi_launch_tables.cu", "rfi_launch_tables_ps0.cu", "rfi_launch_tables_ps1.cu", "rfi_launch_tables_ps2.cu", "rfi_launch_tables_ps3.cu", "rfi_confusion.cu", "rfi_probe.cu", "rfi_sim42.cu", "rfi_rl.cu")]
+DEPS = SOURCES + sorted(glob.glob(os.path.join(CSRC, "*.cuh"))) + sorted(glob.glob(os.path.join(CSRC, "*.inc"))) + [
     os.path.join(CSRC, "rfi_internal.h"), os.path.join(ROOT, "include", "rfi.h")]
+
+# per-file additions: the RL-environment evaluator carries a double-precision ground-truth chain that must not be
+# contracted into fused multiply-adds (its CPU restatement is compiled with -ffp-contract=off)
+EXTRA_FLAGS = {"rfi_rl.cu": ["-fmad=false"]}
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
@@ -53,7 +57,7 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
 
     def compile_one(src):
         obj = os.path.join(OBJ_DIR, os.path.basename(src)[:-3] + f".{os.getpid()}.o")
-        cmd = [nvcc, *NVCC_FLAGS, "-c", "-o", obj, src]
+        cmd = [nvcc, *NVCC_FLAGS, *EXTRA_FLAGS.get(os.path.basename(src), []), "-c", "-o", obj, src]
         return obj, cmd, subprocess.run(cmd, capture_output=True, text=True)
 
     with ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:

@@ -64,6 +64,8 @@ int launch_tma_cellmajor(bool fp16, const rfi::KParams& kp, const CUtensorMap* m
 int tma_rows(int M);                                   // rows per TMA stage for window length M
 int launch_batched(bool fp16, const rfi::KParams& kp, const rfi::BatchThr& bt, cudaStream_t st);
 int launch_tables(const rfi::KParams& kp, cudaStream_t st);
+int launch_tables_ps(const rfi::KParams& kp, cudaStream_t st);          // R = 4, per-sample groups compile-time (256 variants)
+
 int launch_batched_tma_cellmajor(bool fp16, const rfi::KParams& kp, const rfi::BatchThr& bt, const CUtensorMap* map,
                                  int sm_count, int smem_optin, cudaStream_t st);
 int launch_confusion(const uint32_t* d_flags, const uint32_t* d_truth, uint64_t* d_counts, int K, size_t n_words,

@@ -3,6 +3,22 @@
 #include "rfi_tables.cuh"
 
 namespace rfi_host {
+
+int launch_tables_ps_part0(int idx, const rfi::KParams& kp, cudaStream_t st);
+int launch_tables_ps_part1(int idx, const rfi::KParams& kp, cudaStream_t st);
+int launch_tables_ps_part2(int idx, const rfi::KParams& kp, cudaStream_t st);
+int launch_tables_ps_part3(int idx, const rfi::KParams& kp, cudaStream_t st);
+
+int launch_tables_ps(const rfi::KParams& kp, cudaStream_t st) {
+    const int i = (int)((kp.arith_mask & 15u) | (((kp.arith_mask >> 7) & 15u) << 4));   // the 8 per-sample bits
+    switch (i >> 6) {
+        case 0: return launch_tables_ps_part0(i & 63, kp, st);
+        case 1: return launch_tables_ps_part1(i & 63, kp, st);
+        case 2: return launch_tables_ps_part2(i & 63, kp, st);
+        default: return launch_tables_ps_part3(i & 63, kp, st);
+    }
+}
+
 namespace {
 
 template <int R, int MASK>
@@ -18,9 +34,12 @@ int launch_rm(const rfi::KParams& kp, cudaStream_t st) {
 template <int R>
 int launch_r(const rfi::KParams& kp, cudaStream_t st) {
     // compile-time masks: all single, and the assignment the paper's agent learned (Tables 3-4, PAPER.md:196-214:
-    // Table 1 groups 5 and 7 in half, Table 2 groups 4-7 in half); anything else reads the mask at run time
+    // Table 1 groups 5 and 7 in half, Table 2 groups 4-7 in half)
     if (kp.arith_mask == 0u) return launch_rm<R, 0>(kp, st);
     if (kp.arith_mask == 0x3C50u) return launch_rm<R, 0x3C50>(kp, st);
+    // any other mask: block length 4 has one instantiation per assignment of the 8 per-sample groups (the per-window
+    // tail reads its 6 bits at run time); other block lengths read the whole mask at run time
+    if (R == 4 && env_int("RFI_TABLES_PS", 1)) return launch_tables_ps(kp, st);
     return launch_rm<R, -1>(kp, st);
 }
 

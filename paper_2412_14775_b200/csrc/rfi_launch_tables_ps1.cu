@@ -1,0 +1,10 @@
+// rfi_launch_tables_ps1.cu -- per-sample-mask instantiations 64..127 of the tables kernel (rfi_tables_ps.inc).
+#define RFI_PS_PART 1
+#include "rfi_tables_ps.inc"
+
+namespace rfi_host {
+int launch_tables_ps_part1(int idx, const rfi::KParams& kp, cudaStream_t st) {
+    static constexpr auto table = make_table(std::make_integer_sequence<int, 64>{});
+    return table[idx](kp, st);
+}
+}  // namespace rfi_host

@@ -13,8 +13,12 @@
 // therefore bit-identical to the step-by-step CPU restatement in oracle/ -- which shares no code with this file.
 //
 // Mask: bit g-1 = Table 1 group g in half; bit 7+g-1 = Table 2 group g in half (same bits for the real-part and
-// the imaginary-part pass).  MASK >= 0: compile-time mask (all-single 0 and the paper's learned assignment
-// 0x3C50 are instantiated); MASK < 0: the mask is read from the kernel parameters.
+// the imaginary-part pass).  The kernel takes two compile-time masks: SMASK for the per-sample groups (Table 1
+// groups 1-4, Table 2 groups 1-4: where the time goes) and TMASK for the per-window tail (groups 5-7); a negative
+// value means "read the bits from the kernel parameters".  Instantiated: all-single <0,0>, the paper's learned
+// assignment <0x3C50,0x3C50>, every one of the 256 per-sample assignments with a run-time tail <ps,-1> (so that ANY of
+// the 2^14 masks an RL search visits runs at compile-time-mask speed, rfi_launch_tables_ps*.cu), and the fully
+// run-time <-1,-1> for block lengths other than 4.
 // Readings T1-T7 of DESIGN.md section 11 (eps = machine epsilon of the group's format, Eq.(4) brackets, ...).
 #pragma once
 
@@ -115,7 +119,7 @@ __device__ __forceinline__ bool tables_tail(const TabWin& w, const KParams& p, i
     return !keep;
 }
 
-template <int R, int MASK>
+template <int R, int SMASK, int TMASK = SMASK>
 __global__ void __launch_bounds__(128, 4) rfi_tables_kernel(const KParams p) {
     const int lane = threadIdx.x & 31;
     const int n_tiles = (p.n_cells + 31) >> 5;
@@ -149,12 +153,12 @@ __global__ void __launch_bounds__(128, 4) rfi_tables_kernel(const KParams p) {
         for (int r = 0; r < R; ++r) {
             f2 x[4];
             widen(cur[r], x);
-            tables_sample<MASK>(w, x, p.arith_mask);
+            tables_sample<SMASK>(w, x, p.arith_mask);
         }
         ++blk;
         if (++b_in_win == bpw) {
             float tau, r_re, r_im;
-            const bool flag = tables_tail<MASK>(w, p, g.cls, tau, r_re, r_im);
+            const bool flag = tables_tail<TMASK>(w, p, g.cls, tau, r_re, r_im);
             store_flags(p, g, p.k_first, w_global, flag);
             store_stats(p, g, w_global, tau, r_re, r_im);
             if (!flag) {

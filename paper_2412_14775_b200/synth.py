@@ -301,3 +301,28 @@ def sweep_thresholds(M: int, K: int = 64, seed: int = 99):
     s_high = c * (xq[3] + (xq[5] - xq[3]) * u[:, 2])
     gamma = rq[0] + (rq[2] - rq[0]) * u[:, 3]
     return torch.stack([d, s_low, s_high, gamma], 1).tolist()
+
+
+def rl_windows(n: int, T: int = 10, F: int = 2, seed: int = 0, rfi_prob: float = 0.4, device="cpu") -> torch.Tensor:
+    """Windows as the paper's RL training simulator draws them: float32 [n, W = T*F, 4, 2].
+    Complex circular Gaussian noise (standard normal real and imaginary parts) times a scale factor U[0.01, 1000]; with
+    probability 0.4 an RFI signal: a uniformly drawn rectangular footprint inside the T x F window filled with ones
+    times a complex scale factor of modulus U[0.01, 1000], multiplied by a 2 x 2 complex circular Gaussian matrix whose
+    four entries scale the four correlations (reading: the matrix entries are the per-correlation gains that "create
+    correlation between the polarizations of the RFI signal").  Sample order inside a window: time-major (t, f)."""
+    g = torch.Generator(device=device).manual_seed(seed)
+    W = T * F
+    x = torch.randn(n, W, 4, 2, generator=g, device=device)
+    scale = 0.01 + (1000.0 - 0.01) * torch.rand(n, 1, 1, 1, generator=g, device=device)
+    x = x * scale
+    has = torch.rand(n, generator=g, device=device) < rfi_prob
+    t0 = torch.floor(torch.rand(n, generator=g, device=device) * T); t1 = torch.floor(torch.rand(n, generator=g, device=device) * T)
+    f0 = torch.floor(torch.rand(n, generator=g, device=device) * F); f1 = torch.floor(torch.rand(n, generator=g, device=device) * F)
+    tt = torch.arange(T, device=device).view(1, T, 1); ff = torch.arange(F, device=device).view(1, 1, F)
+    foot = ((tt >= torch.minimum(t0, t1).view(n, 1, 1)) & (tt <= torch.maximum(t0, t1).view(n, 1, 1))
+            & (ff >= torch.minimum(f0, f1).view(n, 1, 1)) & (ff <= torch.maximum(f0, f1).view(n, 1, 1)) & has.view(n, 1, 1))
+    amp = torch.polar(0.01 + (1000.0 - 0.01) * torch.rand(n, generator=g, device=device),
+                      2 * math.pi * torch.rand(n, generator=g, device=device))
+    mix = torch.view_as_complex((torch.randn(n, 4, 2, generator=g, device=device) * math.sqrt(0.5)).contiguous())   # 2 x 2, unit variance
+    rfi = foot.reshape(n, W, 1).to(torch.complex64) * (amp.view(n, 1, 1) * mix.view(n, 1, 4))
+    return (x + torch.view_as_real(rfi)).to(torch.float32).contiguous()

@@ -61,6 +61,23 @@ def test_tables_mode_is_bit_exact(mask):
     assert 0.0 < out["flags"].mean() < 0.9
 
 
+def test_tables_any_mask_bit_exact_through_the_per_sample_instantiations(monkeypatch):
+    """An RL search visits arbitrary masks: 24 random ones (block length 4 -> rfi_tables_kernel<4, ps, -1>, the 8
+    per-sample bits compile-time) bit-exact against the oracle and equal to the fully run-time-mask kernel."""
+    w = synth.WORKLOADS["lofar"].scaled(n_stations=4, n_time=320, n_int=160, window_M=16, burst_cell_frac=0.15)
+    c = (16 * 0.9 + 1) / 15
+    thr = (0.9, 0.08 * c, 0.6 * c, 0.5)
+    rng = np.random.default_rng(14)
+    vis, _ = synth.make_chunk(w, seed=1234, device="cpu")
+    for mask in rng.integers(1, 1 << 14, 24).tolist():
+        out, ref = check_tables(w, thr, int(mask))
+        monkeypatch.setenv("RFI_TABLES_PS", "0")
+        rt = run_tables(w, vis, thr, int(mask))
+        monkeypatch.delenv("RFI_TABLES_PS")
+        for key in ("tau", "r_re", "r_im", "flags", "weight", "avg"):
+            np.testing.assert_array_equal(out[key], rt[key], err_msg=f"{key}, mask {mask:#06x}")
+
+
 @pytest.mark.parametrize("M,n_int,n_time,n_chan", [(16, 64, 256, 13), (5, 20, 40, 64), (3, 12, 48, 16)])
 def test_tables_mode_ragged_shapes(M, n_int, n_time, n_chan):
     w = synth.Workload("tab", 4, False, n_chan, n_time, M, n_int, burst_cell_frac=0.2, channel_gain=True)
