@@ -444,6 +444,8 @@ def run_ours(args):
     else:
         plan.set_thresholds(thr)
     plan.set_variant(args.variant)
+    if args.adaptive > 0:                 # on-line threshold adaptation (rfi_plan_set_adaptive): kernel + a one-CTA update per step
+        plan.set_adaptive(args.adaptive, 0.5)
     avg, weight, _ = plan.alloc_outputs(device=dev)
     out_bytes = avg.numel() * 4 + weight.numel() * 4 + max(plan.K, 1) * plan.n_win * plan.n_baselines * plan.wpb * 4
     in_bytes = vis.numel() * vis.element_size()            # this rank's input (the whole chunk unless sharded)
@@ -504,7 +506,7 @@ def run_ours(args):
     # the paper's SK-only / DS-only / BOTH comparison in one batched pass: disabling a detector is
     # a threshold at infinity (include/rfi.h).  Not timed.
     by_detector = None
-    if plan.K == 1 and args.arith == "fast" and rank == 0 and not two_classes and args.layout == "time_major" and not work["sharded"]:
+    if plan.K == 1 and args.arith == "fast" and rank == 0 and not two_classes and args.layout == "time_major" and not work["sharded"] and args.adaptive == 0:
         INF = float("inf")
         d0, lo0, hi0, g0 = thr[0]
         plan3 = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M,
@@ -603,7 +605,7 @@ def run_ours(args):
     # CUDA events (best and median over the launches) and parity-checked on sampled cells
     configs = None
     if (world == 1 and not args.no_configs and args.workload == "lofar" and args.K == 1 and args.arith == "fast"
-            and args.layout == "time_major" and not two_classes and args.variant == "auto"):
+            and args.layout == "time_major" and not two_classes and args.variant == "auto" and args.adaptive == 0):
         configs = []
         n_sub = max(args.steps, 20)
         plan.destroy()
@@ -628,6 +630,7 @@ def run_ours(args):
                    "window_M": w.window_M, "window_F": w.window_F, "n_int": w.n_int, "K": max(plan.K, 1), "variant": variant,
                    "arithmetic": args.arith if args.arith == "fast" else f"tables, mask {args.mask:#06x}",
                    "threshold_classes": 2 if two_classes else 1, "layout": args.layout,
+                   "adaptive_false_alarm": args.adaptive if args.adaptive > 0 else None,
                    "input_bytes": w.input_bytes,
                    "l2": ("L2 flushed between timed iterations (256 MB write, outside the timed events)" if small
                           else "input (>= 9 GB) is far larger than the 126 MB L2: no flush needed"),
@@ -667,6 +670,8 @@ def main():
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="N > 1: weak = one chunk per rank; strong = ONE chunk sharded by baseline (rfi_plan_set_baseline_shard)")
     ap.add_argument("--no-configs", action="store_true", help="skip the per-config sub-records of the default run")
+    ap.add_argument("--adaptive", type=float, default=0.0,
+                    help="hold this false-alarm rate by on-line threshold adaptation (rfi_plan_set_adaptive, DESIGN.md NEXT-3)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -160,6 +160,31 @@ int rfi_plan_set_baseline_shard(rfi_plan *plan, int b_first, int b_count);
  * The statistics planes (d_stats) always carry tau with the d of set 0 (of the cell's class). */
 int rfi_set_thresholds(rfi_plan *plan, int K, const rfi_thresholds *h_sets);
 
+/* On-line threshold adaptation (the thresholds follow from "the desired performance (the false alarm
+ * probability)"; "some fine-tuning for each data stream is necessary ... in an online manner";
+ * "dynamic adaptation of the threshold levels depending on the data streams").  The paper gives no
+ * algorithm; this is a constant-false-alarm-rate rule by rank (readings A1-A6): while a chunk
+ * is processed the kernel histograms tau (Eq.(4)) and max(r_re, r_im) (Eq.(9)) of every window with finite
+ * statistics, per baseline class (geometric bins, 64 per octave, tau in [2^-8, 2^4), r in [2^-6, 1)); after the chunk
+ * a device kernel folds them into running histograms (acc <- forget * acc + chunk) and sets the thresholds of the NEXT
+ * chunk to s_low = Q_tau(beta/2), s_high = Q_tau(1 - beta/2), gamma = Q_r(1 - beta) with beta = 1 - sqrt(1 -
+ * false_alarm), so that the two OR-ed detectors flag a fraction false_alarm of RFI-free data.  The first chunk runs
+ * with the thresholds of rfi_set_thresholds (their d stays in force); a class with fewer than 1000 counted windows
+ * keeps its thresholds.  All on the caller's stream, no host synchronisation.  false_alarm = 0 switches the
+ * adaptation off.  Needs K = 1, RFI_ARITH_FAST, the time-major layout and the direct kernel (else rfi_process_chunk
+ * returns RFI_EINVAL).  RFI_EINVAL unless 0 <= false_alarm < 0.5 and 0 <= forget < 1. */
+int rfi_plan_set_adaptive(rfi_plan *plan, float false_alarm, float forget);
+
+/* The thresholds currently in force, one set per baseline class (h_out[n_classes], host memory): the adapted ones
+ * when adaptation is on (waits for the device work enqueued so far), else set 0 of rfi_set_thresholds. */
+int rfi_plan_get_thresholds(rfi_plan *plan, rfi_thresholds *h_out);
+
+/* Diagnostics: the running histograms of the adaptation, double[2 classes][768 tau bins | 384 r bins] to host memory
+ * (waits for the device work enqueued so far).  RFI_ESTATE unless adaptation is on and a chunk was processed. */
+#define RFI_ADAPT_TAU_BINS 768
+#define RFI_ADAPT_R_BINS 384
+int rfi_plan_get_adaptive_histogram(rfi_plan *plan, double *h_out);
+
 /* Choose a kernel variant (default RFI_VARIANT_AUTO).  RFI_EINVAL if unknown. */
 int rfi_plan_set_variant(rfi_plan *plan, int variant);
 

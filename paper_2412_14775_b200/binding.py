@@ -26,7 +26,8 @@ EXPORTS = [
     "rfi_strerror", "rfi_last_cuda_error", "rfi_flags_bytes", "rfi_avg_bytes", "rfi_weight_bytes",
     "rfi_stats_bytes", "rfi_vis_bytes", "rfi_plan_launch_count", "rfi_plan_last_variant", "rfi_version",
     "rfi_probe_read_bandwidth", "rfi_sim42_generate", "rfi_sim42_vis_bytes", "rfi_sim42_truth_bytes",
-    "rfi_rl_evaluate",
+    "rfi_rl_evaluate", "rfi_plan_set_adaptive", "rfi_plan_get_thresholds",
+    "rfi_plan_get_adaptive_histogram",
 ]
 
 
@@ -96,6 +97,12 @@ def load_library(build_if_missing: bool = True):
     lib.rfi_plan_set_arithmetic.argtypes = [vp, ci, ctypes.c_uint32]
     lib.rfi_set_thresholds.argtypes = [vp, ci, ctypes.POINTER(RfiThresholds)]
     lib.rfi_plan_set_variant.argtypes = [vp, ci]
+    lib.rfi_plan_set_adaptive.argtypes = [vp, ctypes.c_float, ctypes.c_float]
+    lib.rfi_plan_set_adaptive.restype = ci
+    lib.rfi_plan_get_thresholds.argtypes = [vp, ctypes.POINTER(RfiThresholds)]
+    lib.rfi_plan_get_thresholds.restype = ci
+    lib.rfi_plan_get_adaptive_histogram.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
+    lib.rfi_plan_get_adaptive_histogram.restype = ci
     lib.rfi_process_chunk.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.rfi_get_flags.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(sz)]
     lib.rfi_process_chunk_host.argtypes = [vp, vp, vp, vp, vp, vp]
@@ -217,6 +224,24 @@ class RfiPlan:
         arr = (RfiThresholds * len(flat))(*[RfiThresholds(*map(float, s)) for s in flat])
         _check(self._lib.rfi_set_thresholds(self._h, len(sets), arr), "rfi_set_thresholds")
         self.K = len(sets)
+
+    def set_adaptive(self, false_alarm: float, forget: float = 0.0):
+        """rfi_plan_set_adaptive: hold `false_alarm` on RFI-free data by tracking the null quantiles of both statistics
+        per baseline class, chunk by chunk, on the device (0 switches it off)."""
+        _check(self._lib.rfi_plan_set_adaptive(self._h, float(false_alarm), float(forget)), "rfi_plan_set_adaptive")
+
+    def get_thresholds(self):
+        """rfi_plan_get_thresholds: [(d, s_low, s_high, gamma)] per baseline class, as currently in force."""
+        arr = (RfiThresholds * self.n_classes)()
+        _check(self._lib.rfi_plan_get_thresholds(self._h, arr), "rfi_plan_get_thresholds")
+        return [(t.d, t.s_low, t.s_high, t.gamma) for t in arr]
+
+    def get_adaptive_histogram(self):
+        """rfi_plan_get_adaptive_histogram: list over the two classes of (tau histogram [768], r histogram [384]) as float64."""
+        buf = (ctypes.c_double * (2 * 1152))()
+        _check(self._lib.rfi_plan_get_adaptive_histogram(self._h, buf), "rfi_plan_get_adaptive_histogram")
+        a = torch.tensor(list(buf), dtype=torch.float64).view(2, 1152)
+        return [(a[c, :768].clone(), a[c, 768:].clone()) for c in range(2)]
 
     def set_variant(self, variant):
         v = _VARIANTS[variant] if isinstance(variant, str) else int(variant)

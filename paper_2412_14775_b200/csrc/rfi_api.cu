@@ -68,6 +68,13 @@ struct rfi_plan {
     size_t flags_words_cap = 0;
     bool have_result = false;
     std::vector<MapEntry> maps;
+    // on-line threshold adaptation (rfi_plan_set_adaptive): device-resident thresholds, chunk and running histograms
+    double adapt_alpha = 0.0, adapt_forget = 0.0;
+    rfi::Thr* d_thr = nullptr;                 // [2] thresholds the ADAPT kernel loads
+    rfi_thresholds* d_thr_raw = nullptr;       // [2] the same as (d, s_low, s_high, gamma)
+    uint32_t* d_hist = nullptr;                // [2][kAdaptBins] this chunk's counts
+    double* d_hist_acc = nullptr;              // [2][kAdaptBins] running histograms
+    bool adapt_uploaded = false;               // d_thr holds the a-priori thresholds / the state was reset
     // host path
     void* d_stage[2] = {nullptr, nullptr};
     size_t d_stage_cap[2] = {0, 0};
@@ -237,6 +244,7 @@ int enqueue_slab(rfi_plan* p, const void* d_vis_slab, int o_first, int n_out_sla
     kp.K = p->K;
     kp.k_first = 0;
     kp.flags_atomic = (p->n_chan % 32 != 0 && 32 % p->n_chan != 0) ? 1 : 0;
+    if (p->adapt_alpha > 0.0) { kp.d_thr = p->d_thr; kp.hist = p->d_hist; }
 
     const bool fp16 = p->precision == RFI_FP16;
     if (p->arith == RFI_ARITH_TABLES) {
@@ -359,7 +367,44 @@ int prepare(rfi_plan* p, cudaStream_t st) {
     }
     const bool flags_atomic = (p->n_chan % 32 != 0 && 32 % p->n_chan != 0);
     if (flags_atomic) RFI_CUDA(cudaMemsetAsync(p->d_flags, 0, p->flags_words() * sizeof(uint32_t), st));
+    if (p->adapt_alpha > 0.0) {
+        if (p->K != 1 || p->arith != RFI_ARITH_FAST || p->layout != RFI_LAYOUT_TIME_MAJOR || p->variant == RFI_VARIANT_TMA) {
+            snprintf(g_cuda_err, sizeof(g_cuda_err), "adaptive thresholds need K = 1, RFI_ARITH_FAST, the time-major layout "
+                     "and the direct kernel (RFI_VARIANT_AUTO or RFI_VARIANT_DIRECT)");
+            return RFI_EINVAL;
+        }
+        const size_t hb = 2 * (size_t)rfi::kAdaptBins;
+        if (!p->d_thr) {
+            if (cudaMalloc(&p->d_thr, 2 * sizeof(rfi::Thr)) != cudaSuccess || cudaMalloc(&p->d_thr_raw, 2 * sizeof(rfi_thresholds)) != cudaSuccess ||
+                cudaMalloc(&p->d_hist, hb * sizeof(uint32_t)) != cudaSuccess || cudaMalloc(&p->d_hist_acc, hb * sizeof(double)) != cudaSuccess) {
+                cudaGetLastError();
+                return RFI_ENOMEM;
+            }
+            p->adapt_uploaded = false;
+        }
+        if (!p->adapt_uploaded) {
+            // (re)start from the thresholds given a priori: pageable host source, so the copies are
+            // complete with respect to the host when the calls return
+            const int nc = p->n_classes;
+            rfi::Thr t[2] = {to_device_thr(p->thr[0], p->M * p->F), to_device_thr(p->thr[nc - 1], p->M * p->F)};
+            rfi_thresholds r[2] = {p->thr[0], p->thr[nc - 1]};
+            RFI_CUDA(cudaMemcpyAsync(p->d_thr, t, sizeof(t), cudaMemcpyHostToDevice, st));
+            RFI_CUDA(cudaMemcpyAsync(p->d_thr_raw, r, sizeof(r), cudaMemcpyHostToDevice, st));
+            RFI_CUDA(cudaMemsetAsync(p->d_hist, 0, hb * sizeof(uint32_t), st));
+            RFI_CUDA(cudaMemsetAsync(p->d_hist_acc, 0, hb * sizeof(double), st));
+            p->adapt_uploaded = true;
+        }
+    }
     return RFI_OK;
+}
+
+// After the chunk's kernels: fold the chunk's histograms into the running ones and set the next chunk's thresholds.
+int finish_adaptive(rfi_plan* p, cudaStream_t st) {
+    if (p->adapt_alpha <= 0.0) return RFI_OK;
+    const int rc = launch_adapt_update(p->d_hist, p->d_hist_acc, p->d_thr, p->d_thr_raw, p->n_classes, p->adapt_alpha,
+                                       p->adapt_forget, st);
+    if (rc == RFI_OK) p->launches++;
+    return rc;
 }
 
 }  // namespace
@@ -461,6 +506,37 @@ int rfi_set_thresholds(rfi_plan* p, int K, const rfi_thresholds* h_sets) {
     p->thr.assign(h_sets, h_sets + n_sets);
     p->K = K;
     p->have_result = false;
+    p->adapt_uploaded = false;                // adaptation restarts from the new a-priori thresholds
+    return RFI_OK;
+}
+
+int rfi_plan_set_adaptive(rfi_plan* p, float false_alarm, float forget) {
+    if (!p || !(false_alarm >= 0.f) || !(false_alarm < 0.5f) || !(forget >= 0.f) || !(forget < 1.f)) return RFI_EINVAL;
+    p->adapt_alpha = false_alarm;
+    p->adapt_forget = forget;
+    p->adapt_uploaded = false;
+    p->have_result = false;
+    return RFI_OK;
+}
+
+int rfi_plan_get_adaptive_histogram(rfi_plan* p, double* h_out) {
+    if (!p || !h_out) return RFI_EINVAL;
+    if (p->adapt_alpha <= 0.0 || !p->d_hist_acc || !p->adapt_uploaded) return RFI_ESTATE;
+    RFI_CUDA(cudaMemcpy(h_out, p->d_hist_acc, 2 * (size_t)rfi::kAdaptBins * sizeof(double), cudaMemcpyDeviceToHost));
+    return RFI_OK;
+}
+
+int rfi_plan_get_thresholds(rfi_plan* p, rfi_thresholds* h_out) {
+    if (!p || !h_out) return RFI_EINVAL;
+    if (p->K < 1) return RFI_ESTATE;
+    const int nc = p->n_classes;
+    if (p->adapt_alpha > 0.0 && p->d_thr_raw && p->adapt_uploaded) {
+        rfi_thresholds r[2];
+        RFI_CUDA(cudaMemcpy(r, p->d_thr_raw, sizeof(r), cudaMemcpyDeviceToHost));    // waits for the device work so far
+        for (int c = 0; c < nc; ++c) h_out[c] = r[c == 0 ? 0 : 1];
+        return RFI_OK;
+    }
+    for (int c = 0; c < nc; ++c) h_out[c] = p->thr[c];
     return RFI_OK;
 }
 
@@ -483,6 +559,7 @@ int rfi_process_chunk(rfi_plan* p, const void* d_vis, void* d_avg, void* d_weigh
     if (rc != RFI_OK) return rc;
     rc = enqueue_slab(p, d_vis, 0, p->n_out(), static_cast<float*>(d_avg), static_cast<uint32_t*>(d_weight),
                       static_cast<float*>(d_stats), st);
+    if (rc == RFI_OK) rc = finish_adaptive(p, st);
     if (rc == RFI_OK) p->have_result = true;
     return rc;
 }
@@ -558,6 +635,8 @@ int rfi_process_chunk_host(rfi_plan* p, const void* h_vis, void* h_avg, void* h_
             if (rc2 != RFI_OK) return rc2;
             RFI_CUDA(cudaEventRecord(p->ev_done[b], comp_st));
         }
+        const int rc3 = finish_adaptive(p, comp_st);
+        if (rc3 != RFI_OK) return rc3;
         RFI_CUDA(cudaMemcpyAsync(h_avg, p->d_avg, rfi_avg_bytes(p), cudaMemcpyDeviceToHost, comp_st));
         RFI_CUDA(cudaMemcpyAsync(h_weight, p->d_weight, rfi_weight_bytes(p), cudaMemcpyDeviceToHost, comp_st));
         RFI_CUDA(cudaMemcpyAsync(h_flags, p->d_flags, rfi_flags_bytes(p), cudaMemcpyDeviceToHost, comp_st));
@@ -579,6 +658,10 @@ int rfi_plan_destroy(rfi_plan* p) {
     if (p->dev_ready) {
         if (p->d_flags) cudaFree(p->d_flags);
         if (p->d_cls) cudaFree(p->d_cls);
+        if (p->d_thr) cudaFree(p->d_thr);
+        if (p->d_thr_raw) cudaFree(p->d_thr_raw);
+        if (p->d_hist) cudaFree(p->d_hist);
+        if (p->d_hist_acc) cudaFree(p->d_hist_acc);
         if (p->d_avg) cudaFree(p->d_avg);
         if (p->d_weight) cudaFree(p->d_weight);
         if (p->d_stats) cudaFree(p->d_stats);

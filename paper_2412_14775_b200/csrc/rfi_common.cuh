@@ -57,11 +57,25 @@ struct KParams {
     int K;                    // sets handled by this launch (batched kernel: <= kMaxBatch)
     int k_first;              // global index of this launch's first set
     int flags_atomic;         // 1: flag words may be shared between warps -> atomicOr into a zeroed buffer
+    // on-line threshold adaptation (rfi_plan_set_adaptive; rfi_adapt.cu): thresholds of the two classes in device memory
+    // (updated between chunks by a device kernel) and this chunk's histograms of tau and max(r_re, r_im); null otherwise
+    const Thr* d_thr;
+    uint32_t* hist;
     // paper-literal tables mode (rfi_tables.cuh) only: raw thresholds of set 0 and the 14-bit precision mask
     float d, s_low, s_high;
     float d1, s_low1, s_high1;   // class 1
     uint32_t arith_mask;
 };
+
+// Histogram bins of the adaptation (reading A2): geometric, 64 linear sub-bins per octave, read
+// off the float's bit pattern; tau in [2^-8, 2^4) -> 768 bins, max(r_re, r_im) in [2^-6, 1) -> 384 bins.
+constexpr int kAdaptTauBins = 768, kAdaptRBins = 384, kAdaptBins = kAdaptTauBins + kAdaptRBins;
+constexpr int kAdaptTauLoExp = -8, kAdaptRLoExp = -6;
+__device__ __forceinline__ int adapt_bin(float v, int lo_exp, int n_bins) {
+    if (!(v > 0.f)) return 0;                                 // zero and negative values: first bin (NaN is never binned)
+    const int idx = (int)(__float_as_uint(v) >> 17) - ((127 + lo_exp) << 6);
+    return min(max(idx, 0), n_bins - 1);
+}
 
 struct BatchThr { Thr t[kMaxBatch]; Thr t1[kMaxBatch]; };   // by-value kernel parameter (constant bank), 2 KiB: class 0, class 1
 

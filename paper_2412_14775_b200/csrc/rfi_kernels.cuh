@@ -24,13 +24,12 @@ __device__ __forceinline__ void load_block(const uint8_t* ptr, size_t row_stride
     }
 }
 
-template <int R, bool FP16, bool ALIGN32>
-__global__ void __launch_bounds__(128, (FP16 || R <= 4) ? 4 : (R == 5 ? 3 : 2)) rfi_direct_kernel(const KParams p) {
+// One (tile, integration) unit of the direct kernel.  ADAPT (on-line threshold adaptation, rfi_adapt.cu): the lane's
+// thresholds are read from device memory once per unit and every window is counted in the CTA's histogram.
+template <int R, bool FP16, bool ALIGN32, bool ADAPT>
+__device__ __forceinline__ void direct_unit(const KParams& p, const int unit, const int n_tiles, uint32_t* sh_hist) {
     constexpr int SAMPLE_BYTES = FP16 ? 16 : 32;
     const int lane = threadIdx.x & 31;
-    const int n_tiles = (p.n_cells + 31) >> 5;
-    const int unit = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    if (unit >= n_tiles * p.n_out_slab) return;
     const int o_local = unit / n_tiles;
     const int tile = unit - o_local * n_tiles;
     const LaneGeom g = lane_geom(p, tile, lane);
@@ -50,11 +49,13 @@ __global__ void __launch_bounds__(128, (FP16 || R <= 4) ? 4 : (R == 5 ? 3 : 2)) 
     w.reset();
     int blk = 0, b_in_win = 0;
 
+    Thr thr_dev;
+    if constexpr (ADAPT) thr_dev = p.d_thr[g.cls];
     Raw<FP16> A[R], B[R];
     auto window_end = [&]() {
         ++blk;
         if (++b_in_win == bpw) {
-            finish_window(p, g, w, inv_M, w_global, acc, wt);
+            finish_window<ADAPT>(p, g, w, inv_M, w_global, acc, wt, &thr_dev, sh_hist);
             ++w_global;
             b_in_win = 0;
             w.reset();
@@ -109,6 +110,25 @@ __global__ void __launch_bounds__(128, (FP16 || R <= 4) ? 4 : (R == 5 ? 3 : 2)) 
         if (blk < total) step(A, B);
     }
     store_output(p, g, p.k_first, o_global, acc, wt);
+}
+
+template <int R, bool FP16, bool ALIGN32, bool ADAPT = false>
+__global__ void __launch_bounds__(128, (FP16 || R <= 4) ? 4 : (R == 5 ? 3 : 2)) rfi_direct_kernel(const KParams p) {
+    const int n_tiles = (p.n_cells + 31) >> 5;
+    const int unit = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if constexpr (!ADAPT) {
+        if (unit < n_tiles * p.n_out_slab) direct_unit<R, FP16, ALIGN32, false>(p, unit, n_tiles, nullptr);
+    } else {
+        __shared__ uint32_t sh_hist[2 * kAdaptBins];          // [class][tau bins | r bins], flushed once per CTA
+        for (int i = threadIdx.x; i < 2 * kAdaptBins; i += blockDim.x) sh_hist[i] = 0u;
+        __syncthreads();
+        if (unit < n_tiles * p.n_out_slab) direct_unit<R, FP16, ALIGN32, true>(p, unit, n_tiles, sh_hist);
+        __syncthreads();
+        for (int i = threadIdx.x; i < 2 * kAdaptBins; i += blockDim.x) {
+            const uint32_t c = sh_hist[i];
+            if (c) atomicAdd(p.hist + i, c);
+        }
+    }
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -203,16 +203,28 @@ __device__ __forceinline__ void store_output(const KParams& p, const LaneGeom& g
 }
 
 // Single-set window tail shared by the streaming kernels: statistics, decision, flag word, statistics planes,
-// masked accumulation into the output integration.
+// masked accumulation into the output integration.  ADAPT: the thresholds come from device memory
+// (`thr`, the lane's class) and the window's tau and max(r_re, r_im) are counted in the CTA's shared-memory histogram.
+template <bool ADAPT = false>
 __device__ __forceinline__ void finish_window(const KParams& p, const LaneGeom& g, Win& w, float inv_W,
-                                              int w_global, f2 (&acc)[4], uint32_t& wt) {
+                                              int w_global, f2 (&acc)[4], uint32_t& wt,
+                                              const Thr* thr = nullptr, uint32_t* sh_hist = nullptr) {
     float x, r_re, r_im;
     if (p.F > 1) combine_group(w, p.F, p.M);
     window_stats(w, inv_W, x, r_re, r_im);
-    const Thr& t = g.cls ? p.thr1 : p.thr0;                   // per-baseline-class thresholds (cross / auto)
-    const bool flag = decide(x, max_nan(r_re, r_im), t);
+    const Thr& t = ADAPT ? *thr : (g.cls ? p.thr1 : p.thr0);  // per-baseline-class thresholds (cross / auto)
+    const float r_max = max_nan(r_re, r_im);
+    const bool flag = decide(x, r_max, t);
+    const float tau = t.c * x;
     store_flags(p, g, p.k_first, w_global, flag);
-    store_stats(p, g, w_global, t.c * x, r_re, r_im);
+    store_stats(p, g, w_global, tau, r_re, r_im);
+    if constexpr (ADAPT) {
+        if (g.valid && fabsf(tau) <= 3.402823466e38f && fabsf(r_max) <= 3.402823466e38f) {   // finite statistics only
+            uint32_t* h = sh_hist + g.cls * kAdaptBins;
+            atomicAdd(h + adapt_bin(tau, kAdaptTauLoExp, kAdaptTauBins), 1u);
+            atomicAdd(h + kAdaptTauBins + adapt_bin(r_max, kAdaptRLoExp, kAdaptRBins), 1u);
+        }
+    }
     if (!flag) {
 #pragma unroll
         for (int q = 0; q < 4; ++q) acc[q] = add2(acc[q], w.s[q]);

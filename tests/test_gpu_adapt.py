@@ -1,0 +1,135 @@
+"""On-line threshold adaptation on the GPU (rfi_plan_set_adaptive; readings A1-A6) against oracle/adapt_oracle.py:
+the in-kernel histograms bit-exact (both sides bin the float32 statistics the kernel stored), the thresholds of the
+next chunk, the flags the next chunk gets with them, and the false-alarm rate actually held on RFI-free noise."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import paper_2412_14775_b200 as rfi
+from oracle import adapt_oracle as ao
+from paper_2412_14775_b200 import synth
+from tests.parity_util import compare, gpu_outputs_to_numpy
+
+pytestmark = pytest.mark.gpu
+
+
+def _plan(w, thr_cross, thr_auto, alpha, forget=0.0):
+    plan = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M,
+                       rfi.RFI_FP16 if w.fp16 else rfi.RFI_FP32, n_int=w.n_int)
+    if w.window_F > 1:
+        plan.set_window_freq(w.window_F)
+    autos = synth.auto_baseline_mask(w)
+    plan.set_baseline_classes(autos.int().tolist())
+    plan.set_thresholds([[thr_cross, thr_auto]])
+    plan.set_adaptive(alpha, forget)
+    return plan, autos.numpy()
+
+
+def _run(plan, w, vis):
+    avg, weight, stats = plan.alloc_outputs(stats=True)
+    plan.process_chunk(vis.cuda(), avg, weight, stats)
+    torch.cuda.synchronize()
+    out = gpu_outputs_to_numpy(plan, avg, weight, stats, rfi.unpack_flags(plan.get_flags(), w.n_chan))
+    return out
+
+
+@pytest.mark.parametrize("fp16,F,forget", [(False, 1, 0.0), (False, 1, 0.5), (True, 1, 0.25), (False, 2, 0.0)])
+def test_histograms_thresholds_and_next_chunk_flags_match_the_oracle(fp16, F, forget):
+    M = 16 if F == 1 else 10
+    w = synth.Workload("adapt", 12, True, 64, M * 48, M, M * 24, fp16=fp16, window_F=F, channel_gain=True, burst_cell_frac=0.03)
+    W = M * F
+    thr_c, thr_a = synth.default_thresholds(W)[0], synth.auto_thresholds(W)
+    plan, autos = _plan(w, thr_c, thr_a, 0.05, forget)
+    cell_auto = np.repeat(autos, w.n_chan)
+    acc = [None, None]
+    cur = [tuple(thr_c[1:]), tuple(thr_a[1:])]
+    for chunk in range(3):
+        vis, _ = synth.make_chunk(w, seed=100 + chunk)
+        out = _run(plan, w, vis)
+        # the chunk just processed used `cur`: its flags must be the oracle's with those thresholds, per class
+        used = [[thr_c[0], *cur[0]], [thr_a[0], *cur[1]]]
+        v = vis.numpy().reshape(w.n_time, w.n_cells, 4, 2)
+        for cls, sel in ((0, ~cell_auto), (1, cell_auto)):
+            sub = {k: (a[:, :, sel] if a.ndim >= 3 else a[:, sel]) for k, a in out.items()}
+            compare(v[:, sel], M, w.n_int, [used[cls]], sub, tol=2e-3 if fp16 else 1e-5, fp16=fp16, F=F)
+        # oracle update from the statistics the kernel stored (float32: the same numbers the kernel binned)
+        hist = plan.get_adaptive_histogram()
+        got = plan.get_thresholds()
+        for cls, sel in ((0, ~cell_auto), (1, cell_auto)):
+            tau = out["tau"][:, sel]
+            rmax = np.fmax(out["r_re"][:, sel], out["r_im"][:, sel])
+            rmax = np.where(np.isnan(out["r_re"][:, sel]) | np.isnan(out["r_im"][:, sel]), np.nan, rmax)
+            ht, hr = ao.histogram(tau, rmax)
+            acc_t, acc_r, new = ao.update(acc[cls][0] if acc[cls] else None, acc[cls][1] if acc[cls] else None, ht, hr,
+                                          alpha=0.05, forget=forget, previous=cur[cls])
+            acc[cls] = (acc_t, acc_r)
+            assert np.array_equal(hist[cls][0].numpy(), acc_t), f"tau histogram differs (class {cls}, chunk {chunk})"
+            assert np.array_equal(hist[cls][1].numpy(), acc_r), f"r histogram differs (class {cls}, chunk {chunk})"
+            new32 = tuple(float(np.float32(x)) for x in new)
+            assert np.allclose(got[cls][1:], new32, rtol=1e-6, atol=0), (got[cls], new32)
+            assert got[cls][0] == (thr_c, thr_a)[cls][0]                       # d stays in force
+            cur[cls] = tuple(got[cls][1:])                                     # the kernel's own float32 values
+    plan.destroy()
+
+
+def test_false_alarm_rate_is_held_on_clean_noise_for_cross_and_auto_streams():
+    """Done-criterion of VERDICT r01 item 9: measured FA on RFI-free synthetic noise within +-0.5 % (absolute) of the
+    request, separately for the cross- and the auto-correlations, from deliberately wrong a-priori thresholds."""
+    w = synth.Workload("adapt_clean", 24, True, 64, 1024, 16, 512, channel_gain=True)
+    for alpha in (0.05, 0.01):
+        plan, autos = _plan(w, [1.0, 0.0, 50.0, 1.0], [1.0, 0.0, 50.0, 1.0], alpha)       # a priori: flag nothing
+        cell_auto = np.repeat(autos, w.n_chan)
+        fa = []
+        for chunk in range(3):
+            vis, _ = synth.make_chunk(w, seed=500 + chunk)
+            out = _run(plan, w, vis)
+            f = out["flags"][0]
+            fa.append((f[:, ~cell_auto].mean(), f[:, cell_auto].mean()))
+        print(f"alpha {alpha}: flagged fraction (cross, auto) per chunk: {[(round(a, 4), round(b, 4)) for a, b in fa]}; "
+              f"thresholds {plan.get_thresholds()}")
+        assert fa[0] == (0.0, 0.0)
+        for c in (1, 2):
+            assert abs(fa[c][0] - alpha) < 0.005 and abs(fa[c][1] - alpha) < 0.005
+        plan.destroy()
+
+
+def test_adaptation_tracks_a_gain_change_and_the_host_path():
+    """tau and r are scale-invariant so a gain step must NOT move the thresholds; a change of the noise
+    statistics (autos with fewer accumulated spectra would) does.  Also: the host path adapts chunk by chunk."""
+    w = synth.Workload("adapt_host", 8, True, 32, 512, 16, 128, channel_gain=True)
+    plan, _ = _plan(w, synth.default_thresholds(16)[0], synth.auto_thresholds(16), 0.05)
+    vis, _ = synth.make_chunk(w, seed=1)
+    plan.process_chunk_host(vis.pin_memory())
+    t1 = plan.get_thresholds()
+    plan2, _ = _plan(w, synth.default_thresholds(16)[0], synth.auto_thresholds(16), 0.05)
+    plan2.process_chunk_host((vis * 7.5).pin_memory())
+    t2 = plan2.get_thresholds()
+    assert np.allclose(np.array(t1), np.array(t2), rtol=2e-3)
+    assert t1[0] != tuple(synth.default_thresholds(16)[0])                      # it did adapt
+    plan.destroy(); plan2.destroy()
+
+
+def test_adaptive_mode_rejects_unsupported_plans_and_can_be_switched_off():
+    w = synth.Workload("adapt_rej", 4, True, 32, 256, 16, 128)
+    vis, _ = synth.make_chunk(w, seed=2)
+    plan = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, 16, n_int=128)
+    with pytest.raises(rfi.RfiError):
+        plan.set_adaptive(0.7)
+    plan.set_adaptive(0.05)
+    plan.set_thresholds(synth.sweep_thresholds(16, 4))
+    avg, weight, _ = plan.alloc_outputs()
+    with pytest.raises(rfi.RfiError):
+        plan.process_chunk(vis.cuda(), avg, weight)                             # K > 1
+    plan.set_thresholds(synth.default_thresholds(16))
+    plan.set_variant("tma")
+    avg, weight, _ = plan.alloc_outputs()
+    with pytest.raises(rfi.RfiError):
+        plan.process_chunk(vis.cuda(), avg, weight)
+    plan.set_variant("auto")
+    plan.set_adaptive(0.0)                                                      # off: plain run, thresholds as given
+    plan.process_chunk(vis.cuda(), avg, weight)
+    torch.cuda.synchronize()
+    assert plan.get_thresholds()[0] == tuple(np.float32(synth.default_thresholds(16)[0]).tolist())
+    plan.destroy()
