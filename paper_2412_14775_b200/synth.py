@@ -254,8 +254,9 @@ _NULL_Q = {
 
 
 # The same for the auto-correlations of this noise model (Hermitian, Sigma + H/sqrt(n_acc)): |I| is nearly constant,
-# so x sits far below the cross-correlation values; r_im = 0 exactly.  Written by a throw-away run of oracle/ on
-# make_chunk output (40 stations, 20480+ windows); only used to place the class-1 thresholds.
+# so x sits far below the cross-correlation values; r_im = 0 exactly.  Written by tests/golden/make_null_quantiles.py
+# (a committed script that calls only oracle/ and this module; tests/test_synth.py re-derives an entry); only used to
+# place the class-1 thresholds -- parity never depends on them.
 _NULL_Q_AUTO = {
     16: ((0.024, 0.0386, 0.0546, 0.207, 0.2571, 0.3342), (0.418, 0.496, 0.575)),
     20: ((0.031, 0.0447, 0.0602, 0.198, 0.2430, 0.3030), (0.377, 0.449, 0.522)),

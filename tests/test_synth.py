@@ -76,3 +76,36 @@ def test_fp16_and_thresholds():
     assert len(sets) == 64 and all(0.5 <= s[0] <= 1 and s[1] < s[2] and 0 < s[3] < 1 for s in sets)
     d, lo, hi, g = synth.default_thresholds(20)[0]
     assert lo < hi and 0 < g < 1
+
+
+def test_auto_null_quantiles_are_reproduced_by_the_committed_script():
+    """provenance of synth._NULL_Q_AUTO: tests/golden/make_null_quantiles.py (oracle/ + synth only) re-derives W = 16
+    on a smaller sample within Monte-Carlo tolerance"""
+    from tests.golden.make_null_quantiles import null_quantiles_auto
+    xq, rq, n = null_quantiles_auto(16, n_stations=16, n_windows=256, seed=5)
+    ref_x, ref_r = synth._NULL_Q_AUTO[16]
+    assert n == 16 * 16 * 256
+    for got, want, tol in zip(xq[1:5], ref_x[1:5], (0.06, 0.04, 0.04, 0.06)):     # 1, 5, 95, 99 %
+        assert abs(got / want - 1) < tol, (xq, ref_x)
+    assert abs(rq[0] / ref_r[0] - 1) < 0.03 and abs(rq[1] / ref_r[1] - 1) < 0.04
+
+
+def test_fp16_chunk_is_the_rounded_fp32_chunk():
+    """the fp16 gate against the ORIGINAL fp32 data relies on make_chunk rounding as its last step"""
+    w = synth.WORKLOADS["lofar_fp16"].scaled(n_stations=4, n_time=256, n_int=128, burst_cell_frac=0.1, tone_chan_frac=0.05)
+    v16, t16 = synth.make_chunk(w, seed=9)
+    v32, t32 = synth.make_chunk(w.scaled(fp16=False), seed=9)
+    assert v16.dtype == torch.float16 and v32.dtype == torch.float32
+    assert torch.equal(v32.to(torch.float16), v16) and torch.equal(t16, t32)
+
+
+def test_rl_windows_recipe():
+    """scale factors in [0.01, 1000], RFI with probability 0.4 inside a rectangular footprint"""
+    w = synth.rl_windows(4000, 10, 2, seed=3)
+    assert w.shape == (4000, 20, 4, 2) and w.dtype == torch.float32
+    assert torch.equal(w, synth.rl_windows(4000, 10, 2, seed=3))
+    rms = w.pow(2).mean((1, 2, 3)).sqrt()
+    assert rms.min() > 0.005 and rms.max() < 3000
+    clean = synth.rl_windows(4000, 10, 2, seed=3, rfi_prob=0.0)
+    changed = (w != clean).flatten(1).any(1).float().mean()
+    assert abs(changed - 0.4) < 0.03
