@@ -207,14 +207,14 @@ rfi_batched_tma_kernel(const __grid_constant__ CUtensorMap tmap, const KParams p
                             lds_raw(sbase + r * ROW_BYTES + off0, sbase + r * ROW_BYTES + off1, buf[r]);
                         }
                     }
-                    accumulate_block<R, FP16>(w, buf, b);
-                    // stage hand-off (rfi_common.cuh): 32 arrivals after consumption, then the producer's refill
+                    // stage hand-off (rfi_common.cuh): 32 arrivals after the loads, wait, proxy fence, refill
                     mbar_arrive(ebars + 8 * stage);
                     if (lane == 0 && it + stages < total) {
                         mbar_wait(ebars + 8 * stage, parity);
                         fence_proxy_async();
                         pr_issue();
                     }
+                    accumulate_block<R, FP16>(w, buf, b);
                     ++it;
                     if (++stage == stages) { stage = 0; parity ^= 1u; }
                 }

@@ -73,6 +73,7 @@ int launch_adapt_update(uint32_t* d_hist, double* d_acc, rfi::Thr* d_thr, rfi_th
 int launch_confusion(const uint32_t* d_flags, const uint32_t* d_truth, uint64_t* d_counts, int K, size_t n_words,
                      int wpb, int n_chan, int sm_count, cudaStream_t st);
 bool batched_tma_supported(bool fp16, const rfi::KParams& kp, int R);
+
 int launch_batched_tma(bool fp16, const rfi::KParams& kp, const rfi::BatchThr& bt, const CUtensorMap* map, int R,
                        int sm_count, int smem_optin, cudaStream_t st);
 

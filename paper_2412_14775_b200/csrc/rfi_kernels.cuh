@@ -250,15 +250,15 @@ __global__ void __launch_bounds__(512, 1) rfi_tma_kernel(const __grid_constant__
                         lds_raw(sbase + r * ROW_BYTES + off0, sbase + r * ROW_BYTES + off1, buf[r]);
                     }
                 }
-                accumulate_block<R, FP16>(w, buf, b);
-                // hand the stage back: every lane arrives after consuming it, the producer lane waits for all 32
-                // arrivals (same phase parity as the fill it just consumed) before the async-proxy refill
+                // hand the stage back (rfi_common.cuh): every lane arrives after its loads of the stage, the producer
+                // lane waits for the 32 arrivals (same phase parity as the fill just consumed), fences the proxies, refills
                 mbar_arrive(ebars + 8 * stage);
                 if (lane == 0 && it + stages < total) {
                     mbar_wait(ebars + 8 * stage, parity);
                     fence_proxy_async();
                     pr_issue();
                 }
+                accumulate_block<R, FP16>(w, buf, b);
                 ++it;
                 if (++stage == stages) { stage = 0; parity ^= 1u; }
             }
