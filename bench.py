@@ -228,7 +228,8 @@ def sampled_parity(w, plan, vis, truth, thr, avg, weight, stats, n_clean, n_rfi)
         return {"status": "FAILED", "error": str(exc)[:300]}
 
 
-def measure_config(name, K, dev, steps, warmup, peak, read_probe_gbs, vis=None, truth=None, n_clean=512, n_rfi=128):
+def measure_config(name, K, dev, steps, warmup, peak, read_probe_gbs, vis=None, truth=None, n_clean=512, n_rfi=128,
+                   variant="auto"):
     """One sub-record of `configs`: generate (or reuse) the chunk, time `steps` launches one by one with CUDA events
     after `warmup` untimed ones, then check a sample of cells against the oracle."""
     import torch
@@ -254,6 +255,7 @@ def measure_config(name, K, dev, steps, warmup, peak, read_probe_gbs, vis=None, 
     if w.window_F > 1:
         plan.set_window_freq(w.window_F)
     plan.set_thresholds(thr)
+    plan.set_variant(variant)
     avg, weight, stats = plan.alloc_outputs(device=dev, stats=True)
     out_bytes = avg.numel() * 4 + weight.numel() * 4 + max(plan.K, 1) * plan.n_win * plan.n_baselines * plan.wpb * 4
     algo = w.input_bytes + out_bytes
@@ -618,6 +620,8 @@ def run_ours(args):
         configs.append(measure_config("lofar_tf10x2", 1, dev, n_sub, 3, peak, read_probe))
         configs.append(measure_config("large", 1, dev, n_sub, 3, peak, read_probe, n_clean=256, n_rfi=256))
         configs.append(measure_config("tiny", 1, dev, max(n_sub, 50), 5, peak, read_probe, n_clean=96, n_rfi=6))
+        # the same small chunk through the low-latency variant (RFI_VARIANT_SPLIT: a unit's rows split over 16 warps)
+        configs.append(measure_config("tiny", 1, dev, max(n_sub, 50), 5, peak, read_probe, n_clean=96, n_rfi=6, variant="split"))
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,

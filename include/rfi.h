@@ -76,7 +76,13 @@ enum {
     RFI_VARIANT_DIRECT = 1,   /* per-thread 256-bit (fp32) / 128-bit (fp16) streaming loads, register double buffer */
     RFI_VARIANT_TMA    = 2,   /* warp-private TMA (cp.async.bulk.tensor) ring in shared memory */
     RFI_VARIANT_BATCHED = 3,  /* reported by rfi_plan_last_variant when K > 1 (not selectable: K decides) */
-    RFI_VARIANT_TABLES = 4    /* reported when the arithmetic mode is RFI_ARITH_TABLES */
+    RFI_VARIANT_TABLES = 4,   /* reported when the arithmetic mode is RFI_ARITH_TABLES */
+    RFI_VARIANT_SPLIT  = 5    /* small chunks, low latency: one CTA per (tile, integration), its rows split over up to
+                                 16 warps so that the whole unit is in flight at once (windows are kept small
+                                 for latency).  K = 1, RFI_ARITH_FAST, time-major, n_int / block length <= 96.  The SK
+                                 statistic is bit-identical to the direct kernel; alignment statistics and averages are
+                                 summed block-wise, i.e. equal to the other variants within the stated tolerances, not
+                                 bit for bit.  Never chosen by RFI_VARIANT_AUTO. */
 };
 
 /* input layouts (rfi_plan_set_layout) */

@@ -16,7 +16,7 @@ from . import build as _build
 
 RFI_FP32, RFI_FP16 = 0, 1
 VARIANT_AUTO, VARIANT_DIRECT, VARIANT_TMA = 0, 1, 2
-_VARIANTS = {"auto": 0, "direct": 1, "tma": 2}
+_VARIANTS = {"auto": 0, "direct": 1, "tma": 2, "split": 5}
 ARITH_FAST, ARITH_TABLES = 0, 1
 MASK_PAPER_LEARNED = 0x3C50      # Tables 3-4: Table 1 groups 5,7 and Table 2 groups 4-7 in half
 
@@ -319,7 +319,7 @@ class RfiPlan:
     @property
     def last_variant(self) -> str:
         v = self._lib.rfi_plan_last_variant(self._h)
-        return {0: "none", 1: "direct", 2: "tma", 3: "batched", 4: "tables"}.get(v, str(v))
+        return {0: "none", 1: "direct", 2: "tma", 3: "batched", 4: "tables", 5: "split"}.get(v, str(v))
 
     def destroy(self):
         if self._h:

@@ -19,7 +19,7 @@ ROOT = os.path.dirname(HERE)
 LIB = os.path.join(CSRC, "librfi.so")
 OBJ_DIR = os.path.join(CSRC, "build")
 SOURCES = [os.path.join(CSRC, f) for f in
-           ("rfi_api.cu", "rfi_launch_direct.cu", "rfi_launch_tma.cu", "rfi_launch_batched.cu", "rfi_launch_batched_tma.cu", "rfi_launch_tables.cu", "rfi_launch_tables_ps0.cu", "rfi_launch_tables_ps1.cu", "rfi_launch_tables_ps2.cu", "rfi_launch_tables_ps3.cu", "rfi_confusion.cu", "rfi_probe.cu", "rfi_sim42.cu", "rfi_rl.cu", "rfi_adapt.cu")]
+           ("rfi_api.cu", "rfi_launch_direct.cu", "rfi_launch_split.cu", "rfi_launch_tma.cu", "rfi_launch_batched.cu", "rfi_launch_batched_tma.cu", "rfi_launch_tables.cu", "rfi_launch_tables_ps0.cu", "rfi_launch_tables_ps1.cu", "rfi_launch_tables_ps2.cu", "rfi_launch_tables_ps3.cu", "rfi_confusion.cu", "rfi_probe.cu", "rfi_sim42.cu", "rfi_rl.cu", "rfi_adapt.cu")]
 DEPS = SOURCES + sorted(glob.glob(os.path.join(CSRC, "*.cuh"))) + sorted(glob.glob(os.path.join(CSRC, "*.inc"))) + [
     os.path.join(CSRC, "rfi_internal.h"), os.path.join(ROOT, "include", "rfi.h")]
 

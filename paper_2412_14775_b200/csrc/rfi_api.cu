@@ -339,7 +339,9 @@ int enqueue_slab(rfi_plan* p, const void* d_vis_slab, int o_first, int n_out_sla
     }
     p->last_variant = variant;
     int rc;
-    if (variant == RFI_VARIANT_TMA) {
+    if (variant == RFI_VARIANT_SPLIT) {
+        rc = launch_split(fp16, kp, p->smem_optin, st);
+    } else if (variant == RFI_VARIANT_TMA) {
         const int rows = n_out_slab * p->n_int;
         const int R = tma_rows(p->M);
         CUtensorMap map_v;
@@ -368,7 +370,8 @@ int prepare(rfi_plan* p, cudaStream_t st) {
     const bool flags_atomic = (p->n_chan % 32 != 0 && 32 % p->n_chan != 0);
     if (flags_atomic) RFI_CUDA(cudaMemsetAsync(p->d_flags, 0, p->flags_words() * sizeof(uint32_t), st));
     if (p->adapt_alpha > 0.0) {
-        if (p->K != 1 || p->arith != RFI_ARITH_FAST || p->layout != RFI_LAYOUT_TIME_MAJOR || p->variant == RFI_VARIANT_TMA) {
+        if (p->K != 1 || p->arith != RFI_ARITH_FAST || p->layout != RFI_LAYOUT_TIME_MAJOR || p->variant == RFI_VARIANT_TMA ||
+            p->variant == RFI_VARIANT_SPLIT) {
             snprintf(g_cuda_err, sizeof(g_cuda_err), "adaptive thresholds need K = 1, RFI_ARITH_FAST, the time-major layout "
                      "and the direct kernel (RFI_VARIANT_AUTO or RFI_VARIANT_DIRECT)");
             return RFI_EINVAL;
@@ -541,7 +544,8 @@ int rfi_plan_get_thresholds(rfi_plan* p, rfi_thresholds* h_out) {
 }
 
 int rfi_plan_set_variant(rfi_plan* p, int variant) {
-    if (!p || variant < RFI_VARIANT_AUTO || variant > RFI_VARIANT_TMA) return RFI_EINVAL;   // BATCHED is not selectable
+    if (!p || !(variant == RFI_VARIANT_AUTO || variant == RFI_VARIANT_DIRECT || variant == RFI_VARIANT_TMA ||
+                variant == RFI_VARIANT_SPLIT)) return RFI_EINVAL;                             // BATCHED / TABLES are not selectable
     p->variant = variant;
     return RFI_OK;
 }

@@ -57,6 +57,7 @@ inline int pick_rows(int M, bool fp16, int cap = 8) {
 
 // Each returns RFI_OK or RFI_ECUDA / RFI_EINVAL; all only enqueue work on `st`.
 int launch_direct(bool fp16, const rfi::KParams& kp, cudaStream_t st);
+int launch_split(bool fp16, const rfi::KParams& kp, int smem_optin, cudaStream_t st);   // small chunks, low latency
 int launch_tma(bool fp16, const rfi::KParams& kp, const CUtensorMap* map, int R, int sm_count, int smem_optin,
                cudaStream_t st);
 int launch_tma_cellmajor(bool fp16, const rfi::KParams& kp, const CUtensorMap* map, int sm_count, int smem_optin,

@@ -52,23 +52,34 @@ __device__ __forceinline__ float accumulate_sample(Win& w, const f2 (&x)[4]) {
 // R samples (one block) of the window; `blk` = index of the block inside the window (0-based).
 // Merge of (n_a = blk*R, mean, m2) with the block's (R, mb, m2b):
 //   delta = mb - mean;  mean += delta/(blk+1);  m2 += m2b + delta^2 * R*blk/(blk+1)
+// The two halves are separate functions because the split kernel (rfi_split.cuh) computes the block statistics on one
+// warp and merges them, in block order, on another: same operations in the same order, hence the same bits.
 template <int R>
-__device__ __forceinline__ void merge_block(Win& w, const float (&z)[R], int blk) {
+__device__ __forceinline__ void block_stats(const float (&z)[R], float& mb, float& m2b) {
     float zs = z[0];
 #pragma unroll
     for (int r = 1; r < R; ++r) zs += z[r];
-    const float mb = zs * (1.0f / R);
-    float m2b = 0.f;
+    mb = zs * (1.0f / R);
+    m2b = 0.f;
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         const float dz = z[r] - mb;
         m2b = fmaf(dz, dz, m2b);
     }
+}
+template <int R>
+__device__ __forceinline__ void merge_stats(Win& w, float mb, float m2b, int blk) {
     const float fb = (float)blk;
     const float wgt = rcp_approx(fb + 1.0f);                  // 1/(blk+1); blk = 0 -> exactly 1
     const float delta = mb - w.mean;
     w.mean = fmaf(delta, wgt, w.mean);
     w.m2 += fmaf(delta * delta, (float)R * fb * wgt, m2b);
+}
+template <int R>
+__device__ __forceinline__ void merge_block(Win& w, const float (&z)[R], int blk) {
+    float mb, m2b;
+    block_stats<R>(z, mb, m2b);
+    merge_stats<R>(w, mb, m2b, blk);
 }
 
 template <int R, bool FP16>

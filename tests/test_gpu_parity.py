@@ -52,7 +52,7 @@ def check(w, thresholds, variant, seed=1234, tol=None, mutate=None, layout="time
     return rep, out, truth
 
 
-@pytest.mark.parametrize("variant", ["direct", "tma"])
+@pytest.mark.parametrize("variant", ["direct", "tma", "split"])
 def test_tiny_config(variant):
     """BASELINE.json configs[0]: 4 stations, 6 baselines, 16 channels, 1024 samples, M=64, 16 outputs."""
     w = synth.WORKLOADS["tiny"]
@@ -65,7 +65,7 @@ def test_tiny_config(variant):
     assert flagged[~truth.numpy()].mean() < 0.1
 
 
-@pytest.mark.parametrize("variant", ["direct", "tma"])
+@pytest.mark.parametrize("variant", ["direct", "tma", "split"])
 def test_mini_lofar_several_tiles_autos_gain_bursts(variant):
     w = synth.WORKLOADS["lofar"].scaled(n_stations=6, n_time=1024, n_int=256, burst_cell_frac=0.1)
     assert w.n_cells == 21 * 64
@@ -73,7 +73,7 @@ def test_mini_lofar_several_tiles_autos_gain_bursts(variant):
     assert 0.001 < rep["oracle_flag_fraction"] < 0.2
 
 
-@pytest.mark.parametrize("variant", ["direct", "tma"])
+@pytest.mark.parametrize("variant", ["direct", "tma", "split"])
 @pytest.mark.parametrize("M,n_int,n_time", [(20, 100, 400), (10, 50, 200), (2, 8, 64), (3, 12, 48), (7, 28, 56),
                                               (64, 128, 256), (128, 256, 256), (16, 16, 64)])
 def test_window_sizes_and_ragged_channels(variant, M, n_int, n_time):
@@ -102,13 +102,13 @@ def test_cells_not_multiple_of_four_cannot_use_tma():
 @pytest.mark.parametrize("n_chan", [1, 8, 16, 32, 48, 96])
 def test_flag_word_layouts(n_chan):
     w = synth.Workload("words", 4, True, n_chan, 128, 8, 32, burst_cell_frac=0.3)
-    for variant in ("direct", "tma"):
+    for variant in ("direct", "tma", "split"):
         if variant == "tma" and w.n_cells % 4:
             continue
         check(w, [[1.0, 0.05, 1.0, 0.7]], variant, seed=n_chan)
 
 
-@pytest.mark.parametrize("variant", ["direct", "tma"])
+@pytest.mark.parametrize("variant", ["direct", "tma", "split"])
 def test_fp16_storage(variant):
     """configs[2] in miniature: fp16 storage, fp32 accumulation, CW tones on one channel.  Statistics against the
     oracle on the SAME fp16-rounded values at 2e-3; flag agreement >= 99.9 %."""
@@ -128,7 +128,7 @@ def test_fp16_storage(variant):
     assert q["flag_agreement_vs_fp32_original"] >= 0.999
 
 
-@pytest.mark.parametrize("variant", ["direct", "tma"])
+@pytest.mark.parametrize("variant", ["direct", "tma", "split"])
 def test_degenerate_inputs(variant):
     """All-zero cell, NaN / Inf samples, Hermitian (auto) cells, tiny and huge amplitudes, disabled detectors."""
     w = synth.Workload("degenerate", 4, True, 16, 256, 16, 64, burst_cell_frac=0.2)
@@ -212,7 +212,7 @@ def test_non_finite_and_degenerate_inputs_every_kernel_family(name, n_st, autos,
     assert out2["flags"].sum() == K * len(bad)
 
 
-@pytest.mark.parametrize("variant", ["direct", "tma"])
+@pytest.mark.parametrize("variant", ["direct", "tma", "split"])
 def test_exact_ties_are_not_flagged(variant):
     """r = |16 - 2*4|/16 = 0.5 exactly and tau = 0 exactly: thresholds equal to the statistic do not flag (Eq.(5),(10) strict)."""
     M = 16
@@ -309,6 +309,30 @@ def test_baseline_shards_equal_slices_of_the_full_run(K):
             np.testing.assert_array_equal(out[key], full[key][:, sl])
 
 
+def test_split_variant_against_the_direct_kernel_and_its_limits():
+    """RFI_VARIANT_SPLIT (small chunks, low latency): the SK statistic is bit-identical to the direct kernel (same block
+    statistics merged in the same order); alignment statistics and averages are summed block-wise: equal within the
+    parity tolerance.  Units with more than 96 blocks are rejected with a message; AUTO never picks it."""
+    w = synth.WORKLOADS["tiny"]
+    vis, _ = synth.make_chunk(w, seed=1234)
+    thr = synth.default_thresholds(w.window_M)
+    a, used_a = run_gpu(w, vis, thr, "direct")
+    b, used_b = run_gpu(w, vis, thr, "split")
+    c, used_c = run_gpu(w, vis, thr, "auto")
+    assert (used_a, used_b, used_c) == ("direct", "split", "direct")
+    np.testing.assert_array_equal(a["tau"], b["tau"])
+    assert np.abs(a["r_re"] - b["r_re"]).max() < 2e-6 and np.abs(a["r_im"] - b["r_im"]).max() < 2e-6
+    assert np.abs(a["avg"] - b["avg"]).max() <= 1e-5 * np.abs(a["avg"]).max()
+    big = synth.Workload("too_long", 4, True, 16, 1024, 16, 1024)             # 1024 / 4 = 256 blocks per unit
+    plan = rfi.RfiPlan(big.n_stations, big.n_baselines, big.n_chan, big.n_time, 16, n_int=1024)
+    plan.set_thresholds(thr); plan.set_variant("split")
+    avg, weight, _ = plan.alloc_outputs()
+    with pytest.raises(rfi.RfiError) as e:
+        plan.process_chunk(torch.zeros(1024, 10, 16, 4, 2, device="cuda"), avg, weight)
+    assert "small chunks" in str(e.value)
+    plan.destroy()
+
+
 def test_variants_agree_bit_for_bit(monkeypatch):
     """Same block length R (rows merged at a time) -> the two load paths feed identical arithmetic."""
     monkeypatch.setenv("RFI_DIRECT_ROWS", "4")
@@ -370,7 +394,7 @@ def test_batched_fp16_and_host_path():
 # ------------------------------------------------------------------------------------------------------
 # T x F window footprints (the paper's 10 x 2 and 5 x 4, W = 20)
 # ------------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("variant", ["direct", "tma"])
+@pytest.mark.parametrize("variant", ["direct", "tma", "split"])
 @pytest.mark.parametrize("T,F,n_chan", [(10, 2, 64), (5, 4, 64), (16, 2, 20), (4, 8, 24), (2, 32, 64), (8, 16, 48)])
 def test_tf_footprints(variant, T, F, n_chan):
     w = synth.Workload("tf", 5, True, n_chan, T * 24, T, T * 6, window_F=F, burst_cell_frac=0.15, channel_gain=True)
