@@ -397,6 +397,25 @@ def run_sim42(args):
     plan.destroy()
 
 
+def rank_chunk_and_plan(w, work, dev):
+    """This rank's input and plan (sharding.rank_work).  weak: its own subband chunk.  strong: every
+    rank draws the SAME chunk and keeps its contiguous baseline range; the plan then processes b_count baselines (no
+    exchange: PAPER.md:44, every stream is mitigated separately).  Returns (vis, truth [n_win, cells of this rank], plan)."""
+    import torch
+    import paper_2412_14775_b200 as rfi
+    from paper_2412_14775_b200 import synth
+    vis, truth = synth.make_chunk(w, seed=work["seed"], device=dev)
+    plan = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M,
+                       rfi.RFI_FP16 if w.fp16 else rfi.RFI_FP32, n_int=w.n_int)
+    if work["sharded"]:
+        b0, bc = work["b_first"], work["b_count"]
+        vis = vis[:, b0:b0 + bc].contiguous()
+        truth = truth.reshape(-1, w.n_baselines, w.n_chan)[:, b0:b0 + bc].reshape(truth.shape[0], -1).contiguous()
+        plan.set_baseline_shard(b0, bc)
+        torch.cuda.empty_cache()
+    return vis, truth, plan
+
+
 def run_ours(args):
     import numpy as np
     import torch
@@ -419,17 +438,7 @@ def run_ours(args):
     W = w.window_M * w.window_F
     thr = synth.default_thresholds(W) if args.K <= 1 else synth.sweep_thresholds(W, args.K)
     work = sharding.rank_work(w.n_baselines, world, rank, args.scaling)
-    vis, truth = synth.make_chunk(w, seed=work["seed"], device=dev)
-    plan = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M,
-                       rfi.RFI_FP16 if w.fp16 else rfi.RFI_FP32, n_int=w.n_int)
-    if work["sharded"]:
-        # strong scaling: every rank draws the SAME chunk and keeps its contiguous baseline range;
-        # the plan then processes b_count baselines (no exchange: PAPER.md:44, streams are mitigated separately)
-        b0, bc = work["b_first"], work["b_count"]
-        vis = vis[:, b0:b0 + bc].contiguous()
-        truth = truth.reshape(-1, w.n_baselines, w.n_chan)[:, b0:b0 + bc].reshape(truth.shape[0], -1).contiguous()
-        plan.set_baseline_shard(b0, bc)
-        torch.cuda.empty_cache()
+    vis, truth, plan = rank_chunk_and_plan(w, work, dev)
     if w.window_F > 1:
         plan.set_window_freq(w.window_F)
     if args.layout == "cell_major":

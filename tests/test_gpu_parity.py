@@ -659,3 +659,38 @@ def test_cell_major_layout_batched(fp16, n_chan, K):
     tm, _ = run_gpu(w, vis, thr, "auto")
     for key in ("avg", "weight", "flags", "tau", "r_re", "r_im"):
         np.testing.assert_array_equal(out[key], tm[key])
+
+
+def test_bench_strong_scaling_shards_reproduce_the_full_chunk():
+    """bench.py --gpus N --scaling strong on ONE GPU: the per-rank preparation (`bench.rank_chunk_and_plan` with
+    `sharding.rank_work`) run for every rank of a world of 3 in turn -- the shards' outputs are the slices of the
+    unsharded run bit for bit, and their sample counts add up to the one chunk (no multi-GPU box is available)."""
+    import bench
+    from paper_2412_14775_b200 import sharding
+    w = synth.WORKLOADS["lofar"].scaled(n_stations=7, n_time=512, n_int=256, burst_cell_frac=0.1)
+    thr = synth.default_thresholds(16)
+    dev = torch.device("cuda")
+    vis_full, _, plan_full = bench.rank_chunk_and_plan(w, sharding.rank_work(w.n_baselines, 1, 0, "strong"), dev)
+    plan_full.set_thresholds(thr)
+    avg_f, wt_f, _ = plan_full.alloc_outputs()
+    plan_full.process_chunk(vis_full, avg_f, wt_f)
+    torch.cuda.synchronize()
+    flags_f = plan_full.get_flags().clone()
+    world, total = 3, 0
+    for rank in range(world):
+        work = sharding.rank_work(w.n_baselines, world, rank, "strong")
+        vis, truth, plan = bench.rank_chunk_and_plan(w, work, dev)
+        assert work["sharded"] and vis.shape[1] == work["b_count"] and truth.shape[1] == work["b_count"] * w.n_chan
+        plan.set_thresholds(thr)
+        avg, wt, _ = plan.alloc_outputs()
+        plan.process_chunk(vis, avg, wt)
+        torch.cuda.synchronize()
+        b0, bc = work["b_first"], work["b_count"]
+        assert torch.equal(avg, avg_f[:, :, b0:b0 + bc]) and torch.equal(wt, wt_f[:, :, b0:b0 + bc])
+        assert torch.equal(plan.get_flags(), flags_f[:, :, b0:b0 + bc])
+        total += w.n_time * plan.n_cells
+        plan.destroy()
+    assert total == w.n_time * w.n_cells
+    weak = sharding.rank_work(w.n_baselines, world, 2, "weak")
+    assert not weak["sharded"] and weak["seed"] == 1236
+    plan_full.destroy()
