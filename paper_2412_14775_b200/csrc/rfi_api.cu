@@ -293,7 +293,11 @@ int enqueue_slab(rfi_plan* p, const void* d_vis_slab, int o_first, int n_out_sla
                 bt.t[k] = to_device_thr(p->thr[(size_t)(k0 + k) * nc], p->M * p->F);
                 bt.t1[k] = to_device_thr(p->thr[(size_t)(k0 + k) * nc + nc - 1], p->M * p->F);
             }
-            rc = launch_batched_tma_cellmajor(fp16, kp, bt, map, p->sm_count, p->smem_optin, st);
+            if (batched_mask_supported(kp))
+                rc = fp16 ? launch_batched_mask_f16(kp, bt, map, R, true, p->sm_count, p->smem_optin, st)
+                          : launch_batched_mask_f32(kp, bt, map, R, true, p->sm_count, p->smem_optin, st);
+            else
+                rc = launch_batched_tma_cellmajor(fp16, kp, bt, map, p->sm_count, p->smem_optin, st);
             if (rc != RFI_OK) return rc;
             p->launches++;
         }
@@ -321,8 +325,13 @@ int enqueue_slab(rfi_plan* p, const void* d_vis_slab, int o_first, int n_out_sla
                 bt.t[k] = to_device_thr(p->thr[(size_t)(k0 + k) * nc], p->M * p->F);
                 bt.t1[k] = to_device_thr(p->thr[(size_t)(k0 + k) * nc + nc - 1], p->M * p->F);
             }
-            const int rc = use_tma ? launch_batched_tma(fp16, kp, bt, map, R, p->sm_count, p->smem_optin, st)
-                                   : launch_batched(fp16, kp, bt, st);
+            int rc;
+            if (use_tma && batched_mask_supported(kp))
+                rc = fp16 ? launch_batched_mask_f16(kp, bt, map, R, false, p->sm_count, p->smem_optin, st)
+                          : launch_batched_mask_f32(kp, bt, map, R, false, p->sm_count, p->smem_optin, st);
+            else
+                rc = use_tma ? launch_batched_tma(fp16, kp, bt, map, R, p->sm_count, p->smem_optin, st)
+                             : launch_batched(fp16, kp, bt, st);
             if (rc != RFI_OK) return rc;
             p->launches++;
         }

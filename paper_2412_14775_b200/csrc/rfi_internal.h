@@ -78,4 +78,13 @@ bool batched_tma_supported(bool fp16, const rfi::KParams& kp, int R);
 int launch_batched_tma(bool fp16, const rfi::KParams& kp, const rfi::BatchThr& bt, const CUtensorMap* map, int R,
                        int sm_count, int smem_optin, cudaStream_t st);
 
+// second-generation batched kernel (rfi_batched_mask.cuh): whole-word tiles only (n_chan % 32 == 0)
+int launch_batched_mask_f32(const rfi::KParams& kp, const rfi::BatchThr& bt, const CUtensorMap* map, int R, bool cell_major,
+                            int sm_count, int smem_optin, cudaStream_t st);
+int launch_batched_mask_f16(const rfi::KParams& kp, const rfi::BatchThr& bt, const CUtensorMap* map, int R, bool cell_major,
+                            int sm_count, int smem_optin, cudaStream_t st);
+inline bool batched_mask_supported(const rfi::KParams& kp) {
+    return kp.n_chan % 32 == 0 && env_int("RFI_BT_MASK", 1) != 0;
+}
+
 }  // namespace rfi_host
