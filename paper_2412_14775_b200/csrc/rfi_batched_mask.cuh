@@ -13,9 +13,12 @@
 //   contract  thread (warp j, lane l) owns cell l and the sets j*SPW .. j*SPW+SPW-1.  Per record: one predicate per
 //             set from the mask bits, a 0/1 factor, 4 packed fma (exactly acc + sum or acc: see contract_one in
 //             rfi_batched_tma.cuh), a predicated count.
-//   pipeline  the contraction of round g-1 is interleaved, block by block, with the streaming of round g (records are
-//             double-buffered, one CTA barrier per round): the TMA ring keeps refilling while the warp contracts, so
-//             HBM does not idle during the contraction as it does when the two phases alternate.
+//   staging   the flag layout has the tile index fastest (include/rfi.h), so one tile's words are 4 isolated bytes per
+//             (set, window): 32 distinct lines per store instruction, measured at 0.3 ms of a 3.4 ms K = 64 pass.  A CTA
+//             therefore takes G adjacent tiles of one integration in a row (G = 8 when the row length allows) and every
+//             stream warp parks the flag words of its own windows in tensor memory (tcgen05.st, 32 lanes x one column
+//             per word: TMEM is otherwise unused by this path and shared memory is full); after the G-th tile the same
+//             warp reads them back (tcgen05.ld.x8) and stores whole 32-byte sectors.  No cross-warp hand-off.
 //
 // The sums are added per set in window order, as in the single-set kernels: K sets equal K single-set runs bit for bit.
 #pragma once
@@ -100,10 +103,72 @@ __device__ __forceinline__ void contract_records(uint32_t rbuf, int j0, int j1, 
     }
 }
 
-template <int R, bool FP16, int SPW, bool CM, bool PIPE>
+// ---- tensor memory as per-warp scratch (flag-word staging) ----
+__device__ __forceinline__ void tmem_alloc(uint32_t smem_slot, uint32_t cols) {          // one whole warp
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_slot), "r"(cols) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t cols) {             // one whole warp
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(cols) : "memory");
+}
+__device__ __forceinline__ void tmem_st1(uint32_t taddr, uint32_t v) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x1.b32 [%0], {%1};" ::"r"(taddr), "r"(v) : "memory");
+}
+template <int G>
+__device__ __forceinline__ void tmem_ld(uint32_t taddr, uint32_t (&r)[G]) {
+    static_assert(G == 2 || G == 4 || G == 8, "group sizes");
+    if constexpr (G == 8)
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                     : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]) : "r"(taddr) : "memory");
+    else if constexpr (G == 4)
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];"
+                     : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(taddr) : "memory");
+    else
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0,%1}, [%2];" : "=r"(r[0]), "=r"(r[1]) : "r"(taddr) : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+template <int G>
+__device__ __forceinline__ void stg_words(uint32_t* dst, const uint32_t (&r)[G]) {        // dst aligned to 4 G bytes
+    if constexpr (G == 8)
+        asm volatile("st.global.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(dst), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]),
+                     "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]) : "memory");
+    else if constexpr (G == 4)
+        asm volatile("st.global.v4.b32 [%0], {%1,%2,%3,%4};" ::"l"(dst), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]) : "memory");
+    else
+        asm volatile("st.global.v2.b32 [%0], {%1,%2};" ::"l"(dst), "r"(r[0]), "r"(r[1]) : "memory");
+}
+
+// One warp's parked flag words of a finished tile group: for each of its windows (round ri, window ri*NW + warp) and
+// each half of the sets (lane k: set k, set 32 + k), G consecutive TMEM columns = the words of tiles tile0 .. tile0+G-1.
+template <int G>
+__device__ __forceinline__ void flush_group_flags(const KParams& p, uint32_t tcol, int n_rounds, int warp, int lane, int n_valid,
+                                                  uint32_t* flag_lo, size_t flag_set_stride, size_t fwpw, int o_global, int tile0) {
+    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+    const int halves = p.K > 32 ? 2 : 1;
+    for (int ri = 0; ri < n_rounds; ++ri) {
+        const int wl = ri * kBtWarps + warp;
+        if (wl >= p.wpo) break;
+        for (int h = 0; h < halves; ++h) {
+            uint32_t r[G];
+            tmem_ld<G>(tcol + (uint32_t)((ri * 2 + h) * G), r);
+            if (lane + 32 * h < p.K) {
+                uint32_t* dst = flag_lo + (size_t)(32 * h) * flag_set_stride + ((size_t)o_global * p.wpo + wl) * fwpw + tile0;
+                if (n_valid == G) {
+                    stg_words<G>(dst, r);
+                } else {                                       // ragged last group of a row
+#pragma unroll
+                    for (int j = 0; j < G; ++j)
+                        if (j < n_valid) dst[j] = r[j];
+                }
+            }
+        }
+    }
+}
+
+template <int R, bool FP16, int SPW, bool CM>
 __global__ void __launch_bounds__(kBtWarps * 32, 1)
 rfi_batched_mask_kernel(const __grid_constant__ CUtensorMap tmap, const KParams p,
-                        const __grid_constant__ BatchThr bt, const int stages) {
+                        const __grid_constant__ BatchThr bt, const int stages, const int G, const int tm_cols) {
     constexpr int NW = kBtWarps;
     constexpr int ROW_BYTES = FP16 ? 512 : 1024;
     static_assert(!CM || R == (FP16 ? 8 : 4), "cell-major stages hold one 128-byte line per cell");
@@ -117,21 +182,24 @@ rfi_batched_mask_kernel(const __grid_constant__ CUtensorMap tmap, const KParams 
     const uint32_t rec_base = smem_base + (uint32_t)NW * stages * STAGE_BYTES;          // [2][NW] records
     const uint32_t tbl_base = rec_base + 2u * NW * kBmRecBytes;                          // [2 classes] tables
     const uint32_t perm_base = tbl_base + 2u * kBmTblBytes;                              // [6][64] u8 sort permutations
-    const uint32_t bars = perm_base + 384u + (uint32_t)warp * stages * 16;               // per warp: full[], empty[]
+    const uint32_t tm_slot = perm_base + 384u;                                           // TMEM base address (one word)
+    const uint32_t round_bar = tm_slot + 8u;                                             // records of a round complete (all threads arrive)
+    const uint32_t bars = tm_slot + 16u + (uint32_t)warp * stages * 16;                  // per warp: full[], empty[]
     const uint32_t ebars = bars + (uint32_t)stages * 8;
 
+    // Work list: super-unit = (group of G adjacent tiles, output integration); its tiles are units taken in a row.
     const int n_tiles = p.n_cells >> 5;                       // whole tiles only (n_chan % 32 == 0)
-    const int n_units = n_tiles * p.n_out_slab;
-    if ((int)blockIdx.x >= n_units) return;
-    const int my_units = (n_units - 1 - (int)blockIdx.x) / (int)gridDim.x + 1;
+    const int n_groups = (n_tiles + G - 1) / G;
+    const int n_su = n_groups * p.n_out_slab;
+    if ((int)blockIdx.x >= n_su) return;
     const int bpw = p.M / R;                                  // stages per window
     const int n_rounds = (p.wpo + NW - 1) / NW;
-    const int my_n = warp < p.wpo ? (p.wpo - 1 - warp) / NW + 1 : 0;     // windows of a unit streamed by this warp
-    const int total = my_units * my_n * bpw;                  // stages this warp consumes in its lifetime
     const float inv_M = p.inv_W;                              // 1/W, W = T*F
     const size_t fwpw = (size_t)p.n_baselines * p.wpb;        // flag words per window
     const size_t flag_set_stride = (size_t)p.n_win_total * fwpw;
+    const int step_o = (int)gridDim.x / n_groups, step_g = (int)gridDim.x - step_o * n_groups;   // su += gridDim.x
 
+    if (threadIdx.x == 0) mbar_init(round_bar, NW * 32);
     if (lane == 0) {
         for (int s = 0; s < stages; ++s) { mbar_init(bars + 8 * s, 1); mbar_init(ebars + 8 * s, 32); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -139,35 +207,39 @@ rfi_batched_mask_kernel(const __grid_constant__ CUtensorMap tmap, const KParams 
     }
     __syncwarp();
 
-    // ---- producer cursor (lane 0 only): unit -> window (warp, warp+NW, ...) -> stage; no divisions on the way ----
+    // ---- producer cursor (lane 0 only): super-unit -> tile of the group -> window (warp, warp+NW, ...) -> stage ----
     uint64_t pol = 0;
-    const int step_o = (int)gridDim.x / n_tiles, step_t = (int)gridDim.x - step_o * n_tiles;   // unit += gridDim.x
-    int pr_left = total, pr_wl = warp, pr_b = 0;
-    int pr_o = (int)blockIdx.x / n_tiles, pr_tile = (int)blockIdx.x - pr_o * n_tiles;
+    bool pr_active = warp < p.wpo;
+    int pr_su = blockIdx.x, pr_o = (int)blockIdx.x / n_groups, pr_grp = (int)blockIdx.x - pr_o * n_groups;
+    int pr_j = 0, pr_wl = warp, pr_b = 0;
     auto pr_issue = [&](int s) {
         const uint32_t bar = bars + 8 * s;
         const uint32_t dst = ring + (uint32_t)s * STAGE_BYTES;
         const int row = pr_o * p.n_int + pr_wl * p.M + pr_b * R;
+        const int tile = pr_grp * G + pr_j;
         mbar_expect_tx(bar, STAGE_BYTES);
-        if constexpr (CM)        tma_load_3d(dst, &tmap, 0, row / R, pr_tile * 32, bar, pol);
-        else if constexpr (FP16) tma_load_2d(dst, &tmap, pr_tile * 128, row, bar, pol);
-        else                     tma_load_3d(dst, &tmap, 0, pr_tile * 8, row, bar, pol);
-        --pr_left;
+        if constexpr (CM)        tma_load_3d(dst, &tmap, 0, row / R, tile * 32, bar, pol);
+        else if constexpr (FP16) tma_load_2d(dst, &tmap, tile * 128, row, bar, pol);
+        else                     tma_load_3d(dst, &tmap, 0, tile * 8, row, bar, pol);
         if (++pr_b == bpw) {
             pr_b = 0;
             pr_wl += NW;
             if (pr_wl >= p.wpo) {
                 pr_wl = warp;
-                pr_o += step_o;
-                pr_tile += step_t;
-                if (pr_tile >= n_tiles) { pr_tile -= n_tiles; ++pr_o; }
+                if (++pr_j == G || pr_grp * G + pr_j >= n_tiles) {
+                    pr_j = 0;
+                    pr_su += gridDim.x;
+                    pr_o += step_o;
+                    pr_grp += step_g;
+                    if (pr_grp >= n_groups) { pr_grp -= n_groups; ++pr_o; }
+                    pr_active = pr_su < n_su;
+                }
             }
         }
     };
-    if (lane == 0 && total > 0) {
+    if (lane == 0 && pr_active) {
         pol = l2_evict_first_policy();
-        const int pre = total < stages ? total : stages;
-        for (int i = 0; i < pre; ++i) pr_issue(i);
+        for (int i = 0; i < stages && pr_active; ++i) pr_issue(i);
     }
 
     // ---- per-CTA threshold tables: the K sets sorted by x_low, x_high, gamma; prefix masks by rank ----
@@ -189,7 +261,10 @@ rfi_batched_mask_kernel(const __grid_constant__ CUtensorMap tmap, const KParams 
             sts_f32(tbl_base + cls * kBmTblBytes + kind * 256 + rank * 4, v);
             asm volatile("st.shared.u8 [%0], %1;" ::"r"(perm_base + a * 64 + rank), "r"(i) : "memory");
         }
+        if (warp == NW - 1 && G > 1) tmem_alloc(tm_slot, (uint32_t)tm_cols);    // flag staging (warp NW-1 is idle above)
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
         __syncthreads();
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         if (t < 390) {
             const int a = t / 65, n = t - a * 65, cls = a / 3, kind = a - 3 * cls;
             unsigned long long m = 0ull;
@@ -203,6 +278,9 @@ rfi_batched_mask_kernel(const __grid_constant__ CUtensorMap tmap, const KParams 
         }
         __syncthreads();
     }
+    const uint32_t tm_base = G > 1 ? lds_u32(tm_slot) : 0u;
+    // this warp's TMEM window: its lane quarter (warp % 4), columns [(warp / 4) * n_rounds * 2 G, +n_rounds * 2 G)
+    const uint32_t tcol = tm_base + ((uint32_t)(warp & 3) << 21) + (uint32_t)((warp >> 2) * n_rounds * 2 * G);
 
     // lane-constant shared-memory offsets of this lane's sample inside one row (see rfi_tma_kernel)
     uint32_t off0, off1;
@@ -221,124 +299,117 @@ rfi_batched_mask_kernel(const __grid_constant__ CUtensorMap tmap, const KParams 
     const int align = 32 - SPW - ((warp * SPW) & 31);
     f2 acc[SPW][4];
     uint32_t cnt[SPW];
-    auto reset_acc = [&]() {
-#pragma unroll
-        for (int i = 0; i < SPW; ++i) {
-            cnt[i] = 0u;
-#pragma unroll
-            for (int q = 0; q < 4; ++q) acc[i][q] = 0ull;
-        }
-    };
-    auto store_unit = [&](int tile, int o_global) {           // the unit's K averaged outputs
-        LaneGeom g;
-        g.cell = tile * 32 + lane;
-        g.valid = true;
-#pragma unroll
-        for (int i = 0; i < SPW; ++i) {
-            const int k = warp * SPW + i;
-            if (k < p.K) store_output(p, g, p.k_first + k, o_global, acc[i], cnt[i] * (uint32_t)p.M);
-        }
-    };
-    reset_acc();
 
-    // stream side: lane k stores the flag words of sets k and 32 + k
+    // stream side: lane k handles the flag words of sets k and 32 + k
     uint32_t* const flag_lo = p.flags + (size_t)(p.k_first + lane) * flag_set_stride;
-    uint32_t* const flag_hi = flag_lo + 32 * flag_set_stride;
 
     int stage = 0;
-    uint32_t parity = 0;
-    int o_local = (int)blockIdx.x / n_tiles, tile = (int)blockIdx.x - o_local * n_tiles;
-    int prev_tile = 0, prev_o_global = 0, prev_n = 0;         // the round whose records wait to be contracted
-    bool prev_last = false;
-    uint32_t gr = 0;
-    for (int ui = 0; ui < my_units; ++ui) {
+    uint32_t parity = 0, gr = 0;
+    int o_local = (int)blockIdx.x / n_groups, grp = (int)blockIdx.x - o_local * n_groups;
+    for (int su = blockIdx.x; su < n_su; su += gridDim.x) {
         const int o_global = p.o_first + o_local;
-        const int cls = p.cls ? (int)p.cls[p.b_first + (tile * 32) / p.n_chan] : 0;     // a whole-word tile lies in one baseline
-        const uint32_t tbl = tbl_base + (uint32_t)cls * kBmTblBytes;
-        LaneGeom g;
-        g.cell = tile * 32 + lane;
-        g.valid = true;
-
-        for (int round = 0; round < n_rounds; ++round, ++gr) {
-            const uint32_t wbuf = rec_base + (gr & 1u) * (NW * kBmRecBytes);
-            const uint32_t pbuf = rec_base + ((gr & 1u) ^ 1u) * (NW * kBmRecBytes);
-            const int wl = round * NW + warp;
-            const int n_w = min(NW, p.wpo - round * NW);
-            if (wl < p.wpo) {
-                Win w;
-                w.reset();
-                for (int b = 0; b < bpw; ++b) {
-                    mbar_wait(bars + 8 * stage, parity);
-                    const uint32_t sbase = ring + (uint32_t)stage * STAGE_BYTES;
-                    Raw<FP16> buf[R];
+        const int tile0 = grp * G;
+        const int n_valid = min(G, n_tiles - tile0);          // tiles of this group
+        for (int j = 0; j < n_valid; ++j) {
+            const int tile = tile0 + j;
+            const int cls = p.cls ? (int)p.cls[p.b_first + (tile * 32) / p.n_chan] : 0;     // a whole-word tile lies in one baseline
+            const uint32_t tbl = tbl_base + (uint32_t)cls * kBmTblBytes;
+            LaneGeom g;
+            g.cell = tile * 32 + lane;
+            g.valid = true;
 #pragma unroll
-                    for (int r = 0; r < R; ++r) {
-                        if constexpr (CM) {
-                            const uint32_t line = sbase + (uint32_t)lane * 128u, sx = (uint32_t)lane & 7u;
-                            if constexpr (FP16) lds_raw(line + (((uint32_t)r ^ sx) << 4), 0, buf[r]);
-                            else                lds_raw(line + (((uint32_t)(2 * r) ^ sx) << 4), line + (((uint32_t)(2 * r + 1) ^ sx) << 4), buf[r]);
+            for (int i = 0; i < SPW; ++i) {
+                cnt[i] = 0u;
+#pragma unroll
+                for (int q = 0; q < 4; ++q) acc[i][q] = 0ull;
+            }
+
+            for (int round = 0; round < n_rounds; ++round, ++gr) {
+                const uint32_t rbuf = rec_base + (gr & 1u) * (NW * kBmRecBytes);
+                const int wl = round * NW + warp;
+                if (wl < p.wpo) {
+                    Win w;
+                    w.reset();
+                    for (int b = 0; b < bpw; ++b) {
+                        mbar_wait(bars + 8 * stage, parity);
+                        const uint32_t sbase = ring + (uint32_t)stage * STAGE_BYTES;
+                        Raw<FP16> buf[R];
+#pragma unroll
+                        for (int r = 0; r < R; ++r) {
+                            if constexpr (CM) {
+                                const uint32_t line = sbase + (uint32_t)lane * 128u, sx = (uint32_t)lane & 7u;
+                                if constexpr (FP16) lds_raw(line + (((uint32_t)r ^ sx) << 4), 0, buf[r]);
+                                else                lds_raw(line + (((uint32_t)(2 * r) ^ sx) << 4), line + (((uint32_t)(2 * r + 1) ^ sx) << 4), buf[r]);
+                            } else {
+                                lds_raw(sbase + r * ROW_BYTES + off0, sbase + r * ROW_BYTES + off1, buf[r]);
+                            }
+                        }
+                        // stage hand-off (rfi_common.cuh): 32 arrivals after the loads, wait, proxy fence, refill
+                        mbar_arrive(ebars + 8 * stage);
+                        if (lane == 0 && pr_active) {
+                            mbar_wait(ebars + 8 * stage, parity);
+                            fence_proxy_async();
+                            pr_issue(stage);
+                        }
+                        accumulate_block<R, FP16>(w, buf, b);
+                        if (++stage == stages) { stage = 0; parity ^= 1u; }
+                    }
+                    float x, r_re, r_im;
+                    if (p.F > 1) combine_group(w, p.F, p.M);
+                    window_stats(w, inv_M, x, r_re, r_im);
+                    const int w_global = o_global * p.wpo + wl;
+                    uint32_t m_lo, m_hi;
+                    keep_mask(tbl, x, max_nan(r_re, r_im), m_lo, m_hi);
+                    // record: keep mask + window sums (zeros if not finite: such a window is kept by no set, and
+                    // fma(NaN, 0, acc) would poison the accumulator)
+                    const uint32_t ra = rbuf + (uint32_t)warp * kBmRecBytes;
+                    sts_u32(ra + (uint32_t)lane * 4u, m_lo);
+                    sts_u32(ra + 128u + (uint32_t)lane * 4u, m_hi);
+                    const bool fin = finite2(w.s[0]) && finite2(w.s[1]) && finite2(w.s[2]) && finite2(w.s[3]);
+                    sts128_f2(ra + 256u + (uint32_t)lane * 16u, fin ? w.s[0] : 0ull, fin ? w.s[1] : 0ull);
+                    sts128_f2(ra + 768u + (uint32_t)lane * 16u, fin ? w.s[2] : 0ull, fin ? w.s[3] : 0ull);
+                    // The record is out: arrive on the round barrier, then do what nobody waits for.
+                    mbar_arrive(round_bar);
+                    // flag words: transpose (cell, set) -> (set, cell); flagged = not kept
+                    {
+                        const uint32_t f_lo = ~warp_transpose32(m_lo, lane);
+                        const uint32_t f_hi = p.K > 32 ? ~warp_transpose32(m_hi, lane) : 0u;
+                        if (G > 1) {                           // park them until the group's last tile
+                            tmem_st1(tcol + (uint32_t)((round * 2) * G + j), f_lo);
+                            if (p.K > 32) tmem_st1(tcol + (uint32_t)((round * 2 + 1) * G + j), f_hi);
                         } else {
-                            lds_raw(sbase + r * ROW_BYTES + off0, sbase + r * ROW_BYTES + off1, buf[r]);
+                            const size_t wo = (size_t)w_global * fwpw + tile;
+                            if (lane < p.K) flag_lo[wo] = f_lo;
+                            if (lane + 32 < p.K) flag_lo[32 * flag_set_stride + wo] = f_hi;
                         }
                     }
-                    // stage hand-off (rfi_common.cuh): 32 arrivals after the loads, wait, proxy fence, refill
-                    mbar_arrive(ebars + 8 * stage);
-                    if (lane == 0 && pr_left > 0) {
-                        mbar_wait(ebars + 8 * stage, parity);
-                        fence_proxy_async();
-                        pr_issue(stage);
-                    }
-                    accumulate_block<R, FP16>(w, buf, b);
-                    if (++stage == stages) { stage = 0; parity ^= 1u; }
-                    if constexpr (PIPE) {                      // a slice of the previous round's records
-                        contract_records<SPW>(pbuf, (b * prev_n) / bpw, ((b + 1) * prev_n) / bpw, lane, msel, align, acc, cnt);
-                    }
+                    if (p.k_first == 0) store_stats(p, g, w_global, (cls ? p.thr1.c : p.thr0.c) * x, r_re, r_im);
+                } else {
+                    mbar_arrive(round_bar);
                 }
-                float x, r_re, r_im;
-                if (p.F > 1) combine_group(w, p.F, p.M);
-                window_stats(w, inv_M, x, r_re, r_im);
-                const int w_global = o_global * p.wpo + wl;
-                uint32_t m_lo, m_hi;
-                keep_mask(tbl, x, max_nan(r_re, r_im), m_lo, m_hi);
-                // record: keep mask + window sums (zeros if not finite: such a window is kept by no set, and
-                // fma(NaN, 0, acc) would poison the accumulator)
-                const uint32_t ra = wbuf + (uint32_t)warp * kBmRecBytes;
-                sts_u32(ra + (uint32_t)lane * 4u, m_lo);
-                sts_u32(ra + 128u + (uint32_t)lane * 4u, m_hi);
-                const bool fin = finite2(w.s[0]) && finite2(w.s[1]) && finite2(w.s[2]) && finite2(w.s[3]);
-                sts128_f2(ra + 256u + (uint32_t)lane * 16u, fin ? w.s[0] : 0ull, fin ? w.s[1] : 0ull);
-                sts128_f2(ra + 768u + (uint32_t)lane * 16u, fin ? w.s[2] : 0ull, fin ? w.s[3] : 0ull);
-                // flag words: transpose (cell, set) -> (set, cell); flagged = not kept
-                {
-                    const size_t wo = (size_t)w_global * fwpw + tile;
-                    const uint32_t t_lo = warp_transpose32(m_lo, lane);
-                    if (lane < p.K) flag_lo[wo] = ~t_lo;
-                    if (p.K > 32) {
-                        const uint32_t t_hi = warp_transpose32(m_hi, lane);
-                        if (lane + 32 < p.K) flag_hi[wo] = ~t_hi;
-                    }
-                }
-                if (p.k_first == 0) store_stats(p, g, w_global, (cls ? p.thr1.c : p.thr0.c) * x, r_re, r_im);
-            } else if constexpr (PIPE) {
-                contract_records<SPW>(pbuf, 0, prev_n, lane, msel, align, acc, cnt);
+                mbar_wait(round_bar, gr & 1u);                 // every warp's record of this round is in shared memory
+                contract_records<SPW>(rbuf, 0, min(NW, p.wpo - round * NW), lane, msel, align, acc, cnt);
             }
-            if constexpr (PIPE) {
-                if (prev_last) { store_unit(prev_tile, prev_o_global); reset_acc(); }
-                prev_n = n_w; prev_tile = tile; prev_o_global = o_global; prev_last = round == n_rounds - 1;
-                __syncthreads();
-            } else {
-                __syncthreads();
-                contract_records<SPW>(wbuf, 0, n_w, lane, msel, align, acc, cnt);
+#pragma unroll
+            for (int i = 0; i < SPW; ++i) {                     // the unit's averaged outputs
+                const int k = warp * SPW + i;
+                if (k < p.K) store_output(p, g, p.k_first + k, o_global, acc[i], cnt[i] * (uint32_t)p.M);
             }
         }
-        if constexpr (!PIPE) { store_unit(tile, o_global); reset_acc(); }
+        if (G > 1) {
+            if (G == 8)      flush_group_flags<8>(p, tcol, n_rounds, warp, lane, n_valid, flag_lo, flag_set_stride, fwpw, o_global, tile0);
+            else if (G == 4) flush_group_flags<4>(p, tcol, n_rounds, warp, lane, n_valid, flag_lo, flag_set_stride, fwpw, o_global, tile0);
+            else             flush_group_flags<2>(p, tcol, n_rounds, warp, lane, n_valid, flag_lo, flag_set_stride, fwpw, o_global, tile0);
+        }
         o_local += step_o;
-        tile += step_t;
-        if (tile >= n_tiles) { tile -= n_tiles; ++o_local; }
+        grp += step_g;
+        if (grp >= n_groups) { grp -= n_groups; ++o_local; }
     }
-    if constexpr (PIPE) {                                      // drain: the last round's records
-        contract_records<SPW>(rec_base + ((gr & 1u) ^ 1u) * (NW * kBmRecBytes), 0, prev_n, lane, msel, align, acc, cnt);
-        store_unit(prev_tile, prev_o_global);
+    if (G > 1) {                                               // every warp is done with its columns
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncthreads();
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        if (warp == NW - 1) tmem_dealloc(tm_base, (uint32_t)tm_cols);
     }
 }
 

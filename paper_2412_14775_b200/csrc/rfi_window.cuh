@@ -208,8 +208,15 @@ __device__ __forceinline__ void store_output(const KParams& p, const LaneGeom& g
         lo = hi = make_float4(0.f, 0.f, 0.f, 0.f);
     }
     float4* dst = reinterpret_cast<float4*>(p.avg + oi * 8);
-    dst[0] = lo;
-    dst[1] = hi;
+    if ((reinterpret_cast<uintptr_t>(dst) & 31u) == 0) {
+        // one 256-bit store: the cell's 32-byte sector leaves whole (two 128-bit stores write it in halves, which the
+        // load/store unit handles as two transactions per sector: measurable in the K-set kernels, 64 outputs per unit)
+        asm volatile("st.global.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(dst), "f"(lo.x), "f"(lo.y), "f"(lo.z), "f"(lo.w),
+                     "f"(hi.x), "f"(hi.y), "f"(hi.z), "f"(hi.w) : "memory");
+    } else {
+        dst[0] = lo;
+        dst[1] = hi;
+    }
     p.weight[oi] = wt;
 }
 
