@@ -130,12 +130,12 @@ __device__ __forceinline__ void tmem_ld(uint32_t taddr, uint32_t (&r)[G]) {
 template <int G>
 __device__ __forceinline__ void stg_words(uint32_t* dst, const uint32_t (&r)[G]) {        // dst aligned to 4 G bytes
     if constexpr (G == 8)
-        asm volatile("st.global.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(dst), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]),
+        asm volatile("st.global.L1::no_allocate.L2::evict_first.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(dst), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]),
                      "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]) : "memory");
     else if constexpr (G == 4)
-        asm volatile("st.global.v4.b32 [%0], {%1,%2,%3,%4};" ::"l"(dst), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]) : "memory");
+        asm volatile("st.global.cs.v4.b32 [%0], {%1,%2,%3,%4};" ::"l"(dst), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]) : "memory");
     else
-        asm volatile("st.global.v2.b32 [%0], {%1,%2};" ::"l"(dst), "r"(r[0]), "r"(r[1]) : "memory");
+        asm volatile("st.global.cs.v2.b32 [%0], {%1,%2};" ::"l"(dst), "r"(r[0]), "r"(r[1]) : "memory");
 }
 
 // One warp's parked flag words of a finished tile group: for each of its windows (round ri, window ri*NW + warp) and
