@@ -308,10 +308,15 @@ int enqueue_slab(rfi_plan* p, const void* d_vis_slab, int o_first, int n_out_sla
         p->last_variant = RFI_VARIANT_BATCHED;
         // same block length as the single-set direct kernel whenever that one uses R <= 4 (fp32) / 8 (fp16): then
         // K sets equal K single-set runs bit for bit
-        const int R = pick_rows(p->M, fp16, fp16 ? 8 : 4);
+        int R = pick_rows(p->M, fp16, fp16 ? 8 : 4);
+        // the second-generation kernel also has R = 5 (the paper's T = 10 and T = 5, as the direct kernel takes them)
+        const int R5 = pick_rows(p->M, fp16, fp16 ? 8 : 5);
+        const bool mask_ok = batched_mask_supported(kp) && tma_allowed(p) && env_int("RFI_BATCHED_TMA", 1) != 0;
+        if (mask_ok && batched_mask_rows(fp16, R5)) R = R5;
         CUtensorMap map_v;
         const CUtensorMap* map = &map_v;
-        const bool use_tma = batched_tma_supported(fp16, kp, R) && tma_allowed(p);
+        const bool use_mask = mask_ok && batched_mask_rows(fp16, R);
+        const bool use_tma = use_mask || (batched_tma_supported(fp16, kp, R) && tma_allowed(p));
         if (use_tma) {
             const int rc = get_tensor_map(p, kp.vis, n_out_slab * p->n_int, R, &map_v);
             if (rc != RFI_OK) return rc;
@@ -326,7 +331,7 @@ int enqueue_slab(rfi_plan* p, const void* d_vis_slab, int o_first, int n_out_sla
                 bt.t1[k] = to_device_thr(p->thr[(size_t)(k0 + k) * nc + nc - 1], p->M * p->F);
             }
             int rc;
-            if (use_tma && batched_mask_supported(kp))
+            if (use_mask)
                 rc = fp16 ? launch_batched_mask_f16(kp, bt, map, R, false, p->sm_count, p->smem_optin, st)
                           : launch_batched_mask_f32(kp, bt, map, R, false, p->sm_count, p->smem_optin, st);
             else

@@ -1,6 +1,6 @@
 // rfi_batched_mask.cuh -- batched-threshold kernel, second generation: K <= 64 threshold sets in ONE pass over the
 // data, for whole-word tiles (n_chan % 32 == 0).  Same function and same bits as rfi_batched_tma.cuh (which remains for
-// ragged channel counts); what differs is where the K decisions are taken and when the masked sums are formed.
+// ragged channel counts); what differs is where the K decisions are taken and how the flag words leave.
 //
 //   decide    once per (window, cell), by the thread that streamed the window: the K decisions of Eq.(5) / Eq.(10)
 //              are three rank queries.  With the sets sorted by s_low / s_high / gamma (done once
@@ -141,7 +141,7 @@ __device__ __forceinline__ void stg_words(uint32_t* dst, const uint32_t (&r)[G])
 // One warp's parked flag words of a finished tile group: for each of its windows (round ri, window ri*NW + warp) and
 // each half of the sets (lane k: set k, set 32 + k), G consecutive TMEM columns = the words of tiles tile0 .. tile0+G-1.
 template <int G>
-__device__ __forceinline__ void flush_group_flags(const KParams& p, uint32_t tcol, int n_rounds, int warp, int lane, int n_valid,
+__device__ __forceinline__ void flush_group_flags(const KParams& p, uint32_t tcol, int n_rounds, int warp, int lane,
                                                   uint32_t* flag_lo, size_t flag_set_stride, size_t fwpw, int o_global, int tile0) {
     asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
     const int halves = p.K > 32 ? 2 : 1;
@@ -153,13 +153,7 @@ __device__ __forceinline__ void flush_group_flags(const KParams& p, uint32_t tco
             tmem_ld<G>(tcol + (uint32_t)((ri * 2 + h) * G), r);
             if (lane + 32 * h < p.K) {
                 uint32_t* dst = flag_lo + (size_t)(32 * h) * flag_set_stride + ((size_t)o_global * p.wpo + wl) * fwpw + tile0;
-                if (n_valid == G) {
-                    stg_words<G>(dst, r);
-                } else {                                       // ragged last group of a row
-#pragma unroll
-                    for (int j = 0; j < G; ++j)
-                        if (j < n_valid) dst[j] = r[j];
-                }
+                stg_words<G>(dst, r);
             }
         }
     }
@@ -189,7 +183,7 @@ rfi_batched_mask_kernel(const __grid_constant__ CUtensorMap tmap, const KParams 
 
     // Work list: super-unit = (group of G adjacent tiles, output integration); its tiles are units taken in a row.
     const int n_tiles = p.n_cells >> 5;                       // whole tiles only (n_chan % 32 == 0)
-    const int n_groups = (n_tiles + G - 1) / G;
+    const int n_groups = n_tiles / G;                         // G divides the flag row length = n_tiles (launcher)
     const int n_su = n_groups * p.n_out_slab;
     if ((int)blockIdx.x >= n_su) return;
     const int bpw = p.M / R;                                  // stages per window
@@ -226,7 +220,7 @@ rfi_batched_mask_kernel(const __grid_constant__ CUtensorMap tmap, const KParams 
             pr_wl += NW;
             if (pr_wl >= p.wpo) {
                 pr_wl = warp;
-                if (++pr_j == G || pr_grp * G + pr_j >= n_tiles) {
+                if (++pr_j == G) {
                     pr_j = 0;
                     pr_su += gridDim.x;
                     pr_o += step_o;
@@ -309,8 +303,7 @@ rfi_batched_mask_kernel(const __grid_constant__ CUtensorMap tmap, const KParams 
     for (int su = blockIdx.x; su < n_su; su += gridDim.x) {
         const int o_global = p.o_first + o_local;
         const int tile0 = grp * G;
-        const int n_valid = min(G, n_tiles - tile0);          // tiles of this group
-        for (int j = 0; j < n_valid; ++j) {
+        for (int j = 0; j < G; ++j) {
             const int tile = tile0 + j;
             const int cls = p.cls ? (int)p.cls[p.b_first + (tile * 32) / p.n_chan] : 0;     // a whole-word tile lies in one baseline
             const uint32_t tbl = tbl_base + (uint32_t)cls * kBmTblBytes;
@@ -397,9 +390,9 @@ rfi_batched_mask_kernel(const __grid_constant__ CUtensorMap tmap, const KParams 
             }
         }
         if (G > 1) {
-            if (G == 8)      flush_group_flags<8>(p, tcol, n_rounds, warp, lane, n_valid, flag_lo, flag_set_stride, fwpw, o_global, tile0);
-            else if (G == 4) flush_group_flags<4>(p, tcol, n_rounds, warp, lane, n_valid, flag_lo, flag_set_stride, fwpw, o_global, tile0);
-            else             flush_group_flags<2>(p, tcol, n_rounds, warp, lane, n_valid, flag_lo, flag_set_stride, fwpw, o_global, tile0);
+            if (G == 8)      flush_group_flags<8>(p, tcol, n_rounds, warp, lane, flag_lo, flag_set_stride, fwpw, o_global, tile0);
+            else if (G == 4) flush_group_flags<4>(p, tcol, n_rounds, warp, lane, flag_lo, flag_set_stride, fwpw, o_global, tile0);
+            else             flush_group_flags<2>(p, tcol, n_rounds, warp, lane, flag_lo, flag_set_stride, fwpw, o_global, tile0);
         }
         o_local += step_o;
         grp += step_g;

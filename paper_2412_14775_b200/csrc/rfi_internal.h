@@ -86,5 +86,8 @@ int launch_batched_mask_f16(const rfi::KParams& kp, const rfi::BatchThr& bt, con
 inline bool batched_mask_supported(const rfi::KParams& kp) {
     return kp.n_chan % 32 == 0 && env_int("RFI_BT_MASK", 1) != 0;
 }
+inline bool batched_mask_rows(bool fp16, int R) {          // block lengths it is instantiated for
+    return fp16 ? (R == 8 || R == 5 || R == 4 || R == 2) : (R == 5 || R == 4 || R == 2);
+}
 
 }  // namespace rfi_host

@@ -376,6 +376,36 @@ def test_batched_ragged_shapes(M, n_int, n_time, n_chan):
     check(w, thr, "auto", seed=M)
 
 
+@pytest.mark.parametrize("n_st,autos,n_chan,fp16,K,group,M,n_int,n_time,F,layout", [
+    (8, True, 64, False, 64, 8, 16, 256, 512, 1, "time_major"),      # 36 baselines x 2 words = 72 words = 9 full groups
+    (7, True, 64, False, 40, 8, 16, 768, 768, 1, "time_major"),      # 56 words: 7 groups; 48 windows = 3 rounds
+    (6, False, 96, False, 33, 8, 16, 128, 256, 1, "time_major"),     # 15 baselines x 3 words = 45 words: row % 8 != 0 -> G falls to 1
+    (9, False, 32, False, 64, 4, 16, 256, 512, 1, "time_major"),     # 36 words: G = 4, 9 groups
+    (6, True, 64, False, 17, 8, 10, 200, 400, 2, "time_major"),      # 10 x 2 footprints (R = 5), 42 words: row % 8 != 0, G = 2
+    (5, True, 128, True, 64, 8, 16, 256, 512, 1, "time_major"),      # fp16 storage, 60 words -> G = 4
+    (8, True, 64, False, 64, 8, 16, 256, 512, 1, "cell_major"),
+    (8, True, 64, True, 20, 8, 16, 256, 512, 1, "cell_major"),
+])
+def test_batched_tile_groups_in_tensor_memory(monkeypatch, n_st, autos, n_chan, fp16, K, group, M, n_int, n_time, F, layout):
+    """The K-set kernel parks the flag words of G adjacent tiles in tensor memory and stores them as whole sectors
+    (rfi_batched_mask.cuh).  Small chunks would not be grouped (every SM is to get two groups), so the rule is lifted
+    here; outputs must match the oracle and, bit for bit, the ungrouped run (G = 1) of the same kernel."""
+    w = synth.Workload("groups", n_st, autos, n_chan, n_time, M, n_int, window_F=F, fp16=fp16, burst_cell_frac=0.15,
+                       channel_gain=True)
+    thr = synth.sweep_thresholds(M * F, K, seed=K + group)
+    monkeypatch.setenv("RFI_BT_GROUP_ANY", "1")
+    monkeypatch.setenv("RFI_BT_GROUP", str(group))
+    rep, grouped, _ = check(w, thr, "auto", seed=group, layout=layout)
+    assert rep["K"] == K
+    monkeypatch.setenv("RFI_BT_GROUP", "1")
+    vis, _ = synth.make_chunk(w, seed=group)
+    plain, used = run_gpu(w, vis, thr, "auto", layout=layout)
+    assert used == "batched"
+    for key in ("avg", "weight", "flags", "tau", "r_re", "r_im"):
+        np.testing.assert_array_equal(grouped[key], plain[key], err_msg=key)
+    assert 0 < grouped["flags"].mean() < 1
+
+
 def test_batched_fp16_and_host_path():
     w = synth.WORKLOADS["lofar_fp16"].scaled(n_stations=5, n_time=1024, n_int=256, burst_cell_frac=0.1, tone_chan_frac=0.02)
     thr = synth.sweep_thresholds(16, 8, seed=3)
