@@ -277,12 +277,19 @@ def measure_config(name, K, dev, steps, warmup, peak, read_probe_gbs, vis=None, 
     st = _pctl_stats(ms)
     samples = w.n_time * w.n_cells
     gbs_best, gbs_med = algo / (st["kernel_ms_best"] * 1e-3) / 1e9, algo / (st["kernel_ms_median"] * 1e-3) / 1e9
+    mix_probe = None
+    if K > 1 and not small:      # K-set pass: the ceiling is a read/write MIX, measured live with the same output volume
+        try:
+            mix_probe = rfi.probe_mix_bandwidth(vis if w.input_bytes <= (40 << 30) else vis.reshape(-1)[: (40 << 30) // vis.element_size()], out_bytes)
+        except Exception:
+            mix_probe = None
     rec.update(variant=plan.last_variant, gpu_launches=int(plan.launch_count - l0), **st,
                ms_per_step=st["kernel_ms_mean"], samples_per_s=samples / (st["kernel_ms_median"] * 1e-3),
                algorithmic_bytes_per_launch=algo,
                roofline={"bound": "hbm" if not small else "latency", "achieved": gbs_med, "achieved_best": gbs_best, "unit": "GB/s",
                          "peak": peak, "frac": gbs_med / peak, "frac_of_nominal_8TBs": gbs_med / 8000.0,
-                         "frac_of_read_stream_probe": (gbs_med / read_probe_gbs) if read_probe_gbs else None},
+                         "frac_of_read_stream_probe": (gbs_med / read_probe_gbs) if read_probe_gbs else None,
+                         "mix_probe_gbs": mix_probe, "frac_of_mix_probe": (gbs_med / mix_probe) if mix_probe else None},
                l2=("L2 flushed between timed launches (256 MB write outside the events)" if small else "input far larger than the 126 MB L2"))
     if small:
         rec["latency_us"] = {"best": st["kernel_ms_best"] * 1e3, "median": st["kernel_ms_median"] * 1e3}
@@ -549,6 +556,13 @@ def run_ours(args):
         read_probe = rfi.probe_read_bandwidth(vis if in_bytes <= (40 << 30) else vis.reshape(-1)[: (40 << 30) // vis.element_size()])
     except Exception:
         read_probe = None
+    mix_probe = None
+    if plan.K > 1 and algo_bytes > in_bytes:     # zero-arithmetic stream with the same read/write volumes (rfi_probe_mix_bandwidth)
+        try:
+            mix_probe = rfi.probe_mix_bandwidth(vis if in_bytes <= (40 << 30) else vis.reshape(-1)[: (40 << 30) // vis.element_size()],
+                                                algo_bytes - in_bytes)
+        except Exception:
+            mix_probe = None
     traffic = load_ncu_traffic(w.name, variant)
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": traffic,
@@ -562,6 +576,7 @@ def run_ours(args):
                 "frac_of_nominal_8TBs": achieved / 8000.0,
                 "read_stream_probe_gbs": read_probe,
                 "frac_of_read_stream_probe": (achieved / read_probe) if read_probe else None,
+                "mix_probe_gbs": mix_probe, "frac_of_mix_probe": (achieved / mix_probe) if mix_probe else None,
                 "note": "frac = achieved / MEASURED_PEAKS hbm_gbs, a read+write copy_ figure; this kernel is a read-only "
                         "stream, so frac_of_read_stream_probe (same-device read-only probe) and frac_of_nominal_8TBs are the "
                         "fractions that cannot exceed 1"}

@@ -318,6 +318,17 @@ size_t rfi_sim42_truth_bytes(const rfi_sim42_config *cfg);    /* (n_time/window_
  * the like-for-like denominator for its achieved GB/s; MEASURED_PEAKS.json's figure is a read+write copy. */
 int rfi_probe_read_bandwidth(const void *d_buf, size_t bytes, int repeats, float *h_ms_best, void *cuda_stream);
 
+/* Diagnostics (not part of the method): the same for the traffic MIX of a K-set pass (batched-threshold mode, K sets of
+ * averaged outputs per chunk: 32 B in and K * (36/n_int + 1/(8 W)) B out per sample): every warp reads
+ * `reads_per_write` 1 KiB rows of d_in with the streaming load and then writes one 1 KiB row of d_out with an
+ * evict-first 256-bit store, no arithmetic.  d_in, d_out: 32-byte aligned device buffers; floor(in_bytes /
+ * (reads_per_write KiB)) KiB of d_out are written (RFI_EINVAL if out_bytes is smaller, or nothing would be read);
+ * *h_ms_best (host): best of `repeats` timed launches over four launch shapes, *h_bytes_moved (host, may be NULL):
+ * bytes read + written per launch.  Synchronises the stream.  What this reaches is the ceiling for the batched
+ * kernels: HBM serves a 90/10 read/write mix more slowly than a pure read stream. */
+int rfi_probe_mix_bandwidth(const void *d_in, size_t in_bytes, void *d_out, size_t out_bytes, int reads_per_write,
+                            int repeats, float *h_ms_best, size_t *h_bytes_moved, void *cuda_stream);
+
 /* helpers */
 const char *rfi_strerror(int code);
 const char *rfi_last_cuda_error(void);                 /* detail text of the last failed process call of this thread: the

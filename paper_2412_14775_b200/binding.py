@@ -25,7 +25,7 @@ EXPORTS = [
     "rfi_plan_set_variant", "rfi_process_chunk", "rfi_get_flags", "rfi_confusion_counts", "rfi_process_chunk_host", "rfi_plan_destroy",
     "rfi_strerror", "rfi_last_cuda_error", "rfi_flags_bytes", "rfi_avg_bytes", "rfi_weight_bytes",
     "rfi_stats_bytes", "rfi_vis_bytes", "rfi_plan_launch_count", "rfi_plan_last_variant", "rfi_version",
-    "rfi_probe_read_bandwidth", "rfi_sim42_generate", "rfi_sim42_vis_bytes", "rfi_sim42_truth_bytes",
+    "rfi_probe_read_bandwidth", "rfi_probe_mix_bandwidth", "rfi_sim42_generate", "rfi_sim42_vis_bytes", "rfi_sim42_truth_bytes",
     "rfi_rl_evaluate", "rfi_plan_set_adaptive", "rfi_plan_get_thresholds",
     "rfi_plan_get_adaptive_histogram",
 ]
@@ -111,6 +111,8 @@ def load_library(build_if_missing: bool = True):
     lib.rfi_plan_destroy.argtypes = [vp]
     lib.rfi_probe_read_bandwidth.argtypes = [vp, sz, ci, ctypes.POINTER(ctypes.c_float), vp]
     lib.rfi_probe_read_bandwidth.restype = ci
+    lib.rfi_probe_mix_bandwidth.argtypes = [vp, sz, vp, sz, ci, ci, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(sz), vp]
+    lib.rfi_probe_mix_bandwidth.restype = ci
     lib.rfi_rl_evaluate.argtypes = [vp, ctypes.c_int64, ci, ctypes.c_uint32, ctypes.POINTER(RfiThresholds), ctypes.c_double, vp, vp]
     lib.rfi_rl_evaluate.restype = ci
     lib.rfi_sim42_generate.argtypes = [ctypes.POINTER(Sim42Config), vp, vp, vp, vp, vp]
@@ -397,6 +399,24 @@ def probe_read_bandwidth(buf: torch.Tensor, repeats: int = 10) -> float:
         _check(lib.rfi_probe_read_bandwidth(buf.data_ptr(), nbytes, repeats, ctypes.byref(ms),
                                             torch.cuda.current_stream(buf.device).cuda_stream), "rfi_probe_read_bandwidth")
     return (nbytes // 32 * 32) / (ms.value * 1e-3) / 1e9
+
+
+def probe_mix_bandwidth(buf: torch.Tensor, out_bytes: int, repeats: int = 10) -> float:
+    """rfi_probe_mix_bandwidth: GB/s (read + written) of a zero-arithmetic stream that reads buf and writes about
+    out_bytes, 1 KiB row per `reads_per_write` rows read -- the ceiling for a K-set pass with that output volume.
+    buf: contiguous CUDA tensor, 32-byte aligned."""
+    if not (buf.is_cuda and buf.is_contiguous()):
+        raise ValueError("buf must be a contiguous CUDA tensor")
+    lib = load_library()
+    nbytes = buf.numel() * buf.element_size()
+    rpw = max(1, round(nbytes / max(out_bytes, 1)))
+    out = torch.empty(nbytes // (rpw * 1024) * 1024 + 1024, dtype=torch.uint8, device=buf.device)
+    ms, moved = ctypes.c_float(), ctypes.c_size_t()
+    with torch.cuda.device(buf.device):
+        _check(lib.rfi_probe_mix_bandwidth(buf.data_ptr(), nbytes, out.data_ptr(), out.numel(), rpw, repeats, ctypes.byref(ms),
+                                           ctypes.byref(moved), torch.cuda.current_stream(buf.device).cuda_stream),
+               "rfi_probe_mix_bandwidth")
+    return moved.value / (ms.value * 1e-3) / 1e9
 
 
 def unpack_flags(flags: torch.Tensor, n_chan: int) -> torch.Tensor:

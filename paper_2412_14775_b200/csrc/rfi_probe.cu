@@ -1,4 +1,5 @@
-// rfi_probe.cu -- diagnostics: a read-only streaming bandwidth probe (rfi_probe_read_bandwidth, include/rfi.h).
+// rfi_probe.cu -- diagnostics: a read-only streaming bandwidth probe (rfi_probe_read_bandwidth) and a read/write mix
+// probe (rfi_probe_mix_bandwidth), include/rfi.h.
 // The flag-and-average kernels are one-touch READ streams (32 B in, 0.055 B out per sample), while the measured HBM
 // peak of MEASURED_PEAKS.json is a read+write copy; this probe measures what a pure read stream reaches on the same
 // device with the same load instruction the direct kernel uses, so bench.py can quote a like-for-like denominator
@@ -29,7 +30,85 @@ __global__ void __launch_bounds__(256) rfi_probe_read_kernel(const uint8_t* __re
     if (acc == 0x9e3779b97f4a7c15ull) *sink = acc;            // keeps the loads alive; practically never taken
 }
 
+// Read/write mix probe: every warp reads `rpw` 1 KiB rows (256-bit streaming loads, U in flight per lane) and then writes
+// one 1 KiB row (256-bit evict-first stores), i.e. the traffic of a K-set pass -- 32 B in and K x 0.055 B out per sample
+// -- with no arithmetic.  What it reaches is the like-for-like ceiling for the batched kernels (rfi_probe_mix_bandwidth).
+template <int U>
+__global__ void __launch_bounds__(128) rfi_probe_mix_kernel(const uint8_t* __restrict__ in, uint8_t* __restrict__ out,
+                                                            size_t n_groups, int rpw) {
+    const int lane = threadIdx.x & 31;
+    const size_t n_warps = (size_t)gridDim.x * (blockDim.x >> 5);
+    for (size_t g = (size_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); g < n_groups; g += n_warps) {
+        const uint8_t* src = in + (g * rpw) * 1024 + (size_t)lane * 32;
+        f2 acc[4] = {0ull, 0ull, 0ull, 0ull};
+        int r = 0;
+        for (; r + U <= rpw; r += U) {
+            Raw<false> v[U];
+#pragma unroll
+            for (int u = 0; u < U; ++u) ldg_stream(src + (size_t)(r + u) * 1024, v[u]);
+#pragma unroll
+            for (int u = 0; u < U; ++u)
+#pragma unroll
+                for (int q = 0; q < 4; ++q) acc[q] ^= v[u].p[q];
+        }
+        for (; r < rpw; ++r) {
+            Raw<false> v;
+            ldg_stream(src + (size_t)r * 1024, v);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) acc[q] ^= v.p[q];
+        }
+        asm volatile("st.global.L1::no_allocate.L2::evict_first.v4.b64 [%0], {%1,%2,%3,%4};" ::"l"(out + g * 1024 + (size_t)lane * 32),
+                     "l"(acc[0]), "l"(acc[1]), "l"(acc[2]), "l"(acc[3]) : "memory");
+    }
+}
+
 }  // namespace rfi
+
+extern "C" int rfi_probe_mix_bandwidth(const void* d_in, size_t in_bytes, void* d_out, size_t out_bytes, int reads_per_write,
+                                       int repeats, float* h_ms_best, size_t* h_bytes_moved, void* cuda_stream) {
+    using namespace rfi_host;
+    g_cuda_err[0] = 0;
+    if (!d_in || !d_out || !h_ms_best || reads_per_write < 1 || repeats < 1 || reinterpret_cast<uintptr_t>(d_in) % 32 ||
+        reinterpret_cast<uintptr_t>(d_out) % 32) return RFI_EINVAL;
+    const size_t n_groups = in_bytes / ((size_t)reads_per_write * 1024);
+    if (n_groups < 1 || n_groups * 1024 > out_bytes) return RFI_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    int dev = 0, sms = 0;
+    RFI_CUDA(cudaGetDevice(&dev));
+    RFI_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    cudaEvent_t a = nullptr, b = nullptr;
+    float best = 0.f;
+    auto run = [&]() -> int {
+        RFI_CUDA(cudaEventCreate(&a));
+        RFI_CUDA(cudaEventCreate(&b));
+        const int shapes[4][2] = {{4, 4}, {4, 8}, {8, 4}, {8, 8}};   // {U, CTAs of 4 warps per SM}
+        for (int sh = 0; sh < 4; ++sh) {
+            for (int it = 0; it < repeats + 2; ++it) {        // two untimed warm-up launches per shape
+                RFI_CUDA(cudaEventRecord(a, st));
+                const unsigned grid = (unsigned)(sms * shapes[sh][1]);
+                const uint8_t* src = static_cast<const uint8_t*>(d_in);
+                uint8_t* dst = static_cast<uint8_t*>(d_out);
+                if (shapes[sh][0] == 4) rfi::rfi_probe_mix_kernel<4><<<grid, 128, 0, st>>>(src, dst, n_groups, reads_per_write);
+                else                    rfi::rfi_probe_mix_kernel<8><<<grid, 128, 0, st>>>(src, dst, n_groups, reads_per_write);
+                RFI_CUDA(cudaGetLastError());
+                RFI_CUDA(cudaEventRecord(b, st));
+                RFI_CUDA(cudaEventSynchronize(b));
+                float ms = 0.f;
+                RFI_CUDA(cudaEventElapsedTime(&ms, a, b));
+                if (it >= 2 && (best == 0.f || ms < best)) best = ms;
+            }
+        }
+        return RFI_OK;
+    };
+    const int rc = run();
+    if (a) cudaEventDestroy(a);
+    if (b) cudaEventDestroy(b);
+    if (rc == RFI_OK) {
+        *h_ms_best = best;
+        if (h_bytes_moved) *h_bytes_moved = n_groups * ((size_t)reads_per_write + 1) * 1024;
+    }
+    return rc;
+}
 
 extern "C" int rfi_probe_read_bandwidth(const void* d_buf, size_t bytes, int repeats, float* h_ms_best, void* cuda_stream) {
     using namespace rfi_host;

@@ -724,3 +724,26 @@ def test_bench_strong_scaling_shards_reproduce_the_full_chunk():
     weak = sharding.rank_work(w.n_baselines, world, 2, "weak")
     assert not weak["sharded"] and weak["seed"] == 1236
     plan_full.destroy()
+
+
+def test_mix_probe_moves_the_bytes_it_reports():
+    """rfi_probe_mix_bandwidth (diagnostics): reads every 1 KiB row once, writes one row per `reads_per_write` rows --
+    the XOR of the rows read -- and rejects an output buffer that is too small."""
+    import ctypes
+    lib = rfi.load_library()
+    g = torch.Generator().manual_seed(5)
+    rows, rpw = 4096 * 9, 9
+    buf = torch.randint(-2**31, 2**31 - 1, (rows, 256), dtype=torch.int32, generator=g).cuda()
+    out = torch.zeros(rows // rpw, 256, dtype=torch.int32, device="cuda")
+    ms, moved = ctypes.c_float(), ctypes.c_size_t()
+    rc = lib.rfi_probe_mix_bandwidth(buf.data_ptr(), buf.numel() * 4, out.data_ptr(), out.numel() * 4, rpw, 2,
+                                     ctypes.byref(ms), ctypes.byref(moved), None)
+    assert rc == 0 and ms.value > 0 and moved.value == (rows + rows // rpw) * 1024
+    want = buf.view(rows // rpw, rpw, 256)[:, 0].clone()
+    for r in range(1, rpw):
+        want ^= buf.view(rows // rpw, rpw, 256)[:, r]
+    assert torch.equal(out, want)
+    rc = lib.rfi_probe_mix_bandwidth(buf.data_ptr(), buf.numel() * 4, out.data_ptr(), out.numel() * 4 - 1024, rpw, 2,
+                                     ctypes.byref(ms), ctypes.byref(moved), None)
+    assert rc != 0
+    assert rfi.probe_mix_bandwidth(buf, out.numel() * 4, repeats=2) > 0

@@ -66,8 +66,9 @@ def _workload(fp16):
 
 
 def stress(fp16, K, iters, layouts=("time_major", "cell_major"), seed=1234):
-    """`iters` repetitions: batched (TMA) vs itself, vs the register-staged batched kernel and vs single-set direct
-    and TMA runs of sets 0 and K-1; bit for bit.  Returns the number of kernel launches compared."""
+    """`iters` repetitions: the K-set kernel (rfi_batched_mask.cuh) vs itself, vs the first-generation TMA-staged kernel,
+    vs the register-staged batched kernel, with and without tile groups in tensor memory, and vs single-set direct and
+    TMA runs of sets 0 and K-1; bit for bit.  Returns the number of kernel launches compared."""
     w = _workload(fp16)
     thr = synth.sweep_thresholds(w.window_M, K, seed=K)
     vis, _ = synth.make_chunk(w, seed=seed)
@@ -101,6 +102,22 @@ def stress(fp16, K, iters, layouts=("time_major", "cell_major"), seed=1234):
             finally:
                 os.environ.pop("RFI_BATCHED_TMA", None)
             _same(f"iter {it}: register-staged batched vs batched_tma (K={K}, fp16={fp16})", got, ref)
+            n += 1
+        if it % 4 == 1:
+            os.environ["RFI_BT_MASK"] = "0"               # the first-generation TMA-staged kernel (rfi_batched_tma.cuh)
+            try:
+                got = _run(w, d_vis, thr)
+            finally:
+                os.environ.pop("RFI_BT_MASK", None)
+            _same(f"iter {it}: first-generation batched_tma vs rank-query kernel (K={K}, fp16={fp16})", got, ref)
+            n += 1
+        if it % 4 == 2:
+            os.environ["RFI_BT_GROUP_ANY"] = "1"          # flag words of G tiles parked in tensor memory (G = 2 here)
+            try:
+                got = _run(w, d_vis, thr)
+            finally:
+                os.environ.pop("RFI_BT_GROUP_ANY", None)
+            _same(f"iter {it}: tile groups in tensor memory vs ungrouped (K={K}, fp16={fp16})", got, ref)
             n += 1
         for k, s in singles.items():
             again = _run(w, d_vis, [thr[k]], "direct")
