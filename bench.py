@@ -256,6 +256,12 @@ def measure_config(name, K, dev, steps, warmup, peak, read_probe_gbs, vis=None, 
         plan.set_window_freq(w.window_F)
     plan.set_thresholds(thr)
     plan.set_variant(variant)
+    counts = tw = None
+    if K > 1 and truth is not None:
+        # configs[4]: "per-set flag fraction against injected-RFI ground truth" is an output of the pass -- the K-set kernel
+        # fills the K x 4 confusion counters in the timed launch itself (rfi_plan_set_truth)
+        tw = rfi.pack_flags(truth.reshape(plan.n_win, plan.n_baselines, w.n_chan))
+        counts = plan.set_truth(tw)
     avg, weight, stats = plan.alloc_outputs(device=dev, stats=True)
     out_bytes = avg.numel() * 4 + weight.numel() * 4 + max(plan.K, 1) * plan.n_win * plan.n_baselines * plan.wpb * 4
     algo = w.input_bytes + out_bytes
@@ -293,6 +299,16 @@ def measure_config(name, K, dev, steps, warmup, peak, read_probe_gbs, vis=None, 
                l2=("L2 flushed between timed launches (256 MB write outside the events)" if small else "input far larger than the 126 MB L2"))
     if small:
         rec["latency_us"] = {"best": st["kernel_ms_best"] * 1e3, "median": st["kernel_ms_median"] * 1e3}
+    if counts is not None:
+        torch.cuda.synchronize(dev)
+        c = counts.cpu().double()
+        fa, md = (c[:, 0] / c[:, 1].clamp(min=1)), (c[:, 2] / c[:, 3].clamp(min=1))
+        sep = plan.confusion_counts(tw).cpu()
+        rec["detection"] = {"source": "K x 4 confusion counters filled by the timed K-set launch (rfi_plan_set_truth)",
+                            "equal_to_separate_mask_pass": bool(torch.equal(sep, counts.cpu())),
+                            "false_alarm_min_max": [float(fa.min()), float(fa.max())],
+                            "missed_detection_min_max": [float(md.min()), float(md.max())]}
+        plan.set_truth(None)
     # one more launch with the statistics planes, then the sampled-cell oracle check (not timed)
     plan.process_chunk(vis, avg, weight, stats)
     torch.cuda.synchronize(dev)

@@ -215,6 +215,16 @@ int rfi_get_flags(rfi_plan *plan, const uint32_t **d_flags, size_t *n_words);
  * RFI_ESTATE before the first process call; RFI_EINVAL for NULL / misaligned pointers. */
 int rfi_confusion_counts(rfi_plan *plan, const uint32_t *d_truth, uint64_t *d_counts, void *cuda_stream);
 
+/* The same counters as part of every rfi_process_chunk call (device path): with a ground-truth mask d_truth (layout as
+ * above) and d_counts (uint64_t [K][4], both device pointers that must stay valid; both NULL switches it off), each
+ * call zeroes d_counts on its stream and fills it for the chunk it processes.  The K-set kernel counts in the same
+ * launch -- the thread that packs a (set, window) flag word compares it with the truth word, so a tuning loop
+ * (false-alarm / missed-detection probabilities per candidate threshold set) needs no second pass over
+ * the K masks; the other kernels are followed by the mask pass of rfi_confusion_counts on the same stream.  Same
+ * exact integers either way.  rfi_process_chunk_host does not count.  RFI_EINVAL if exactly one pointer is NULL or a
+ * pointer is misaligned (4 / 8 bytes). */
+int rfi_plan_set_truth(rfi_plan *plan, const uint32_t *d_truth, uint64_t *d_counts);
+
 /* End-to-end host path: vis in HOST memory (pinned for full speed), results to HOST memory.  Streams the
  * chunk to the device one output integration at a time on two internal streams so that host->device copies
  * overlap the kernel, then copies avg / weight / flags (and stats if non-NULL) back and synchronises.

@@ -22,7 +22,7 @@ MASK_PAPER_LEARNED = 0x3C50      # Tables 3-4: Table 1 groups
 
 EXPORTS = [
     "rfi_plan_create", "rfi_plan_set_integration", "rfi_plan_set_baseline_shard", "rfi_plan_set_window_freq", "rfi_plan_set_arithmetic", "rfi_plan_set_baseline_classes", "rfi_plan_set_layout", "rfi_set_thresholds",
-    "rfi_plan_set_variant", "rfi_process_chunk", "rfi_get_flags", "rfi_confusion_counts", "rfi_process_chunk_host", "rfi_plan_destroy",
+    "rfi_plan_set_variant", "rfi_process_chunk", "rfi_get_flags", "rfi_confusion_counts", "rfi_plan_set_truth", "rfi_process_chunk_host", "rfi_plan_destroy",
     "rfi_strerror", "rfi_last_cuda_error", "rfi_flags_bytes", "rfi_avg_bytes", "rfi_weight_bytes",
     "rfi_stats_bytes", "rfi_vis_bytes", "rfi_plan_launch_count", "rfi_plan_last_variant", "rfi_version",
     "rfi_probe_read_bandwidth", "rfi_probe_mix_bandwidth", "rfi_sim42_generate", "rfi_sim42_vis_bytes", "rfi_sim42_truth_bytes",
@@ -108,6 +108,8 @@ def load_library(build_if_missing: bool = True):
     lib.rfi_process_chunk_host.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.rfi_confusion_counts.argtypes = [vp, vp, vp, vp]
     lib.rfi_confusion_counts.restype = ci
+    lib.rfi_plan_set_truth.argtypes = [vp, vp, vp]
+    lib.rfi_plan_set_truth.restype = ci
     lib.rfi_plan_destroy.argtypes = [vp]
     lib.rfi_probe_read_bandwidth.argtypes = [vp, sz, ci, ctypes.POINTER(ctypes.c_float), vp]
     lib.rfi_probe_read_bandwidth.restype = ci
@@ -294,6 +296,23 @@ class RfiPlan:
         s = stream if stream is not None else torch.cuda.current_stream(truth_words.device)
         _check(self._lib.rfi_confusion_counts(self._h, truth_words.data_ptr(), counts.data_ptr(), s.cuda_stream),
                "rfi_confusion_counts")
+        return counts
+
+    def set_truth(self, truth_words: Optional[torch.Tensor]) -> Optional[torch.Tensor]:
+        """rfi_plan_set_truth: every following process_chunk also fills int64 counts[K, 4] = {false alarms, clean windows,
+        missed detections, RFI windows} against truth_words (= pack_flags(bool truth) on the device); the K-set kernel
+        counts in the same launch.  Returns the counts tensor (refilled by every call); None switches it off."""
+        if truth_words is None:
+            _check(self._lib.rfi_plan_set_truth(self._h, None, None), "rfi_plan_set_truth")
+            self._truth = self._counts = None
+            return None
+        if not (truth_words.is_cuda and truth_words.is_contiguous() and truth_words.dtype == torch.int32):
+            raise ValueError("truth_words must be a contiguous int32 CUDA tensor (pack_flags)")
+        if truth_words.numel() != self.n_win * self.n_baselines * self.wpb:
+            raise ValueError("truth_words has the wrong size for this plan")
+        counts = torch.zeros(max(self.K, 1), 4, dtype=torch.int64, device=truth_words.device)
+        _check(self._lib.rfi_plan_set_truth(self._h, truth_words.data_ptr(), counts.data_ptr()), "rfi_plan_set_truth")
+        self._truth, self._counts = truth_words, counts                      # keep both alive
         return counts
 
     def process_chunk_host(self, vis: torch.Tensor, want_stats: bool = False):

@@ -53,6 +53,10 @@ struct rfi_plan {
     std::vector<uint8_t> h_cls;               // class of every baseline of the whole array (n_classes == 2)
     uint8_t* d_cls = nullptr;
     bool cls_uploaded = false;
+    const uint32_t* d_truth = nullptr;        // rfi_plan_set_truth: ground-truth mask and [K][4] counters of every device-path call
+    uint64_t* d_counts = nullptr;
+    bool truth_fused = false;                 // the last enqueue counted in its own kernel
+    bool count_now = false;                   // inside rfi_process_chunk with a truth mask set
     int n_baselines_total = 0, b_first = 0;   // n_baselines is the shard this plan processes (default: all)
     int K = 0;
     std::vector<rfi_thresholds> thr;
@@ -245,6 +249,7 @@ int enqueue_slab(rfi_plan* p, const void* d_vis_slab, int o_first, int n_out_sla
     kp.k_first = 0;
     kp.flags_atomic = (p->n_chan % 32 != 0 && 32 % p->n_chan != 0) ? 1 : 0;
     if (p->adapt_alpha > 0.0) { kp.d_thr = p->d_thr; kp.hist = p->d_hist; }
+    p->truth_fused = false;
 
     const bool fp16 = p->precision == RFI_FP16;
     if (p->arith == RFI_ARITH_TABLES) {
@@ -293,6 +298,11 @@ int enqueue_slab(rfi_plan* p, const void* d_vis_slab, int o_first, int n_out_sla
                 bt.t[k] = to_device_thr(p->thr[(size_t)(k0 + k) * nc], p->M * p->F);
                 bt.t1[k] = to_device_thr(p->thr[(size_t)(k0 + k) * nc + nc - 1], p->M * p->F);
             }
+            if (batched_mask_supported(kp) && p->count_now) {
+                kp.truth = p->d_truth;
+                kp.counts = reinterpret_cast<unsigned long long*>(p->d_counts);
+                p->truth_fused = true;
+            }
             if (batched_mask_supported(kp))
                 rc = fp16 ? launch_batched_mask_f16(kp, bt, map, R, true, p->sm_count, p->smem_optin, st)
                           : launch_batched_mask_f32(kp, bt, map, R, true, p->sm_count, p->smem_optin, st);
@@ -331,6 +341,11 @@ int enqueue_slab(rfi_plan* p, const void* d_vis_slab, int o_first, int n_out_sla
                 bt.t1[k] = to_device_thr(p->thr[(size_t)(k0 + k) * nc + nc - 1], p->M * p->F);
             }
             int rc;
+            if (use_mask && p->count_now) {   // counters in the same kernel (device path)
+                kp.truth = p->d_truth;
+                kp.counts = reinterpret_cast<unsigned long long*>(p->d_counts);
+                p->truth_fused = true;
+            }
             if (use_mask)
                 rc = fp16 ? launch_batched_mask_f16(kp, bt, map, R, false, p->sm_count, p->smem_optin, st)
                           : launch_batched_mask_f32(kp, bt, map, R, false, p->sm_count, p->smem_optin, st);
@@ -527,6 +542,14 @@ int rfi_set_thresholds(rfi_plan* p, int K, const rfi_thresholds* h_sets) {
     return RFI_OK;
 }
 
+int rfi_plan_set_truth(rfi_plan* p, const uint32_t* d_truth, uint64_t* d_counts) {
+    if (!p || (d_truth == nullptr) != (d_counts == nullptr)) return RFI_EINVAL;
+    if (reinterpret_cast<uintptr_t>(d_truth) % 4 || reinterpret_cast<uintptr_t>(d_counts) % 8) return RFI_EINVAL;
+    p->d_truth = d_truth;
+    p->d_counts = d_counts;
+    return RFI_OK;
+}
+
 int rfi_plan_set_adaptive(rfi_plan* p, float false_alarm, float forget) {
     if (!p || !(false_alarm >= 0.f) || !(false_alarm < 0.5f) || !(forget >= 0.f) || !(forget < 1.f)) return RFI_EINVAL;
     p->adapt_alpha = false_alarm;
@@ -575,8 +598,16 @@ int rfi_process_chunk(rfi_plan* p, const void* d_vis, void* d_avg, void* d_weigh
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     int rc = prepare(p, st);
     if (rc != RFI_OK) return rc;
+    if (p->d_truth) RFI_CUDA(cudaMemsetAsync(p->d_counts, 0, (size_t)p->K * 4 * sizeof(uint64_t), st));
+    p->count_now = p->d_truth != nullptr;
     rc = enqueue_slab(p, d_vis, 0, p->n_out(), static_cast<float*>(d_avg), static_cast<uint32_t*>(d_weight),
                       static_cast<float*>(d_stats), st);
+    p->count_now = false;
+    if (rc == RFI_OK && p->d_truth && !p->truth_fused) {     // kernels without in-kernel counters: a pass over the masks
+        rc = launch_confusion(p->d_flags, p->d_truth, p->d_counts, p->K, (size_t)p->n_win() * p->n_baselines * p->wpb(),
+                              p->wpb(), p->n_chan, p->sm_count, st);
+        if (rc == RFI_OK) p->launches++;
+    }
     if (rc == RFI_OK) rc = finish_adaptive(p, st);
     if (rc == RFI_OK) p->have_result = true;
     return rc;

@@ -29,6 +29,7 @@ namespace rfi {
 
 constexpr int kBmRecBytes = 1280;                 // per (round buffer, window): mask[2][32] u32, s01[32] 16 B, s23[32] 16 B
 constexpr int kBmTblBytes = 3 * 64 * 4 + 3 * 65 * 8;   // per class: sorted x_low, x_high, gamma; prefix masks by rank
+constexpr int kBmCntBytes = kBtWarps * 6 * 32 * 4;     // per warp: {fa, md} x {sets k, 32+k}, clean, rfi; one word per lane
 
 __device__ __forceinline__ float lds_f32(uint32_t a) { float v; asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a)); return v; }
 __device__ __forceinline__ uint32_t lds_u32(uint32_t a) { uint32_t v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a)); return v; }
@@ -37,6 +38,7 @@ __device__ __forceinline__ void lds_u32x2(uint32_t a, uint32_t& lo, uint32_t& hi
 }
 __device__ __forceinline__ void sts_u32(uint32_t a, uint32_t v) { asm volatile("st.shared.u32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
 __device__ __forceinline__ void sts_f32(uint32_t a, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v) : "memory"); }
+__device__ __forceinline__ void red_shared_add(uint32_t a, uint32_t v) { asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
 __device__ __forceinline__ void sts_u32x2(uint32_t a, uint32_t lo, uint32_t hi) {
     asm volatile("st.shared.v2.u32 [%0], {%1,%2};" ::"r"(a), "r"(lo), "r"(hi) : "memory");
 }
@@ -176,7 +178,8 @@ rfi_batched_mask_kernel(const __grid_constant__ CUtensorMap tmap, const KParams 
     const uint32_t rec_base = smem_base + (uint32_t)NW * stages * STAGE_BYTES;          // [2][NW] records
     const uint32_t tbl_base = rec_base + 2u * NW * kBmRecBytes;                          // [2 classes] tables
     const uint32_t perm_base = tbl_base + 2u * kBmTblBytes;                              // [6][64] u8 sort permutations
-    const uint32_t tm_slot = perm_base + 384u;                                           // TMEM base address (one word)
+    const uint32_t cnt_base = perm_base + 384u;                                          // [NW][6][32] u32 confusion counters
+    const uint32_t tm_slot = cnt_base + kBmCntBytes;                                           // TMEM base address (one word)
     const uint32_t round_bar = tm_slot + 8u;                                             // records of a round complete (all threads arrive)
     const uint32_t bars = tm_slot + 16u + (uint32_t)warp * stages * 16;                  // per warp: full[], empty[]
     const uint32_t ebars = bars + (uint32_t)stages * 8;
@@ -255,6 +258,8 @@ rfi_batched_mask_kernel(const __grid_constant__ CUtensorMap tmap, const KParams 
             sts_f32(tbl_base + cls * kBmTblBytes + kind * 256 + rank * 4, v);
             asm volatile("st.shared.u8 [%0], %1;" ::"r"(perm_base + a * 64 + rank), "r"(i) : "memory");
         }
+        if (p.truth)
+            for (int i = t; i < kBmCntBytes / 4; i += NW * 32) sts_u32(cnt_base + 4u * i, 0u);
         if (warp == NW - 1 && G > 1) tmem_alloc(tm_slot, (uint32_t)tm_cols);    // flag staging (warp NW-1 is idle above)
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
         __syncthreads();
@@ -367,6 +372,16 @@ rfi_batched_mask_kernel(const __grid_constant__ CUtensorMap tmap, const KParams 
                     {
                         const uint32_t f_lo = ~warp_transpose32(m_lo, lane);
                         const uint32_t f_hi = p.K > 32 ? ~warp_transpose32(m_hi, lane) : 0u;
+                        if (p.truth) {                         // confusion counters of sets k and 32 + k (rfi_plan_set_truth)
+                            const uint32_t tw = __ldg(p.truth + (size_t)w_global * fwpw + tile);
+                            const uint32_t cw = cnt_base + (uint32_t)warp * 768u + (uint32_t)lane * 4u;
+                            red_shared_add(cw, __popc(f_lo & ~tw));
+                            red_shared_add(cw + 128u, __popc(~f_lo & tw));
+                            red_shared_add(cw + 256u, __popc(f_hi & ~tw));
+                            red_shared_add(cw + 384u, __popc(~f_hi & tw));
+                            red_shared_add(cw + 512u, __popc(~tw));
+                            red_shared_add(cw + 640u, __popc(tw));
+                        }
                         if (G > 1) {                           // park them until the group's last tile
                             tmem_st1(tcol + (uint32_t)((round * 2) * G + j), f_lo);
                             if (p.K > 32) tmem_st1(tcol + (uint32_t)((round * 2 + 1) * G + j), f_hi);
@@ -397,6 +412,21 @@ rfi_batched_mask_kernel(const __grid_constant__ CUtensorMap tmap, const KParams 
         o_local += step_o;
         grp += step_g;
         if (grp >= n_groups) { grp -= n_groups; ++o_local; }
+    }
+    if (p.truth) {                                             // this warp's counters: lane k -> sets k and 32 + k
+        const uint32_t cw = cnt_base + (uint32_t)warp * 768u + (uint32_t)lane * 4u;
+        const unsigned long long clean = lds_u32(cw + 512u), rfi_n = lds_u32(cw + 640u);
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const int k = lane + 32 * h;
+            if (k < p.K) {
+                unsigned long long* c = p.counts + (size_t)(p.k_first + k) * 4;
+                atomicAdd(c + 0, (unsigned long long)lds_u32(cw + 256u * h));
+                atomicAdd(c + 1, clean);
+                atomicAdd(c + 2, (unsigned long long)lds_u32(cw + 256u * h + 128u));
+                atomicAdd(c + 3, rfi_n);
+            }
+        }
     }
     if (G > 1) {                                               // every warp is done with its columns
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");

@@ -61,6 +61,10 @@ struct KParams {
     // (updated between chunks by a device kernel) and this chunk's histograms of tau and max(r_re, r_im); null otherwise
     const Thr* d_thr;
     uint32_t* hist;
+    // in-kernel confusion counters (rfi_plan_set_truth; K-set kernel only): ground-truth mask laid out like one set of the
+    // flag mask, and uint64 counts[K][4] = {false alarms, clean windows, missed detections, RFI windows}; null otherwise
+    const uint32_t* truth;
+    unsigned long long* counts;
     // paper-literal tables mode (rfi_tables.cuh) only: raw thresholds of set 0 and the 14-bit precision mask
     float d, s_low, s_high;
     float d1, s_low1, s_high1;   // class 1

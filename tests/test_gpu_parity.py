@@ -478,6 +478,41 @@ def test_confusion_counts_are_exact(n_chan, K):
     assert counts[:, 1].min() > 0 and counts[:, 3].min() > 0
 
 
+@pytest.mark.parametrize("n_chan,K,fp16,layout,group", [(64, 64, False, "time_major", 8), (64, 5, False, "time_major", 1),
+                                                        (32, 40, True, "time_major", 4), (64, 70, False, "time_major", 8),
+                                                        (64, 33, False, "cell_major", 8), (48, 6, False, "time_major", 1),
+                                                        (64, 1, False, "time_major", 1)])
+def test_in_kernel_confusion_counters_equal_the_mask_pass(monkeypatch, n_chan, K, fp16, layout, group):
+    """rfi_plan_set_truth: the counters filled by rfi_process_chunk itself (the K-set kernel counts while it packs the
+    flag words; ragged channel counts and K = 1 are followed by the mask pass) equal rfi_confusion_counts, which
+    test_confusion_counts_are_exact pins against the flags and the oracle.  Refilled, not accumulated, by a second call."""
+    monkeypatch.setenv("RFI_BT_GROUP_ANY", "1")
+    monkeypatch.setenv("RFI_BT_GROUP", str(group))
+    w = synth.Workload("conf2", 8, True, n_chan, 512, 16, 256, fp16=fp16, burst_cell_frac=0.2, channel_gain=True)
+    thr = synth.sweep_thresholds(16, K, seed=K) if K > 1 else synth.default_thresholds(16)
+    vis, truth = synth.make_chunk(w, seed=21)
+    plan = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M, rfi.RFI_FP16 if fp16 else rfi.RFI_FP32,
+                       n_int=w.n_int)
+    plan.set_thresholds(thr)
+    d_vis = vis.cuda()
+    if layout == "cell_major":
+        plan.set_layout("cell_major")
+        d_vis = d_vis.permute(1, 2, 0, 3, 4).contiguous()
+    tw = rfi.pack_flags(truth.reshape(plan.n_win, w.n_baselines, n_chan).cuda())
+    counts = plan.set_truth(tw)
+    avg, weight, _ = plan.alloc_outputs()
+    for _ in range(2):
+        plan.process_chunk(d_vis, avg, weight)
+    torch.cuda.synchronize()
+    fused = counts.cpu().numpy().copy()
+    plan.set_truth(None)
+    plan.process_chunk(d_vis, avg, weight)
+    separate = plan.confusion_counts(tw).cpu().numpy()
+    plan.destroy()
+    np.testing.assert_array_equal(fused, separate)
+    assert fused[:, 1].min() > 0 and fused[:, 3].min() > 0 and (fused[:, 0] + fused[:, 2]).max() > 0
+
+
 # ------------------------------------------------------------------------------------------------------
 # guard bands: compute-sanitizer is not available on the pool, so out-of-bounds stores are caught by canaries
 # ------------------------------------------------------------------------------------------------------
