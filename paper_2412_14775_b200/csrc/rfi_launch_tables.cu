@@ -37,16 +37,22 @@ int launch_r(const rfi::KParams& kp, cudaStream_t st) {
     // Table 1 groups 5 and 7 in half, Table 2 groups 4-7 in half)
     if (kp.arith_mask == 0u) return launch_rm<R, 0>(kp, st);
     if (kp.arith_mask == 0x3C50u) return launch_rm<R, 0x3C50>(kp, st);
-    // any other mask: block length 4 has one instantiation per assignment of the 8 per-sample groups (the per-window
+    // any other mask: block length 2 has one instantiation per assignment of the 8 per-sample groups (the per-window
     // tail reads its 6 bits at run time); other block lengths read the whole mask at run time
-    if (R == 4 && env_int("RFI_TABLES_PS", 1)) return launch_tables_ps(kp, st);
+    if (R == 2 && env_int("RFI_TABLES_PS", 1)) return launch_tables_ps(kp, st);
     return launch_rm<R, -1>(kp, st);
 }
 
 }  // namespace
 
 int launch_tables(const rfi::KParams& kp, cudaStream_t st) {
-    switch (pick_rows(kp.M, false, 4)) {
+    // The arithmetic runs sample by sample whatever the block length (sums are sequential, rfi_tables.cuh), and this mode
+    // is bound by instruction issue (nine IEEE divisions / square roots per sample), not by bytes in flight: short blocks
+    // leave registers for more resident warps (R = 2: 24 warps per SM instead of 16, measured 4.18 -> 3.90 ms).
+    int R = kp.M % 2 == 0 ? 2 : 1;
+    const int force = env_int("RFI_TABLES_ROWS", 0);
+    if (force >= 1 && force <= 4 && kp.M % force == 0) R = force;
+    switch (R) {
         case 1: return launch_r<1>(kp, st);
         case 2: return launch_r<2>(kp, st);
         case 3: return launch_r<3>(kp, st);

@@ -18,7 +18,9 @@
 // value means "read the bits from the kernel parameters".  Instantiated: all-single <0,0>, the paper's learned
 // assignment <0x3C50,0x3C50>, every one of the 256 per-sample assignments with a run-time tail <ps,-1> (so that ANY of
 // the 2^14 masks an RL search visits runs at compile-time-mask speed, rfi_launch_tables_ps*.cu), and the fully
-// run-time <-1,-1> for block lengths other than 4.
+// run-time <-1,-1> for odd window lengths.  Block length R = 2 (1 for odd windows): the arithmetic is sequential in the
+// samples whatever R is, and the mode is bound by instruction issue, so the registers go to resident warps (24 per SM)
+// rather than to bytes in flight.
 // Readings T1-T7 of DESIGN.md section 11 (eps = machine epsilon of the group's format, Eq.(4) brackets, ...).
 #pragma once
 
@@ -120,7 +122,7 @@ __device__ __forceinline__ bool tables_tail(const TabWin& w, const KParams& p, i
 }
 
 template <int R, int SMASK, int TMASK = SMASK>
-__global__ void __launch_bounds__(128, 4) rfi_tables_kernel(const KParams p) {
+__global__ void __launch_bounds__(128, R == 1 ? 8 : (R == 2 ? 6 : 4)) rfi_tables_kernel(const KParams p) {
     const int lane = threadIdx.x & 31;
     const int n_tiles = (p.n_cells + 31) >> 5;
     const int unit = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);

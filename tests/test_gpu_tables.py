@@ -62,7 +62,7 @@ def test_tables_mode_is_bit_exact(mask):
 
 
 def test_tables_any_mask_bit_exact_through_the_per_sample_instantiations(monkeypatch):
-    """An RL search visits arbitrary masks: 24 random ones (block length 4 -> rfi_tables_kernel<4, ps, -1>, the 8
+    """An RL search visits arbitrary masks: 24 random ones (even windows -> rfi_tables_kernel<2, ps, -1>, the 8
     per-sample bits compile-time) bit-exact against the oracle and equal to the fully run-time-mask kernel."""
     w = synth.WORKLOADS["lofar"].scaled(n_stations=4, n_time=320, n_int=160, window_M=16, burst_cell_frac=0.15)
     c = (16 * 0.9 + 1) / 15
@@ -76,6 +76,17 @@ def test_tables_any_mask_bit_exact_through_the_per_sample_instantiations(monkeyp
         monkeypatch.delenv("RFI_TABLES_PS")
         for key in ("tau", "r_re", "r_im", "flags", "weight", "avg"):
             np.testing.assert_array_equal(out[key], rt[key], err_msg=f"{key}, mask {mask:#06x}")
+    # the block length does not enter the arithmetic (sums are sequential in the samples): 1, 2 and 4 rows agree bit for bit
+    for mask in (0, 0x3C50, 0x0A53):
+        ref_out = None
+        for rows in (1, 2, 4):
+            monkeypatch.setenv("RFI_TABLES_ROWS", str(rows))
+            o = run_tables(w, vis, thr, mask)
+            monkeypatch.delenv("RFI_TABLES_ROWS")
+            if ref_out is None:
+                ref_out = o
+            for key in ("tau", "r_re", "r_im", "flags", "weight", "avg"):
+                np.testing.assert_array_equal(o[key], ref_out[key], err_msg=f"{key}, mask {mask:#06x}, rows {rows}")
 
 
 @pytest.mark.parametrize("M,n_int,n_time,n_chan", [(16, 64, 256, 13), (5, 20, 40, 64), (3, 12, 48, 16)])
