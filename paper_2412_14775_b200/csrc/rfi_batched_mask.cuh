@@ -328,6 +328,8 @@ rfi_batched_mask_kernel(const __grid_constant__ CUtensorMap tmap, const KParams 
                 if (wl < p.wpo) {
                     Win w;
                     w.reset();
+                    // the window's ground-truth word, if counters are wanted: asked for now, used after the statistics
+                    const uint32_t tw = p.truth ? __ldg(p.truth + ((size_t)o_global * p.wpo + wl) * fwpw + tile) : 0u;
                     for (int b = 0; b < bpw; ++b) {
                         mbar_wait(bars + 8 * stage, parity);
                         const uint32_t sbase = ring + (uint32_t)stage * STAGE_BYTES;
@@ -373,7 +375,6 @@ rfi_batched_mask_kernel(const __grid_constant__ CUtensorMap tmap, const KParams 
                         const uint32_t f_lo = ~warp_transpose32(m_lo, lane);
                         const uint32_t f_hi = p.K > 32 ? ~warp_transpose32(m_hi, lane) : 0u;
                         if (p.truth) {                         // confusion counters of sets k and 32 + k (rfi_plan_set_truth)
-                            const uint32_t tw = __ldg(p.truth + (size_t)w_global * fwpw + tile);
                             const uint32_t cw = cnt_base + (uint32_t)warp * 768u + (uint32_t)lane * 4u;
                             red_shared_add(cw, __popc(f_lo & ~tw));
                             red_shared_add(cw + 128u, __popc(~f_lo & tw));
