@@ -57,6 +57,7 @@ struct rfi_plan {
     uint64_t* d_counts = nullptr;
     bool truth_fused = false;                 // the last enqueue counted in its own kernel
     bool count_now = false;                   // inside rfi_process_chunk with a truth mask set
+    int truth_K = 0;                          // K at rfi_plan_set_truth time: d_counts was sized for it
     int n_baselines_total = 0, b_first = 0;   // n_baselines is the shard this plan processes (default: all)
     int K = 0;
     std::vector<rfi_thresholds> thr;
@@ -547,6 +548,7 @@ int rfi_plan_set_truth(rfi_plan* p, const uint32_t* d_truth, uint64_t* d_counts)
     if (reinterpret_cast<uintptr_t>(d_truth) % 4 || reinterpret_cast<uintptr_t>(d_counts) % 8) return RFI_EINVAL;
     p->d_truth = d_truth;
     p->d_counts = d_counts;
+    p->truth_K = p->K;
     return RFI_OK;
 }
 
@@ -598,6 +600,11 @@ int rfi_process_chunk(rfi_plan* p, const void* d_vis, void* d_avg, void* d_weigh
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     int rc = prepare(p, st);
     if (rc != RFI_OK) return rc;
+    if (p->d_truth && p->truth_K != p->K) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "rfi_plan_set_truth was called with K = %d threshold sets, the plan now has %d: "
+                 "set the truth mask (and a counter buffer of K x 4) again", p->truth_K, p->K);
+        return RFI_ESTATE;
+    }
     if (p->d_truth) RFI_CUDA(cudaMemsetAsync(p->d_counts, 0, (size_t)p->K * 4 * sizeof(uint64_t), st));
     p->count_now = p->d_truth != nullptr;
     rc = enqueue_slab(p, d_vis, 0, p->n_out(), static_cast<float*>(d_avg), static_cast<uint32_t*>(d_weight),

@@ -510,6 +510,15 @@ def test_in_kernel_confusion_counters_equal_the_mask_pass(monkeypatch, n_chan, K
     separate = plan.confusion_counts(tw).cpu().numpy()
     plan.destroy()
     np.testing.assert_array_equal(fused, separate)
+    if K == 5:                                             # the counter buffer was sized for K sets: a new K needs a new one
+        plan2 = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M, n_int=w.n_int)
+        plan2.set_thresholds(thr)
+        plan2.set_truth(tw)
+        plan2.set_thresholds(thr[:3])
+        avg3, weight3, _ = plan2.alloc_outputs()
+        with pytest.raises(rfi.RfiError):
+            plan2.process_chunk(d_vis, avg3, weight3)
+        plan2.destroy()
     assert fused[:, 1].min() > 0 and fused[:, 3].min() > 0 and (fused[:, 0] + fused[:, 2]).max() > 0
 
 
