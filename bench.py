@@ -480,6 +480,8 @@ def run_ours(args):
     plan.set_variant(args.variant)
     if args.adaptive > 0:                 # on-line threshold adaptation (rfi_plan_set_adaptive): kernel + a one-CTA update per step
         plan.set_adaptive(args.adaptive, 0.5)
+        if args.adaptive_scope == "baseline":
+            plan.set_adaptive_scope("baseline")
     avg, weight, _ = plan.alloc_outputs(device=dev)
     out_bytes = avg.numel() * 4 + weight.numel() * 4 + max(plan.K, 1) * plan.n_win * plan.n_baselines * plan.wpb * 4
     in_bytes = vis.numel() * vis.element_size()            # this rank's input (the whole chunk unless sharded)
@@ -674,6 +676,7 @@ def run_ours(args):
                    "arithmetic": args.arith if args.arith == "fast" else f"tables, mask {args.mask:#06x}",
                    "threshold_classes": 2 if two_classes else 1, "layout": args.layout,
                    "adaptive_false_alarm": args.adaptive if args.adaptive > 0 else None,
+                   "adaptive_scope": args.adaptive_scope if args.adaptive > 0 else None,
                    "input_bytes": w.input_bytes,
                    "l2": ("L2 flushed between timed iterations (256 MB write, outside the timed events)" if small
                           else "input (>= 9 GB) is far larger than the 126 MB L2: no flush needed"),
@@ -714,6 +717,8 @@ def main():
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="N > 1: weak = one chunk per rank; strong = ONE chunk sharded by baseline (rfi_plan_set_baseline_shard)")
     ap.add_argument("--no-configs", action="store_true", help="skip the per-config sub-records of the default run")
+    ap.add_argument("--adaptive-scope", default="class", choices=["class", "baseline"],
+                    help="with --adaptive: one threshold set per baseline class, or per baseline stream (rfi_plan_set_adaptive_scope)")
     ap.add_argument("--adaptive", type=float, default=0.0,
                     help="hold this false-alarm rate by on-line threshold adaptation (rfi_plan_set_adaptive, DESIGN.md NEXT-3)")
     ap.add_argument("--no-e2e", action="store_true")

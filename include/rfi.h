@@ -181,6 +181,23 @@ int rfi_set_thresholds(rfi_plan *plan, int K, const rfi_thresholds *h_sets);
  * returns RFI_EINVAL).  RFI_EINVAL unless 0 <= false_alarm < 0.5 and 0 <= forget < 1. */
 int rfi_plan_set_adaptive(rfi_plan *plan, float false_alarm, float forget);
 
+/* Scope of the adaptation.  RFI_ADAPT_PER_CLASS (default): one pair of histograms and one threshold set per baseline
+ * class, as above.  RFI_ADAPT_PER_BASELINE: "fine-tuning for each data stream" (every baseline stream is
+ * mitigated separately) -- every baseline of the plan (of its shard) keeps its own running histograms and
+ * its own (s_low, s_high, gamma); it starts from the a-priori set of its class and follows its own null distribution
+ * from the second chunk on (same rule, readings A1-A6 with "class" read as "baseline"; a baseline contributes
+ * n_chan / F x windows counts per chunk, and keeps its thresholds while it has fewer than 1000).  The streaming kernel
+ * counts into a histogram private to the warp -- a 32-cell tile lies in one baseline, hence n_chan % 32 == 0 is required
+ * (RFI_EINVAL from rfi_process_chunk otherwise) -- and adds it to the baseline's device histogram at the end of each
+ * (tile, integration) unit; the update kernel runs one CTA per two baselines.  Restarts the adaptation. */
+enum { RFI_ADAPT_PER_CLASS = 0, RFI_ADAPT_PER_BASELINE = 1 };
+int rfi_plan_set_adaptive_scope(rfi_plan *plan, int scope);
+/* RFI_ADAPT_PER_BASELINE only: the thresholds in force for the next chunk, h_out[n_baselines] (of the shard), and the
+ * running histograms, h_out[n_baselines][768 tau bins | 384 r bins] doubles.  Both wait for the device work issued so
+ * far.  RFI_ESTATE before the first adaptive chunk or in the per-class scope. */
+int rfi_plan_get_stream_thresholds(rfi_plan *plan, rfi_thresholds *h_out);
+int rfi_plan_get_stream_histograms(rfi_plan *plan, double *h_out);
+
 /* The thresholds currently in force, one set per baseline class (h_out[n_classes], host memory): the adapted ones
  * when adaptation is on (waits for the device work enqueued so far), else set 0 of rfi_set_thresholds. */
 int rfi_plan_get_thresholds(rfi_plan *plan, rfi_thresholds *h_out);

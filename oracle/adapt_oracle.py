@@ -18,6 +18,10 @@ The paper names the problem and gives no algorithm: the hyper-parameters come fr
   A6  a class with fewer than n_min counted windows keeps its thresholds; the thresholds of chunk n+1 are those
       computed after chunk n (the first chunk runs with the thresholds given a priori).
 
+  A7  scope: the functions below serve ONE stream kind; the product keeps one state per baseline class or, with
+      RFI_ADAPT_PER_BASELINE, one per baseline ("fine-tuning for each data stream") -- the tests then call
+      them baseline by baseline.
+
 Plain numpy / fp64; shares no code with csrc/rfi_adapt.cu; only tests/ may import it.
 """
 from __future__ import annotations

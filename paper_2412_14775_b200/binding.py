@@ -26,7 +26,8 @@ EXPORTS = [
     "rfi_strerror", "rfi_last_cuda_error", "rfi_flags_bytes", "rfi_avg_bytes", "rfi_weight_bytes",
     "rfi_stats_bytes", "rfi_vis_bytes", "rfi_plan_launch_count", "rfi_plan_last_variant", "rfi_version",
     "rfi_probe_read_bandwidth", "rfi_probe_mix_bandwidth", "rfi_sim42_generate", "rfi_sim42_vis_bytes", "rfi_sim42_truth_bytes",
-    "rfi_rl_evaluate", "rfi_plan_set_adaptive", "rfi_plan_get_thresholds",
+    "rfi_rl_evaluate", "rfi_plan_set_adaptive", "rfi_plan_set_adaptive_scope", "rfi_plan_get_stream_thresholds",
+    "rfi_plan_get_stream_histograms", "rfi_plan_get_thresholds",
     "rfi_plan_get_adaptive_histogram",
 ]
 
@@ -99,6 +100,12 @@ def load_library(build_if_missing: bool = True):
     lib.rfi_plan_set_variant.argtypes = [vp, ci]
     lib.rfi_plan_set_adaptive.argtypes = [vp, ctypes.c_float, ctypes.c_float]
     lib.rfi_plan_set_adaptive.restype = ci
+    lib.rfi_plan_set_adaptive_scope.argtypes = [vp, ci]
+    lib.rfi_plan_set_adaptive_scope.restype = ci
+    lib.rfi_plan_get_stream_thresholds.argtypes = [vp, ctypes.POINTER(RfiThresholds)]
+    lib.rfi_plan_get_stream_thresholds.restype = ci
+    lib.rfi_plan_get_stream_histograms.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
+    lib.rfi_plan_get_stream_histograms.restype = ci
     lib.rfi_plan_get_thresholds.argtypes = [vp, ctypes.POINTER(RfiThresholds)]
     lib.rfi_plan_get_thresholds.restype = ci
     lib.rfi_plan_get_adaptive_histogram.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
@@ -233,6 +240,26 @@ class RfiPlan:
         """rfi_plan_set_adaptive: hold `false_alarm` on RFI-free data by tracking the null quantiles of both statistics
         per baseline class, chunk by chunk, on the device (0 switches it off)."""
         _check(self._lib.rfi_plan_set_adaptive(self._h, float(false_alarm), float(forget)), "rfi_plan_set_adaptive")
+
+    def set_adaptive_scope(self, scope: str):
+        """rfi_plan_set_adaptive_scope: "class" (one threshold set per baseline class) or "baseline" (every baseline
+        stream adapts its own thresholds: the paper's "fine-tuning for each data stream")."""
+        _check(self._lib.rfi_plan_set_adaptive_scope(self._h, {"class": 0, "baseline": 1}[scope]), "rfi_plan_set_adaptive_scope")
+
+    def get_stream_thresholds(self):
+        """rfi_plan_get_stream_thresholds: float64 array [n_baselines, 4] = (d, s_low, s_high, gamma) per baseline stream."""
+        import numpy as np
+        arr = (RfiThresholds * self.n_baselines)()
+        _check(self._lib.rfi_plan_get_stream_thresholds(self._h, arr), "rfi_plan_get_stream_thresholds")
+        return np.array([(t.d, t.s_low, t.s_high, t.gamma) for t in arr], dtype=np.float64)
+
+    def get_stream_histograms(self):
+        """rfi_plan_get_stream_histograms: float64 array [n_baselines, 1152] (768 tau bins | 384 r bins), running counts."""
+        import numpy as np
+        buf = np.empty((self.n_baselines, 1152), dtype=np.float64)
+        _check(self._lib.rfi_plan_get_stream_histograms(self._h, buf.ctypes.data_as(ctypes.POINTER(ctypes.c_double))),
+               "rfi_plan_get_stream_histograms")
+        return buf
 
     def get_thresholds(self):
         """rfi_plan_get_thresholds: [(d, s_low, s_high, gamma)] per baseline class, as currently in force."""

@@ -55,12 +55,17 @@ __device__ double adapt_quantile_warp(const double* h, int n_bins, int lo_exp, d
 
 // hist: this chunk's counts [2][kAdaptBins] (zeroed here for the next chunk); acc: running histograms (double);
 // thr: the device thresholds the streaming kernel reads; raw: the same as (d, s_low, s_high, gamma) for inspection.
-__global__ void __launch_bounds__(256) rfi_adapt_update_kernel(uint32_t* __restrict__ hist, double* __restrict__ acc,
-                                                               Thr* __restrict__ thr, rfi_thresholds* __restrict__ raw,
+__global__ void __launch_bounds__(256) rfi_adapt_update_kernel(uint32_t* hist, double* acc, Thr* thr, rfi_thresholds* raw,
                                                                int n_classes, double beta, double forget, double n_min) {
     __shared__ double sh[2 * kAdaptBins];
     __shared__ double tot[4];
-    for (int i = threadIdx.x; i < 2 * kAdaptBins; i += blockDim.x) {
+    // one CTA per pair of histograms: the two classes, or baseline streams 2 b, 2 b + 1 (n_classes = streams in all)
+    hist += (size_t)blockIdx.x * 2 * kAdaptBins;
+    acc += (size_t)blockIdx.x * 2 * kAdaptBins;
+    thr += blockIdx.x * 2;
+    raw += blockIdx.x * 2;
+    n_classes = min(2, n_classes - 2 * (int)blockIdx.x);
+    for (int i = threadIdx.x; i < n_classes * kAdaptBins; i += blockDim.x) {
         const double v = forget * acc[i] + (double)hist[i];   // A3
         acc[i] = v;
         sh[i] = v;
@@ -68,7 +73,7 @@ __global__ void __launch_bounds__(256) rfi_adapt_update_kernel(uint32_t* __restr
     }
     __syncthreads();
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    if (warp < 4) {                                           // totals: warp w sums histogram (class w/2, tau or r)
+    if (warp < 2 * n_classes) {                               // totals: warp w sums histogram (class w/2, tau or r)
         const int cls = warp >> 1, is_r = warp & 1;
         const double* h = sh + cls * kAdaptBins + (is_r ? kAdaptTauBins : 0);
         const int seg = (is_r ? kAdaptRBins : kAdaptTauBins) >> 5;
@@ -105,7 +110,7 @@ namespace rfi_host {
 int launch_adapt_update(uint32_t* d_hist, double* d_acc, rfi::Thr* d_thr, rfi_thresholds* d_raw, int n_classes,
                         double alpha, double forget, cudaStream_t st) {
     const double beta = 1.0 - sqrt(1.0 - alpha);
-    rfi::rfi_adapt_update_kernel<<<1, 256, 0, st>>>(d_hist, d_acc, d_thr, d_raw, n_classes, beta, forget, 1000.0);
+    rfi::rfi_adapt_update_kernel<<<(unsigned)((n_classes + 1) / 2), 256, 0, st>>>(d_hist, d_acc, d_thr, d_raw, n_classes, beta, forget, 1000.0);
     RFI_CUDA(cudaGetLastError());
     return RFI_OK;
 }

@@ -79,7 +79,12 @@ struct rfi_plan {
     rfi_thresholds* d_thr_raw = nullptr;       // [2] the same as (d, s_low, s_high, gamma)
     uint32_t* d_hist = nullptr;                // [2][kAdaptBins] this chunk's counts
     double* d_hist_acc = nullptr;              // [2][kAdaptBins] running histograms
+    std::vector<rfi::Thr> adapt_stage_thr;     // host staging of the a-priori thresholds (per class or per stream)
+    std::vector<rfi_thresholds> adapt_stage_raw;
     bool adapt_uploaded = false;               // d_thr holds the a-priori thresholds / the state was reset
+    int adapt_scope = RFI_ADAPT_PER_CLASS;     // thresholds and histograms per class ([2]) or per baseline stream
+    int adapt_cap = 0;                         // streams the adaptation buffers were allocated for
+    int adapt_streams() const { return adapt_scope == RFI_ADAPT_PER_BASELINE ? n_baselines : 2; }
     // host path
     void* d_stage[2] = {nullptr, nullptr};
     size_t d_stage_cap[2] = {0, 0};
@@ -249,7 +254,7 @@ int enqueue_slab(rfi_plan* p, const void* d_vis_slab, int o_first, int n_out_sla
     kp.K = p->K;
     kp.k_first = 0;
     kp.flags_atomic = (p->n_chan % 32 != 0 && 32 % p->n_chan != 0) ? 1 : 0;
-    if (p->adapt_alpha > 0.0) { kp.d_thr = p->d_thr; kp.hist = p->d_hist; }
+    if (p->adapt_alpha > 0.0) { kp.d_thr = p->d_thr; kp.hist = p->d_hist; kp.adapt_streams = p->adapt_scope == RFI_ADAPT_PER_BASELINE; }
     p->truth_fused = false;
 
     const bool fp16 = p->precision == RFI_FP16;
@@ -406,23 +411,37 @@ int prepare(rfi_plan* p, cudaStream_t st) {
                      "and the direct kernel (RFI_VARIANT_AUTO or RFI_VARIANT_DIRECT)");
             return RFI_EINVAL;
         }
-        const size_t hb = 2 * (size_t)rfi::kAdaptBins;
-        if (!p->d_thr) {
-            if (cudaMalloc(&p->d_thr, 2 * sizeof(rfi::Thr)) != cudaSuccess || cudaMalloc(&p->d_thr_raw, 2 * sizeof(rfi_thresholds)) != cudaSuccess ||
+        if (p->adapt_scope == RFI_ADAPT_PER_BASELINE && p->n_chan % 32 != 0) {
+            snprintf(g_cuda_err, sizeof(g_cuda_err), "adaptation per baseline stream needs n_chan %% 32 == 0 (a 32-cell tile must lie in one baseline)");
+            return RFI_EINVAL;
+        }
+        const int ns = p->adapt_streams();
+        const size_t hb = (size_t)ns * rfi::kAdaptBins;
+        if (!p->d_thr || ns > p->adapt_cap) {
+            cudaFree(p->d_thr); cudaFree(p->d_thr_raw); cudaFree(p->d_hist); cudaFree(p->d_hist_acc);
+            p->d_thr = nullptr; p->d_thr_raw = nullptr; p->d_hist = nullptr; p->d_hist_acc = nullptr; p->adapt_cap = 0;
+            if (cudaMalloc(&p->d_thr, ns * sizeof(rfi::Thr)) != cudaSuccess || cudaMalloc(&p->d_thr_raw, ns * sizeof(rfi_thresholds)) != cudaSuccess ||
                 cudaMalloc(&p->d_hist, hb * sizeof(uint32_t)) != cudaSuccess || cudaMalloc(&p->d_hist_acc, hb * sizeof(double)) != cudaSuccess) {
                 cudaGetLastError();
                 return RFI_ENOMEM;
             }
+            p->adapt_cap = ns;
             p->adapt_uploaded = false;
         }
         if (!p->adapt_uploaded) {
-            // (re)start from the thresholds given a priori: pageable host source, so the copies are
-            // complete with respect to the host when the calls return
+            // (re)start from the thresholds given a priori: every stream begins with its class's set.  The host
+            // staging vectors live in the plan, so the asynchronous copies may complete after this call returns.
             const int nc = p->n_classes;
-            rfi::Thr t[2] = {to_device_thr(p->thr[0], p->M * p->F), to_device_thr(p->thr[nc - 1], p->M * p->F)};
-            rfi_thresholds r[2] = {p->thr[0], p->thr[nc - 1]};
-            RFI_CUDA(cudaMemcpyAsync(p->d_thr, t, sizeof(t), cudaMemcpyHostToDevice, st));
-            RFI_CUDA(cudaMemcpyAsync(p->d_thr_raw, r, sizeof(r), cudaMemcpyHostToDevice, st));
+            p->adapt_stage_thr.resize(ns);
+            p->adapt_stage_raw.resize(ns);
+            for (int i = 0; i < ns; ++i) {
+                int cls = i == 0 ? 0 : nc - 1;                // per class: [0] = class 0, [1] = class 1 (or 0 again)
+                if (p->adapt_scope == RFI_ADAPT_PER_BASELINE) cls = nc > 1 ? (int)p->h_cls[p->b_first + i] : 0;
+                p->adapt_stage_thr[i] = to_device_thr(p->thr[cls], p->M * p->F);
+                p->adapt_stage_raw[i] = p->thr[cls];
+            }
+            RFI_CUDA(cudaMemcpyAsync(p->d_thr, p->adapt_stage_thr.data(), ns * sizeof(rfi::Thr), cudaMemcpyHostToDevice, st));
+            RFI_CUDA(cudaMemcpyAsync(p->d_thr_raw, p->adapt_stage_raw.data(), ns * sizeof(rfi_thresholds), cudaMemcpyHostToDevice, st));
             RFI_CUDA(cudaMemsetAsync(p->d_hist, 0, hb * sizeof(uint32_t), st));
             RFI_CUDA(cudaMemsetAsync(p->d_hist_acc, 0, hb * sizeof(double), st));
             p->adapt_uploaded = true;
@@ -434,7 +453,8 @@ int prepare(rfi_plan* p, cudaStream_t st) {
 // After the chunk's kernels: fold the chunk's histograms into the running ones and set the next chunk's thresholds.
 int finish_adaptive(rfi_plan* p, cudaStream_t st) {
     if (p->adapt_alpha <= 0.0) return RFI_OK;
-    const int rc = launch_adapt_update(p->d_hist, p->d_hist_acc, p->d_thr, p->d_thr_raw, p->n_classes, p->adapt_alpha,
+    const int rc = launch_adapt_update(p->d_hist, p->d_hist_acc, p->d_thr, p->d_thr_raw,
+                                       p->adapt_scope == RFI_ADAPT_PER_BASELINE ? p->n_baselines : p->n_classes, p->adapt_alpha,
                                        p->adapt_forget, st);
     if (rc == RFI_OK) p->launches++;
     return rc;
@@ -524,6 +544,7 @@ int rfi_plan_set_baseline_shard(rfi_plan* p, int b_first, int b_count) {
     p->b_first = b_first;
     p->n_baselines = b_count;
     p->have_result = false;
+    p->adapt_uploaded = false;                // per-stream adaptation state belongs to the old baseline range
     p->maps.clear();
     return RFI_OK;
 }
@@ -561,9 +582,31 @@ int rfi_plan_set_adaptive(rfi_plan* p, float false_alarm, float forget) {
     return RFI_OK;
 }
 
+int rfi_plan_set_adaptive_scope(rfi_plan* p, int scope) {
+    if (!p || (scope != RFI_ADAPT_PER_CLASS && scope != RFI_ADAPT_PER_BASELINE)) return RFI_EINVAL;
+    p->adapt_scope = scope;
+    p->adapt_uploaded = false;
+    p->have_result = false;
+    return RFI_OK;
+}
+
+int rfi_plan_get_stream_thresholds(rfi_plan* p, rfi_thresholds* h_out) {
+    if (!p || !h_out) return RFI_EINVAL;
+    if (p->adapt_scope != RFI_ADAPT_PER_BASELINE || p->adapt_alpha <= 0.0 || !p->d_thr_raw || !p->adapt_uploaded) return RFI_ESTATE;
+    RFI_CUDA(cudaMemcpy(h_out, p->d_thr_raw, (size_t)p->n_baselines * sizeof(rfi_thresholds), cudaMemcpyDeviceToHost));
+    return RFI_OK;
+}
+
+int rfi_plan_get_stream_histograms(rfi_plan* p, double* h_out) {
+    if (!p || !h_out) return RFI_EINVAL;
+    if (p->adapt_scope != RFI_ADAPT_PER_BASELINE || p->adapt_alpha <= 0.0 || !p->d_hist_acc || !p->adapt_uploaded) return RFI_ESTATE;
+    RFI_CUDA(cudaMemcpy(h_out, p->d_hist_acc, (size_t)p->n_baselines * rfi::kAdaptBins * sizeof(double), cudaMemcpyDeviceToHost));
+    return RFI_OK;
+}
+
 int rfi_plan_get_adaptive_histogram(rfi_plan* p, double* h_out) {
     if (!p || !h_out) return RFI_EINVAL;
-    if (p->adapt_alpha <= 0.0 || !p->d_hist_acc || !p->adapt_uploaded) return RFI_ESTATE;
+    if (p->adapt_scope != RFI_ADAPT_PER_CLASS || p->adapt_alpha <= 0.0 || !p->d_hist_acc || !p->adapt_uploaded) return RFI_ESTATE;
     RFI_CUDA(cudaMemcpy(h_out, p->d_hist_acc, 2 * (size_t)rfi::kAdaptBins * sizeof(double), cudaMemcpyDeviceToHost));
     return RFI_OK;
 }
@@ -572,7 +615,7 @@ int rfi_plan_get_thresholds(rfi_plan* p, rfi_thresholds* h_out) {
     if (!p || !h_out) return RFI_EINVAL;
     if (p->K < 1) return RFI_ESTATE;
     const int nc = p->n_classes;
-    if (p->adapt_alpha > 0.0 && p->d_thr_raw && p->adapt_uploaded) {
+    if (p->adapt_alpha > 0.0 && p->d_thr_raw && p->adapt_uploaded && p->adapt_scope == RFI_ADAPT_PER_CLASS) {
         rfi_thresholds r[2];
         RFI_CUDA(cudaMemcpy(r, p->d_thr_raw, sizeof(r), cudaMemcpyDeviceToHost));    // waits for the device work so far
         for (int c = 0; c < nc; ++c) h_out[c] = r[c == 0 ? 0 : 1];

@@ -26,7 +26,7 @@ __device__ __forceinline__ void load_block(const uint8_t* ptr, size_t row_stride
 
 // One (tile, integration) unit of the direct kernel.  ADAPT (on-line threshold adaptation, rfi_adapt.cu): the lane's
 // thresholds are read from device memory once per unit and every window is counted in the CTA's histogram.
-template <int R, bool FP16, bool ALIGN32, bool ADAPT>
+template <int R, bool FP16, bool ALIGN32, int ADAPT>
 __device__ __forceinline__ void direct_unit(const KParams& p, const int unit, const int n_tiles, uint32_t* sh_hist) {
     constexpr int SAMPLE_BYTES = FP16 ? 16 : 32;
     const int lane = threadIdx.x & 31;
@@ -50,7 +50,10 @@ __device__ __forceinline__ void direct_unit(const KParams& p, const int unit, co
     int blk = 0, b_in_win = 0;
 
     Thr thr_dev;
-    if constexpr (ADAPT) thr_dev = p.d_thr[g.cls];
+    // ADAPT = 1: thresholds and histograms per baseline class; ADAPT = 2: per baseline STREAM (the tile lies in one baseline:
+    // n_chan % 32 == 0, checked by the host), histogram private to the warp and flushed at the end of the unit
+    const int stream = ADAPT == 2 ? (tile * 32) / p.n_chan : g.cls;
+    if constexpr (ADAPT != 0) thr_dev = p.d_thr[stream];
     Raw<FP16> A[R], B[R];
     auto window_end = [&]() {
         ++blk;
@@ -110,24 +113,39 @@ __device__ __forceinline__ void direct_unit(const KParams& p, const int unit, co
         if (blk < total) step(A, B);
     }
     store_output(p, g, p.k_first, o_global, acc, wt);
+    if constexpr (ADAPT == 2) {
+        __syncwarp();
+        uint32_t* dst = p.hist + (size_t)stream * kAdaptBins;
+        for (int i = lane; i < kAdaptBins; i += 32) {
+            const uint32_t c = sh_hist[i];
+            if (c) { atomicAdd(dst + i, c); sh_hist[i] = 0u; }
+        }
+        __syncwarp();
+    }
 }
 
-template <int R, bool FP16, bool ALIGN32, bool ADAPT = false>
+template <int R, bool FP16, bool ALIGN32, int ADAPT = 0>
 __global__ void __launch_bounds__(128, (FP16 || R <= 4) ? 4 : (R == 5 ? 3 : 2)) rfi_direct_kernel(const KParams p) {
     const int n_tiles = (p.n_cells + 31) >> 5;
     const int unit = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    if constexpr (!ADAPT) {
-        if (unit < n_tiles * p.n_out_slab) direct_unit<R, FP16, ALIGN32, false>(p, unit, n_tiles, nullptr);
-    } else {
+    if constexpr (ADAPT == 0) {
+        if (unit < n_tiles * p.n_out_slab) direct_unit<R, FP16, ALIGN32, 0>(p, unit, n_tiles, nullptr);
+    } else if constexpr (ADAPT == 1) {
         __shared__ uint32_t sh_hist[2 * kAdaptBins];          // [class][tau bins | r bins], flushed once per CTA
         for (int i = threadIdx.x; i < 2 * kAdaptBins; i += blockDim.x) sh_hist[i] = 0u;
         __syncthreads();
-        if (unit < n_tiles * p.n_out_slab) direct_unit<R, FP16, ALIGN32, true>(p, unit, n_tiles, sh_hist);
+        if (unit < n_tiles * p.n_out_slab) direct_unit<R, FP16, ALIGN32, 1>(p, unit, n_tiles, sh_hist);
         __syncthreads();
         for (int i = threadIdx.x; i < 2 * kAdaptBins; i += blockDim.x) {
             const uint32_t c = sh_hist[i];
             if (c) atomicAdd(p.hist + i, c);
         }
+    } else {
+        __shared__ uint32_t sh_hist[4 * kAdaptBins];          // one [tau bins | r bins] histogram per warp (= per unit = one stream)
+        uint32_t* mine = sh_hist + (threadIdx.x >> 5) * kAdaptBins;
+        for (int i = threadIdx.x & 31; i < kAdaptBins; i += 32) mine[i] = 0u;
+        __syncwarp();
+        if (unit < n_tiles * p.n_out_slab) direct_unit<R, FP16, ALIGN32, 2>(p, unit, n_tiles, mine);
     }
 }
 

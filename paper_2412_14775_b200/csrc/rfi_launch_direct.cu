@@ -12,9 +12,12 @@ int launch_r(const rfi::KParams& kp, cudaStream_t st) {
     const unsigned grid = (unsigned)((n_units + 3) / 4);
     // 256-bit loads need a 32-byte aligned sample: base % 32 == 0 (the sample stride is 32 B)
     const bool a32 = FP16 || (reinterpret_cast<uintptr_t>(kp.vis) % 32 == 0);
-    if (kp.d_thr) {                                            // on-line threshold adaptation (rfi_plan_set_adaptive)
-        if (a32) rfi::rfi_direct_kernel<R, FP16, true, true><<<grid, 128, 0, st>>>(kp);
-        else     rfi::rfi_direct_kernel<R, FP16, false, true><<<grid, 128, 0, st>>>(kp);
+    if (kp.d_thr && kp.adapt_streams) {                        // on-line adaptation per baseline stream
+        if (a32) rfi::rfi_direct_kernel<R, FP16, true, 2><<<grid, 128, 0, st>>>(kp);
+        else     rfi::rfi_direct_kernel<R, FP16, false, 2><<<grid, 128, 0, st>>>(kp);
+    } else if (kp.d_thr) {                                     // on-line threshold adaptation per class (rfi_plan_set_adaptive)
+        if (a32) rfi::rfi_direct_kernel<R, FP16, true, 1><<<grid, 128, 0, st>>>(kp);
+        else     rfi::rfi_direct_kernel<R, FP16, false, 1><<<grid, 128, 0, st>>>(kp);
     } else {
         if (a32) rfi::rfi_direct_kernel<R, FP16, true><<<grid, 128, 0, st>>>(kp);
         else     rfi::rfi_direct_kernel<R, FP16, false><<<grid, 128, 0, st>>>(kp);

@@ -223,8 +223,9 @@ __device__ __forceinline__ void store_output(const KParams& p, const LaneGeom& g
 
 // Single-set window tail shared by the streaming kernels: statistics, decision, flag word, statistics planes,
 // masked accumulation into the output integration.  ADAPT: the thresholds come from device memory
-// (`thr`, the lane's class) and the window's tau and max(r_re, r_im) are counted in the CTA's shared-memory histogram.
-template <bool ADAPT = false>
+// (`thr`: the lane's class, ADAPT = 1, or the lane's baseline stream, ADAPT = 2) and the window's tau and max(r_re, r_im)
+// are counted in a shared-memory histogram (the CTA's per-class pair, or the warp's own for its stream).
+template <int ADAPT = 0>
 __device__ __forceinline__ void finish_window(const KParams& p, const LaneGeom& g, Win& w, float inv_W,
                                               int w_global, f2 (&acc)[4], uint32_t& wt,
                                               const Thr* thr = nullptr, uint32_t* sh_hist = nullptr) {
@@ -239,7 +240,7 @@ __device__ __forceinline__ void finish_window(const KParams& p, const LaneGeom& 
     store_stats(p, g, w_global, tau, r_re, r_im);
     if constexpr (ADAPT) {
         if (g.valid && fabsf(tau) <= 3.402823466e38f && fabsf(r_max) <= 3.402823466e38f) {   // finite statistics only
-            uint32_t* h = sh_hist + g.cls * kAdaptBins;
+            uint32_t* h = sh_hist + (ADAPT == 1 ? g.cls * kAdaptBins : 0);   // per class: the CTA's; per stream: the warp's own
             atomicAdd(h + adapt_bin(tau, kAdaptTauLoExp, kAdaptTauBins), 1u);
             atomicAdd(h + kAdaptTauBins + adapt_bin(r_max, kAdaptRLoExp, kAdaptRBins), 1u);
         }

@@ -74,6 +74,76 @@ def test_histograms_thresholds_and_next_chunk_flags_match_the_oracle(fp16, F, fo
     plan.destroy()
 
 
+@pytest.mark.parametrize("fp16,F,forget,shard", [(False, 1, 0.0, None), (True, 1, 0.5, None), (False, 2, 0.25, None), (False, 1, 0.0, (5, 40))])
+def test_per_baseline_adaptation_matches_the_oracle_stream_by_stream(fp16, F, forget, shard):
+    """RFI_ADAPT_PER_BASELINE ("fine-tuning for each data stream"): every baseline keeps its own running
+    histograms and thresholds.  Per baseline and chunk: the flags are the oracle's with the thresholds in force, the running
+    histograms equal the oracle's (bit-exact: both bin the float32 statistics the kernel stored), the next thresholds match."""
+    M = 16 if F == 1 else 10
+    w = synth.Workload("adapt_streams", 10, True, 64, M * 64, M, M * 32, fp16=fp16, window_F=F, channel_gain=True, burst_cell_frac=0.03)
+    W = M * F
+    thr_c, thr_a = synth.default_thresholds(W)[0], synth.auto_thresholds(W)
+    plan, autos = _plan(w, thr_c, thr_a, 0.05, forget)
+    plan.set_adaptive_scope("baseline")
+    b0, nb = shard if shard else (0, w.n_baselines)
+    if shard:
+        plan.set_baseline_shard(b0, nb)
+    acc = [None] * nb
+    cur = [tuple((thr_a if autos[b0 + b] else thr_c)[1:]) for b in range(nb)]
+    d_of = [float((thr_a if autos[b0 + b] else thr_c)[0]) for b in range(nb)]
+    for chunk in range(3):
+        vis, _ = synth.make_chunk(w, seed=300 + chunk)
+        vis = vis[:, b0:b0 + nb].contiguous()
+        out = _run(plan, w, vis)
+        v = vis.numpy().reshape(w.n_time, nb * w.n_chan, 4, 2)
+        hist = plan.get_stream_histograms()
+        got = plan.get_stream_thresholds()
+        assert hist.shape == (nb, 1152) and got.shape == (nb, 4)
+        for b in range(nb):
+            sel = slice(b * w.n_chan, (b + 1) * w.n_chan)
+            if b % 7 == 0 or chunk == 2:                      # the fp64 flag comparison on a subset (it is the slow part)
+                sub = {k: (a[:, :, sel] if a.ndim >= 3 else a[:, sel]) for k, a in out.items()}
+                compare(v[:, sel], M, w.n_int, [[d_of[b], *cur[b]]], sub, tol=2e-3 if fp16 else 1e-5, fp16=fp16, F=F)
+            tau = out["tau"][:, sel]
+            rmax = np.fmax(out["r_re"][:, sel], out["r_im"][:, sel])
+            rmax = np.where(np.isnan(out["r_re"][:, sel]) | np.isnan(out["r_im"][:, sel]), np.nan, rmax)
+            ht, hr = ao.histogram(tau, rmax)
+            acc_t, acc_r, new = ao.update(acc[b][0] if acc[b] else None, acc[b][1] if acc[b] else None, ht, hr,
+                                          alpha=0.05, forget=forget, previous=cur[b])
+            acc[b] = (acc_t, acc_r)
+            assert np.array_equal(hist[b, :768], acc_t) and np.array_equal(hist[b, 768:], acc_r), f"histogram of baseline {b}, chunk {chunk}"
+            new32 = tuple(float(np.float32(x)) for x in new)
+            assert np.allclose(got[b, 1:], new32, rtol=1e-6, atol=0), (b, got[b], new32)
+            assert got[b, 0] == np.float32(d_of[b])
+            cur[b] = tuple(float(x) for x in got[b, 1:])
+    # the streams really went their own ways
+    assert np.unique(plan.get_stream_thresholds()[:, 3]).size > nb // 2
+    plan.destroy()
+
+
+def test_per_baseline_adaptation_holds_the_rate_on_every_stream_and_rejects_ragged_channels():
+    w = synth.Workload("adapt_streams_clean", 12, True, 64, 2048, 16, 512, channel_gain=True)
+    plan, autos = _plan(w, [1.0, 0.0, 50.0, 1.0], [1.0, 0.0, 50.0, 1.0], 0.05)            # a priori: flag nothing
+    plan.set_adaptive_scope("baseline")
+    for chunk in range(3):
+        vis, _ = synth.make_chunk(w, seed=700 + chunk)
+        out = _run(plan, w, vis)
+        per_b = out["flags"][0].reshape(-1, w.n_baselines, w.n_chan).mean(axis=(0, 2))
+        if chunk == 0:
+            assert per_b.max() == 0.0
+        else:                                                # 8192 windows per baseline and chunk: sigma of the rate ~ 0.003
+            assert np.all(np.abs(per_b - 0.05) < 0.015), (per_b.min(), per_b.max())
+            assert abs(per_b.mean() - 0.05) < 0.003
+    plan.destroy()
+    w2 = synth.Workload("adapt_streams_ragged", 4, True, 48, 256, 16, 128)
+    plan, _ = _plan(w2, [1.0, 0.0, 50.0, 1.0], [1.0, 0.0, 50.0, 1.0], 0.05)
+    plan.set_adaptive_scope("baseline")
+    avg, weight, _ = plan.alloc_outputs()
+    with pytest.raises(rfi.RfiError):
+        plan.process_chunk(synth.make_chunk(w2, seed=1)[0].cuda(), avg, weight)
+    plan.destroy()
+
+
 def test_false_alarm_rate_is_held_on_clean_noise_for_cross_and_auto_streams():
     """Done-criterion of VERDICT r01 item 9: measured FA on RFI-free synthetic noise within +-0.5 % (absolute) of the
     request, separately for the cross- and the auto-correlations, from deliberately wrong a-priori thresholds."""
