@@ -205,7 +205,8 @@ def test_adaptive_mode_rejects_unsupported_plans_and_can_be_switched_off():
     plan.destroy()
 
 
-def test_adaptive_step_is_cuda_graph_capturable():
+@pytest.mark.parametrize("scope", ["class", "baseline"])
+def test_adaptive_step_is_cuda_graph_capturable(scope):
     """kernel + device-side threshold update are pure stream work: a captured graph replayed chunk after chunk adapts
     exactly like eager calls (same thresholds, same flags) -- no host synchronisation inside rfi_process_chunk."""
     w = synth.Workload("adapt_graph", 8, True, 32, 512, 16, 128, channel_gain=True, burst_cell_frac=0.02)
@@ -215,21 +216,25 @@ def test_adaptive_step_is_cuda_graph_capturable():
         plan = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, 16, n_int=128)
         plan.set_thresholds(synth.default_thresholds(16))
         plan.set_adaptive(0.05, 0.5)
+        plan.set_adaptive_scope(scope)
         return plan, plan.alloc_outputs()
+
+    def thresholds(plan):
+        return plan.get_thresholds() if scope == "class" else plan.get_stream_thresholds().tolist()
 
     eager, (avg_e, wt_e, _) = make()
     ref = []
     for c in chunks:
         eager.process_chunk(c, avg_e, wt_e)
         torch.cuda.synchronize()
-        ref.append((eager.get_thresholds(), eager.get_flags().clone(), avg_e.clone()))
+        ref.append((thresholds(eager), eager.get_flags().clone(), avg_e.clone()))
     eager.destroy()
 
     plan, (avg, wt, _) = make()
     d_vis = chunks[0].clone()
     plan.process_chunk(d_vis, avg, wt)                        # warm-up call = chunk 0 (allocations, a-priori upload)
     torch.cuda.synchronize()
-    assert plan.get_thresholds() == ref[0][0]
+    assert thresholds(plan) == ref[0][0]
     side = torch.cuda.Stream()
     graph = torch.cuda.CUDAGraph()
     with torch.cuda.stream(side):
@@ -240,6 +245,6 @@ def test_adaptive_step_is_cuda_graph_capturable():
         torch.cuda.synchronize()
         graph.replay()
         torch.cuda.synchronize()
-        assert plan.get_thresholds() == ref[i][0]
+        assert thresholds(plan) == ref[i][0]
         assert torch.equal(plan.get_flags(), ref[i][1]) and torch.equal(avg, ref[i][2])
     plan.destroy()
