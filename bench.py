@@ -624,11 +624,26 @@ def run_ours(args):
                 plan.process_chunk_host_into(h_vis, h_avg, h_weight, h_flags)      # synchronises before returning
             dt = (time.perf_counter() - t0) / n_e2e
             same = bool(torch.equal(h_avg, avg.cpu()) and torch.equal(h_weight, weight.cpu()))
+            # what the link itself does: a plain pinned host-to-device copy of 2 GiB of the same buffer (not part of the step)
+            n_probe = min(h_vis.numel(), (2 << 30) // h_vis.element_size())
+            src, dst = h_vis.reshape(-1)[:n_probe], vis.reshape(-1)[:n_probe]
+            keep = dst.clone()
+            dst.copy_(src, non_blocking=True)
+            ea, eb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            ea.record()
+            for _ in range(3):
+                dst.copy_(src, non_blocking=True)
+            eb.record()
+            torch.cuda.synchronize(dev)
+            link_gbs = 3 * n_probe * h_vis.element_size() / (ea.elapsed_time(eb) * 1e-3) / 1e9
+            dst.copy_(keep)
+            del keep
             # N > 1: measured on rank 0 alone (pinning N x 18.5 GB of host memory is not safe on every box), so the
             # figure is ONE GPU's end-to-end rate and is not multiplied by N
             e2e = {"value": samples / dt, "unit": UNIT, "ranks_measured": 1, "h2d_bytes_per_step": w.input_bytes,
                    "d2h_bytes_per_step": out_bytes, "ms_per_step": dt * 1e3, "steps": n_e2e,
-                   "h2d_gbs": w.input_bytes / dt / 1e9, "matches_device_path": same,
+                   "h2d_gbs": w.input_bytes / dt / 1e9, "h2d_link_probe_gbs": link_gbs,
+                   "frac_of_h2d_link": (w.input_bytes / dt / 1e9) / link_gbs, "matches_device_path": same,
                    "api": "rfi_process_chunk_host (pinned host buffers; per-integration H2D overlapped with the kernel)"}
             del h_vis
         except Exception as exc:  # e.g. not enough pinnable host memory on the box
