@@ -194,8 +194,16 @@ enum { RFI_ADAPT_PER_CLASS = 0, RFI_ADAPT_PER_BASELINE = 1 };
 int rfi_plan_set_adaptive_scope(rfi_plan *plan, int scope);
 /* RFI_ADAPT_PER_BASELINE only: the thresholds in force for the next chunk, h_out[n_baselines] (of the shard), and the
  * running histograms, h_out[n_baselines][768 tau bins | 384 r bins] doubles.  Both wait for the device work issued so
- * far.  RFI_ESTATE before the first adaptive chunk or in the per-class scope. */
+ * far.  RFI_ESTATE before the first chunk processed in a per-stream mode. */
 int rfi_plan_get_stream_thresholds(rfi_plan *plan, rfi_thresholds *h_out);
+/* Thresholds given per baseline stream by the caller (the result of an off-line fine-tuning "for each data stream",
+ * PAPER.md:259): h_sets[n_baselines] (of the shard; copied; d > 0, no NaN), NULL switches the table off.  Without
+ * adaptation every window of baseline b is decided with h_sets[b] (the stats plane carries tau with its d); with
+ * RFI_ADAPT_PER_BASELINE the table is the a-priori state the streams start from (the per-class adaptation ignores it).
+ * Same restrictions as the adaptive
+ * mode (K = 1 set with rfi_set_thresholds, RFI_ARITH_FAST, time-major, direct kernel, n_chan % 32 == 0; RFI_EINVAL from
+ * rfi_process_chunk otherwise, RFI_ESTATE if the shard has changed since).  rfi_plan_get_stream_thresholds returns it. */
+int rfi_plan_set_stream_thresholds(rfi_plan *plan, const rfi_thresholds *h_sets);
 int rfi_plan_get_stream_histograms(rfi_plan *plan, double *h_out);
 
 /* The thresholds currently in force, one set per baseline class (h_out[n_classes], host memory): the adapted ones

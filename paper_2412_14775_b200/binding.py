@@ -26,7 +26,7 @@ EXPORTS = [
     "rfi_strerror", "rfi_last_cuda_error", "rfi_flags_bytes", "rfi_avg_bytes", "rfi_weight_bytes",
     "rfi_stats_bytes", "rfi_vis_bytes", "rfi_plan_launch_count", "rfi_plan_last_variant", "rfi_version",
     "rfi_probe_read_bandwidth", "rfi_probe_mix_bandwidth", "rfi_sim42_generate", "rfi_sim42_vis_bytes", "rfi_sim42_truth_bytes",
-    "rfi_rl_evaluate", "rfi_plan_set_adaptive", "rfi_plan_set_adaptive_scope", "rfi_plan_get_stream_thresholds",
+    "rfi_rl_evaluate", "rfi_plan_set_adaptive", "rfi_plan_set_adaptive_scope", "rfi_plan_set_stream_thresholds", "rfi_plan_get_stream_thresholds",
     "rfi_plan_get_stream_histograms", "rfi_plan_get_thresholds",
     "rfi_plan_get_adaptive_histogram",
 ]
@@ -102,6 +102,8 @@ def load_library(build_if_missing: bool = True):
     lib.rfi_plan_set_adaptive.restype = ci
     lib.rfi_plan_set_adaptive_scope.argtypes = [vp, ci]
     lib.rfi_plan_set_adaptive_scope.restype = ci
+    lib.rfi_plan_set_stream_thresholds.argtypes = [vp, ctypes.POINTER(RfiThresholds)]
+    lib.rfi_plan_set_stream_thresholds.restype = ci
     lib.rfi_plan_get_stream_thresholds.argtypes = [vp, ctypes.POINTER(RfiThresholds)]
     lib.rfi_plan_get_stream_thresholds.restype = ci
     lib.rfi_plan_get_stream_histograms.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
@@ -245,6 +247,17 @@ class RfiPlan:
         """rfi_plan_set_adaptive_scope: "class" (one threshold set per baseline class) or "baseline" (every baseline
         stream adapts its own thresholds: the paper's "fine-tuning for each data stream")."""
         _check(self._lib.rfi_plan_set_adaptive_scope(self._h, {"class": 0, "baseline": 1}[scope]), "rfi_plan_set_adaptive_scope")
+
+    def set_stream_thresholds(self, sets):
+        """rfi_plan_set_stream_thresholds: sets[b] = (d, s_low, s_high, gamma) for every baseline of the plan's shard
+        (None switches the table off).  K must be 1."""
+        if sets is None:
+            _check(self._lib.rfi_plan_set_stream_thresholds(self._h, None), "rfi_plan_set_stream_thresholds")
+            return
+        if len(sets) != self.n_baselines:
+            raise ValueError("one threshold set per baseline of the plan is needed")
+        arr = (RfiThresholds * self.n_baselines)(*[RfiThresholds(*map(float, t)) for t in sets])
+        _check(self._lib.rfi_plan_set_stream_thresholds(self._h, arr), "rfi_plan_set_stream_thresholds")
 
     def get_stream_thresholds(self):
         """rfi_plan_get_stream_thresholds: float64 array [n_baselines, 4] = (d, s_low, s_high, gamma) per baseline stream."""

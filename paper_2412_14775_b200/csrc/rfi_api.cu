@@ -84,7 +84,9 @@ struct rfi_plan {
     bool adapt_uploaded = false;               // d_thr holds the a-priori thresholds / the state was reset
     int adapt_scope = RFI_ADAPT_PER_CLASS;     // thresholds and histograms per class ([2]) or per baseline stream
     int adapt_cap = 0;                         // streams the adaptation buffers were allocated for
-    int adapt_streams() const { return adapt_scope == RFI_ADAPT_PER_BASELINE ? n_baselines : 2; }
+    std::vector<rfi_thresholds> stream_thr;    // rfi_plan_set_stream_thresholds: one set per baseline of the shard (empty: off)
+    bool per_stream() const { return adapt_scope == RFI_ADAPT_PER_BASELINE || (!stream_thr.empty() && adapt_alpha <= 0.0); }
+    int adapt_streams() const { return per_stream() ? n_baselines : 2; }
     // host path
     void* d_stage[2] = {nullptr, nullptr};
     size_t d_stage_cap[2] = {0, 0};
@@ -255,6 +257,7 @@ int enqueue_slab(rfi_plan* p, const void* d_vis_slab, int o_first, int n_out_sla
     kp.k_first = 0;
     kp.flags_atomic = (p->n_chan % 32 != 0 && 32 % p->n_chan != 0) ? 1 : 0;
     if (p->adapt_alpha > 0.0) { kp.d_thr = p->d_thr; kp.hist = p->d_hist; kp.adapt_streams = p->adapt_scope == RFI_ADAPT_PER_BASELINE; }
+    else if (!p->stream_thr.empty()) { kp.d_thr = p->d_thr; kp.adapt_streams = 2; }
     p->truth_fused = false;
 
     const bool fp16 = p->precision == RFI_FP16;
@@ -404,15 +407,21 @@ int prepare(rfi_plan* p, cudaStream_t st) {
     }
     const bool flags_atomic = (p->n_chan % 32 != 0 && 32 % p->n_chan != 0);
     if (flags_atomic) RFI_CUDA(cudaMemsetAsync(p->d_flags, 0, p->flags_words() * sizeof(uint32_t), st));
-    if (p->adapt_alpha > 0.0) {
+    const bool stream_table = !p->stream_thr.empty();
+    if (stream_table && (int)p->stream_thr.size() != p->n_baselines) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "rfi_plan_set_stream_thresholds was given %zu sets, the plan now processes %d baselines",
+                 p->stream_thr.size(), p->n_baselines);
+        return RFI_ESTATE;
+    }
+    if (p->adapt_alpha > 0.0 || stream_table) {
         if (p->K != 1 || p->arith != RFI_ARITH_FAST || p->layout != RFI_LAYOUT_TIME_MAJOR || p->variant == RFI_VARIANT_TMA ||
             p->variant == RFI_VARIANT_SPLIT) {
-            snprintf(g_cuda_err, sizeof(g_cuda_err), "adaptive thresholds need K = 1, RFI_ARITH_FAST, the time-major layout "
+            snprintf(g_cuda_err, sizeof(g_cuda_err), "adaptive and per-stream thresholds need K = 1, RFI_ARITH_FAST, the time-major layout "
                      "and the direct kernel (RFI_VARIANT_AUTO or RFI_VARIANT_DIRECT)");
             return RFI_EINVAL;
         }
-        if (p->adapt_scope == RFI_ADAPT_PER_BASELINE && p->n_chan % 32 != 0) {
-            snprintf(g_cuda_err, sizeof(g_cuda_err), "adaptation per baseline stream needs n_chan %% 32 == 0 (a 32-cell tile must lie in one baseline)");
+        if (p->per_stream() && p->n_chan % 32 != 0) {
+            snprintf(g_cuda_err, sizeof(g_cuda_err), "thresholds / adaptation per baseline stream need n_chan %% 32 == 0 (a 32-cell tile must lie in one baseline)");
             return RFI_EINVAL;
         }
         const int ns = p->adapt_streams();
@@ -436,9 +445,11 @@ int prepare(rfi_plan* p, cudaStream_t st) {
             p->adapt_stage_raw.resize(ns);
             for (int i = 0; i < ns; ++i) {
                 int cls = i == 0 ? 0 : nc - 1;                // per class: [0] = class 0, [1] = class 1 (or 0 again)
-                if (p->adapt_scope == RFI_ADAPT_PER_BASELINE) cls = nc > 1 ? (int)p->h_cls[p->b_first + i] : 0;
-                p->adapt_stage_thr[i] = to_device_thr(p->thr[cls], p->M * p->F);
-                p->adapt_stage_raw[i] = p->thr[cls];
+                if (p->per_stream()) cls = nc > 1 ? (int)p->h_cls[p->b_first + i] : 0;
+                // a stream table given by the caller is the a-priori state of its streams (and all there is without adaptation)
+                const rfi_thresholds& src = (stream_table && p->per_stream()) ? p->stream_thr[i] : p->thr[cls];
+                p->adapt_stage_thr[i] = to_device_thr(src, p->M * p->F);
+                p->adapt_stage_raw[i] = src;
             }
             RFI_CUDA(cudaMemcpyAsync(p->d_thr, p->adapt_stage_thr.data(), ns * sizeof(rfi::Thr), cudaMemcpyHostToDevice, st));
             RFI_CUDA(cudaMemcpyAsync(p->d_thr_raw, p->adapt_stage_raw.data(), ns * sizeof(rfi_thresholds), cudaMemcpyHostToDevice, st));
@@ -452,7 +463,7 @@ int prepare(rfi_plan* p, cudaStream_t st) {
 
 // After the chunk's kernels: fold the chunk's histograms into the running ones and set the next chunk's thresholds.
 int finish_adaptive(rfi_plan* p, cudaStream_t st) {
-    if (p->adapt_alpha <= 0.0) return RFI_OK;
+    if (p->adapt_alpha <= 0.0) return RFI_OK;                 // (static per-stream thresholds: nothing to update)
     const int rc = launch_adapt_update(p->d_hist, p->d_hist_acc, p->d_thr, p->d_thr_raw,
                                        p->adapt_scope == RFI_ADAPT_PER_BASELINE ? p->n_baselines : p->n_classes, p->adapt_alpha,
                                        p->adapt_forget, st);
@@ -582,6 +593,22 @@ int rfi_plan_set_adaptive(rfi_plan* p, float false_alarm, float forget) {
     return RFI_OK;
 }
 
+int rfi_plan_set_stream_thresholds(rfi_plan* p, const rfi_thresholds* h_sets) {
+    if (!p) return RFI_EINVAL;
+    if (h_sets) {
+        for (int b = 0; b < p->n_baselines; ++b) {
+            const rfi_thresholds& t = h_sets[b];
+            if (!(t.d > 0.f) || std::isinf(t.d) || std::isnan(t.s_low) || std::isnan(t.s_high) || std::isnan(t.gamma)) return RFI_EINVAL;
+        }
+        p->stream_thr.assign(h_sets, h_sets + p->n_baselines);
+    } else {
+        p->stream_thr.clear();
+    }
+    p->adapt_uploaded = false;
+    p->have_result = false;
+    return RFI_OK;
+}
+
 int rfi_plan_set_adaptive_scope(rfi_plan* p, int scope) {
     if (!p || (scope != RFI_ADAPT_PER_CLASS && scope != RFI_ADAPT_PER_BASELINE)) return RFI_EINVAL;
     p->adapt_scope = scope;
@@ -592,7 +619,7 @@ int rfi_plan_set_adaptive_scope(rfi_plan* p, int scope) {
 
 int rfi_plan_get_stream_thresholds(rfi_plan* p, rfi_thresholds* h_out) {
     if (!p || !h_out) return RFI_EINVAL;
-    if (p->adapt_scope != RFI_ADAPT_PER_BASELINE || p->adapt_alpha <= 0.0 || !p->d_thr_raw || !p->adapt_uploaded) return RFI_ESTATE;
+    if (!p->per_stream() || !p->d_thr_raw || !p->adapt_uploaded) return RFI_ESTATE;
     RFI_CUDA(cudaMemcpy(h_out, p->d_thr_raw, (size_t)p->n_baselines * sizeof(rfi_thresholds), cudaMemcpyDeviceToHost));
     return RFI_OK;
 }

@@ -61,7 +61,8 @@ struct KParams {
     // (updated between chunks by a device kernel) and this chunk's histograms of tau and max(r_re, r_im); null otherwise
     const Thr* d_thr;
     uint32_t* hist;
-    int adapt_streams;        // 0: thresholds / histograms per baseline class ([2]); 1: per baseline stream ([n_baselines])
+    int adapt_streams;        // 0: thresholds / histograms per baseline class ([2]); 1: per baseline stream ([n_baselines]);
+                              // 2: per-stream thresholds given by the caller, no adaptation
     // in-kernel confusion counters (rfi_plan_set_truth; K-set kernel only): ground-truth mask laid out like one set of the
     // flag mask, and uint64 counts[K][4] = {false alarms, clean windows, missed detections, RFI windows}; null otherwise
     const uint32_t* truth;

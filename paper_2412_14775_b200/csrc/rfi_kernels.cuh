@@ -51,8 +51,9 @@ __device__ __forceinline__ void direct_unit(const KParams& p, const int unit, co
 
     Thr thr_dev;
     // ADAPT = 1: thresholds and histograms per baseline class; ADAPT = 2: per baseline STREAM (the tile lies in one baseline:
-    // n_chan % 32 == 0, checked by the host), histogram private to the warp and flushed at the end of the unit
-    const int stream = ADAPT == 2 ? (tile * 32) / p.n_chan : g.cls;
+    // n_chan % 32 == 0, checked by the host), histogram private to the warp and flushed at the end of the unit; ADAPT = 3:
+    // per-stream thresholds given by the caller, no histogram
+    const int stream = ADAPT >= 2 ? (tile * 32) / p.n_chan : g.cls;
     if constexpr (ADAPT != 0) thr_dev = p.d_thr[stream];
     Raw<FP16> A[R], B[R];
     auto window_end = [&]() {
@@ -140,6 +141,8 @@ __global__ void __launch_bounds__(128, (FP16 || R <= 4) ? 4 : (R == 5 ? 3 : 2)) 
             const uint32_t c = sh_hist[i];
             if (c) atomicAdd(p.hist + i, c);
         }
+    } else if constexpr (ADAPT == 3) {
+        if (unit < n_tiles * p.n_out_slab) direct_unit<R, FP16, ALIGN32, 3>(p, unit, n_tiles, nullptr);
     } else {
         __shared__ uint32_t sh_hist[4 * kAdaptBins];          // one [tau bins | r bins] histogram per warp (= per unit = one stream)
         uint32_t* mine = sh_hist + (threadIdx.x >> 5) * kAdaptBins;

@@ -12,7 +12,10 @@ int launch_r(const rfi::KParams& kp, cudaStream_t st) {
     const unsigned grid = (unsigned)((n_units + 3) / 4);
     // 256-bit loads need a 32-byte aligned sample: base % 32 == 0 (the sample stride is 32 B)
     const bool a32 = FP16 || (reinterpret_cast<uintptr_t>(kp.vis) % 32 == 0);
-    if (kp.d_thr && kp.adapt_streams) {                        // on-line adaptation per baseline stream
+    if (kp.d_thr && kp.adapt_streams == 2) {                   // static thresholds per baseline stream (rfi_plan_set_stream_thresholds)
+        if (a32) rfi::rfi_direct_kernel<R, FP16, true, 3><<<grid, 128, 0, st>>>(kp);
+        else     rfi::rfi_direct_kernel<R, FP16, false, 3><<<grid, 128, 0, st>>>(kp);
+    } else if (kp.d_thr && kp.adapt_streams) {                 // on-line adaptation per baseline stream
         if (a32) rfi::rfi_direct_kernel<R, FP16, true, 2><<<grid, 128, 0, st>>>(kp);
         else     rfi::rfi_direct_kernel<R, FP16, false, 2><<<grid, 128, 0, st>>>(kp);
     } else if (kp.d_thr) {                                     // on-line threshold adaptation per class (rfi_plan_set_adaptive)

@@ -223,8 +223,9 @@ __device__ __forceinline__ void store_output(const KParams& p, const LaneGeom& g
 
 // Single-set window tail shared by the streaming kernels: statistics, decision, flag word, statistics planes,
 // masked accumulation into the output integration.  ADAPT: the thresholds come from device memory
-// (`thr`: the lane's class, ADAPT = 1, or the lane's baseline stream, ADAPT = 2) and the window's tau and max(r_re, r_im)
-// are counted in a shared-memory histogram (the CTA's per-class pair, or the warp's own for its stream).
+// (`thr`: the lane's class, ADAPT = 1, or the lane's baseline stream, ADAPT = 2, 3) and, for ADAPT = 1, 2, the window's tau
+// and max(r_re, r_im) are counted in a shared-memory histogram (the CTA's per-class pair, or the warp's own for its stream).
+// ADAPT = 3: static per-stream thresholds (rfi_plan_set_stream_thresholds), nothing counted.
 template <int ADAPT = 0>
 __device__ __forceinline__ void finish_window(const KParams& p, const LaneGeom& g, Win& w, float inv_W,
                                               int w_global, f2 (&acc)[4], uint32_t& wt,
@@ -238,7 +239,7 @@ __device__ __forceinline__ void finish_window(const KParams& p, const LaneGeom& 
     const float tau = t.c * x;
     store_flags(p, g, p.k_first, w_global, flag);
     store_stats(p, g, w_global, tau, r_re, r_im);
-    if constexpr (ADAPT) {
+    if constexpr (ADAPT == 1 || ADAPT == 2) {
         if (g.valid && fabsf(tau) <= 3.402823466e38f && fabsf(r_max) <= 3.402823466e38f) {   // finite statistics only
             uint32_t* h = sh_hist + (ADAPT == 1 ? g.cls * kAdaptBins : 0);   // per class: the CTA's; per stream: the warp's own
             atomicAdd(h + adapt_bin(tau, kAdaptTauLoExp, kAdaptTauBins), 1u);

@@ -144,6 +144,56 @@ def test_per_baseline_adaptation_holds_the_rate_on_every_stream_and_rejects_ragg
     plan.destroy()
 
 
+@pytest.mark.parametrize("fp16,F", [(False, 1), (True, 1), (False, 2)])
+def test_static_thresholds_per_baseline_stream(fp16, F):
+    """rfi_plan_set_stream_thresholds: every baseline is decided with its own (d, s_low, s_high, gamma); per baseline the
+    statistics, flags and averages are the oracle's with that set.  The same table is the a-priori state of the per-baseline
+    adaptation, and a table of the wrong length (after a shard change) is refused."""
+    M = 16 if F == 1 else 10
+    w = synth.Workload("stream_thr", 7, True, 64, M * 32, M, M * 16, fp16=fp16, window_F=F, channel_gain=True, burst_cell_frac=0.05)
+    W = M * F
+    rng = np.random.default_rng(3)
+    base = synth.default_thresholds(W)[0]
+    sets = [[float(rng.uniform(0.5, 1.0)), base[1] * float(rng.uniform(0.6, 1.4)), base[2] * float(rng.uniform(0.7, 1.3)),
+             float(np.clip(base[3] * rng.uniform(0.8, 1.2), 0.05, 0.99))] for _ in range(w.n_baselines)]
+    sets[3] = [1.0, -math.inf, math.inf, math.inf]            # one stream with both detectors off
+    plan = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, M, rfi.RFI_FP16 if fp16 else rfi.RFI_FP32, n_int=w.n_int)
+    if F > 1:
+        plan.set_window_freq(F)
+    plan.set_thresholds([base])
+    plan.set_stream_thresholds(sets)
+    vis, _ = synth.make_chunk(w, seed=11)
+    out = _run(plan, w, vis)
+    assert plan.last_variant == "direct"
+    v = vis.numpy().reshape(w.n_time, w.n_cells, 4, 2)
+    for b in range(w.n_baselines):
+        sel = slice(b * w.n_chan, (b + 1) * w.n_chan)
+        sub = {k: (a[:, :, sel] if a.ndim >= 3 else a[:, sel]) for k, a in out.items()}
+        compare(v[:, sel], M, w.n_int, [sets[b]], sub, tol=2e-3 if fp16 else 1e-5, fp16=fp16, F=F)
+    assert out["flags"][0][:, 3 * w.n_chan:4 * w.n_chan].sum() == 0
+    got = plan.get_stream_thresholds()
+    assert np.allclose(got, np.asarray(sets, np.float32).astype(np.float64), rtol=0, atol=0, equal_nan=True)
+    # the table as the a-priori state of the per-baseline adaptation: chunk 1 is decided with it
+    plan.set_adaptive(0.05, 0.0)
+    plan.set_adaptive_scope("baseline")
+    out2 = _run(plan, w, vis)
+    for key in ("flags", "weight", "avg", "tau"):
+        np.testing.assert_array_equal(out2[key], out[key])
+    assert not np.allclose(plan.get_stream_thresholds()[:, 1:], got[:, 1:])      # ... and the streams have moved on
+    plan.set_adaptive(0.0, 0.0)
+    # switched off: one set for all again
+    plan.set_stream_thresholds(None)
+    out3 = _run(plan, w, vis)
+    compare(v, M, w.n_int, [base], out3, tol=2e-3 if fp16 else 1e-5, fp16=fp16, F=F)
+    # a table for 28 baselines does not fit a shard of 10
+    plan.set_stream_thresholds(sets)
+    plan.set_baseline_shard(0, 10)
+    avg, weight, _ = plan.alloc_outputs()
+    with pytest.raises(rfi.RfiError):
+        plan.process_chunk(vis[:, :10].contiguous().cuda(), avg, weight)
+    plan.destroy()
+
+
 def test_false_alarm_rate_is_held_on_clean_noise_for_cross_and_auto_streams():
     """Done-criterion of VERDICT r01 item 9: measured FA on RFI-free synthetic noise within +-0.5 % (absolute) of the
     request, separately for the cross- and the auto-correlations, from deliberately wrong a-priori thresholds."""
