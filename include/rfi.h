@@ -289,6 +289,12 @@ int rfi_plan_destroy(rfi_plan *plan);
 #define RFI_RL_RECORD_DOUBLES 52
 int rfi_rl_evaluate(const float *d_windows, int64_t n_windows, int W, uint32_t mask14,
                     const rfi_thresholds *h_thr, double reward_per_match, double *d_out, void *cuda_stream);
+/* The same with one precision mask PER WINDOW: d_masks[n_windows] uint16_t on the device (bits 0-13; higher bits are
+ * ignored) -- a batch of (state, action) pairs, as a vectorised environment or a replay batch of the agent produces
+ * them (the action selects the precision of every group).  Record n equals what rfi_rl_evaluate
+ * gives for window n with mask d_masks[n].  RFI_EINVAL for a NULL / misaligned d_masks. */
+int rfi_rl_evaluate_masks(const float *d_windows, int64_t n_windows, int W, const uint16_t *d_masks,
+                          const rfi_thresholds *h_thr, double reward_per_match, double *d_out, void *cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------------------------
  * Section-4.2 simulator: seeded synthetic blocks with injected RFI at a set

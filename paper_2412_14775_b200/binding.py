@@ -26,7 +26,7 @@ EXPORTS = [
     "rfi_strerror", "rfi_last_cuda_error", "rfi_flags_bytes", "rfi_avg_bytes", "rfi_weight_bytes",
     "rfi_stats_bytes", "rfi_vis_bytes", "rfi_plan_launch_count", "rfi_plan_last_variant", "rfi_version",
     "rfi_probe_read_bandwidth", "rfi_probe_mix_bandwidth", "rfi_sim42_generate", "rfi_sim42_vis_bytes", "rfi_sim42_truth_bytes",
-    "rfi_rl_evaluate", "rfi_plan_set_adaptive", "rfi_plan_set_adaptive_scope", "rfi_plan_set_stream_thresholds", "rfi_plan_get_stream_thresholds",
+    "rfi_rl_evaluate", "rfi_rl_evaluate_masks", "rfi_plan_set_adaptive", "rfi_plan_set_adaptive_scope", "rfi_plan_set_stream_thresholds", "rfi_plan_get_stream_thresholds",
     "rfi_plan_get_stream_histograms", "rfi_plan_get_thresholds",
     "rfi_plan_get_adaptive_histogram",
 ]
@@ -125,6 +125,8 @@ def load_library(build_if_missing: bool = True):
     lib.rfi_probe_mix_bandwidth.argtypes = [vp, sz, vp, sz, ci, ci, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(sz), vp]
     lib.rfi_probe_mix_bandwidth.restype = ci
     lib.rfi_rl_evaluate.argtypes = [vp, ctypes.c_int64, ci, ctypes.c_uint32, ctypes.POINTER(RfiThresholds), ctypes.c_double, vp, vp]
+    lib.rfi_rl_evaluate_masks.argtypes = [vp, ctypes.c_int64, ci, vp, ctypes.POINTER(RfiThresholds), ctypes.c_double, vp, vp]
+    lib.rfi_rl_evaluate_masks.restype = ci
     lib.rfi_rl_evaluate.restype = ci
     lib.rfi_sim42_generate.argtypes = [ctypes.POINTER(Sim42Config), vp, vp, vp, vp, vp]
     lib.rfi_sim42_generate.restype = ci
@@ -401,7 +403,8 @@ RL_FIELDS = {"features": slice(0, 10), "bits": slice(10, 24), "errors": slice(24
 
 def rl_evaluate(windows: torch.Tensor, mask14: int, threshold, reward_per_match: float = 3.0,
                 out: Optional[torch.Tensor] = None) -> torch.Tensor:
-    """rfi_rl_evaluate: the RL environment of PAPER.md:149-172 for a batch of windows and one precision mask.
+    """rfi_rl_evaluate: the RL environment of PAPER.md:149-172 for a batch of windows and one precision mask -- or, with
+    mask14 a CUDA int16 tensor [n], one mask per window (rfi_rl_evaluate_masks: a batch of (state, action) pairs).
     windows: contiguous CUDA float32 [n, W, 4, 2]; returns float64 [n, 52] (layout RL_FIELDS / include/rfi.h)."""
     if not (windows.is_cuda and windows.is_contiguous() and windows.dtype == torch.float32 and windows.dim() == 4
             and tuple(windows.shape[2:]) == (4, 2)):
@@ -409,6 +412,15 @@ def rl_evaluate(windows: torch.Tensor, mask14: int, threshold, reward_per_match:
     n, W = windows.shape[0], windows.shape[1]
     rec = out if out is not None else torch.empty(n, RL_RECORD_DOUBLES, dtype=torch.float64, device=windows.device)
     thr = RfiThresholds(*map(float, threshold))
+    if isinstance(mask14, torch.Tensor):
+        if not (mask14.is_cuda and mask14.is_contiguous() and mask14.dtype == torch.int16 and mask14.numel() == n):
+            raise ValueError("per-window masks must be a contiguous CUDA int16 tensor [n]")
+        with torch.cuda.device(windows.device):
+            _check(load_library().rfi_rl_evaluate_masks(windows.data_ptr(), n, W, mask14.data_ptr(), ctypes.byref(thr),
+                                                        float(reward_per_match), rec.data_ptr(),
+                                                        torch.cuda.current_stream(windows.device).cuda_stream),
+                   "rfi_rl_evaluate_masks")
+        return rec
     with torch.cuda.device(windows.device):
         _check(load_library().rfi_rl_evaluate(windows.data_ptr(), n, W, int(mask14), ctypes.byref(thr), float(reward_per_match),
                                               rec.data_ptr(), torch.cuda.current_stream(windows.device).cuda_stream),

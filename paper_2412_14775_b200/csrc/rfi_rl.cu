@@ -74,11 +74,13 @@ __device__ __forceinline__ void rl_cost(uint32_t mask, int W, double& op_cost, d
     conv = c1 + 2 * c2;
 }
 
-__global__ void __launch_bounds__(128) rfi_rl_kernel(const float* __restrict__ win, long long n_windows, int W, uint32_t mask,
+__global__ void __launch_bounds__(128) rfi_rl_kernel(const float* __restrict__ win, long long n_windows, int W, uint32_t mask_all,
+                                                     const uint16_t* __restrict__ masks,
                                                      float d, float s_low, float s_high, float gamma, double rho,
                                                      double* __restrict__ out) {
     const long long n = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (n >= n_windows) return;
+    const uint32_t mask = masks ? (uint32_t)masks[n] & 0x3FFFu : mask_all;      // one action per window, or one for the batch
     const float4* x = reinterpret_cast<const float4*>(win + n * W * 8);
     double* o = out + n * kRlRec;
     RlEvents ev{0.0, 0.0};
@@ -186,20 +188,35 @@ __global__ void __launch_bounds__(128) rfi_rl_kernel(const float* __restrict__ w
 
 }  // namespace rfi
 
-extern "C" int rfi_rl_evaluate(const float* d_windows, int64_t n_windows, int W, uint32_t mask14,
-                               const rfi_thresholds* h_thr, double reward_per_match, double* d_out, void* cuda_stream) {
+namespace {
+int rl_launch(const float* d_windows, int64_t n_windows, int W, uint32_t mask14, const uint16_t* d_masks,
+              const rfi_thresholds* h_thr, double reward_per_match, double* d_out, void* cuda_stream, const char* who) {
     using namespace rfi_host;
     g_cuda_err[0] = 0;
     if (!d_windows || !d_out || !h_thr || n_windows < 0 || W < 2 || (mask14 >> 14) != 0 ||
-        reinterpret_cast<uintptr_t>(d_windows) % 16 || reinterpret_cast<uintptr_t>(d_out) % 8) {
-        snprintf(g_cuda_err, sizeof(g_cuda_err), "rfi_rl_evaluate: NULL / misaligned pointer, W < 2 or mask bits above 13");
+        reinterpret_cast<uintptr_t>(d_windows) % 16 || reinterpret_cast<uintptr_t>(d_out) % 8 ||
+        reinterpret_cast<uintptr_t>(d_masks) % 2) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: NULL / misaligned pointer, W < 2 or mask bits above 13", who);
         return RFI_EINVAL;
     }
     if (!(h_thr->d > 0.f)) return RFI_EINVAL;
     if (n_windows == 0) return RFI_OK;
     const unsigned grid = (unsigned)((n_windows + 127) / 128);
     rfi::rfi_rl_kernel<<<grid, 128, 0, static_cast<cudaStream_t>(cuda_stream)>>>(
-        d_windows, (long long)n_windows, W, mask14, h_thr->d, h_thr->s_low, h_thr->s_high, h_thr->gamma, reward_per_match, d_out);
+        d_windows, (long long)n_windows, W, mask14, d_masks, h_thr->d, h_thr->s_low, h_thr->s_high, h_thr->gamma,
+        reward_per_match, d_out);
     RFI_CUDA(cudaGetLastError());
     return RFI_OK;
+}
+}  // namespace
+
+extern "C" int rfi_rl_evaluate(const float* d_windows, int64_t n_windows, int W, uint32_t mask14,
+                               const rfi_thresholds* h_thr, double reward_per_match, double* d_out, void* cuda_stream) {
+    return rl_launch(d_windows, n_windows, W, mask14, nullptr, h_thr, reward_per_match, d_out, cuda_stream, "rfi_rl_evaluate");
+}
+
+extern "C" int rfi_rl_evaluate_masks(const float* d_windows, int64_t n_windows, int W, const uint16_t* d_masks,
+                                     const rfi_thresholds* h_thr, double reward_per_match, double* d_out, void* cuda_stream) {
+    if (!d_masks) return RFI_EINVAL;
+    return rl_launch(d_windows, n_windows, W, 0u, d_masks, h_thr, reward_per_match, d_out, cuda_stream, "rfi_rl_evaluate_masks");
 }

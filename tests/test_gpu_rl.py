@@ -69,6 +69,32 @@ def test_rl_large_batch_and_random_masks():
     assert quiet.any() and (rec[quiet, F["matches"]] == 3).mean() > 0.9
 
 
+def test_rl_one_mask_per_window_is_the_batch_of_single_mask_runs():
+    """rfi_rl_evaluate_masks: a batch of (state, action) pairs.  Record n must be what the one-mask call -- and hence the
+    oracle -- gives for window n with mask[n]; the records of 2000 windows with 12 different masks are compared field by
+    field with the oracle run mask by mask, and bit for bit with the one-mask GPU call."""
+    w = synth.rl_windows(2000, 10, 2, seed=17)
+    rng = np.random.default_rng(6)
+    pool = np.array([0, 0x3C50, 0x3FFF] + rng.integers(0, 1 << 14, 9).tolist(), dtype=np.int16)
+    masks = pool[rng.integers(0, pool.size, w.shape[0])]
+    thr = (1.0, 0.3, 2.2, 0.55)
+    got = rfi.rl_evaluate(w.cuda(), torch.from_numpy(masks).cuda(), thr, 3.0).cpu().numpy()
+    for m in pool.tolist():
+        sel = masks == m
+        ref = orc.rl_evaluate(w.numpy()[sel], int(m), thr, 3.0)
+        one = rfi.rl_evaluate(w[torch.from_numpy(sel)].contiguous().cuda(), int(m), thr, 3.0).cpu().numpy()
+        g = got[sel]
+        assert np.array_equal(g.view(np.uint64), one.view(np.uint64)), f"mask {m:#06x}: differs from the one-mask launch"
+        for key in ("bits", "op_cost", "conversions", "overflow", "underflow", "matches", "flags"):
+            assert (g[:, F[key]] == ref[:, F[key]]).all(), f"{key} differs (mask {m:#06x})"
+        fin = np.isfinite(ref[:, F["errors"]])
+        assert (np.isfinite(g[:, F["errors"]]) == fin).all()
+        assert np.allclose(g[:, F["errors"]][fin], ref[:, F["errors"]][fin], rtol=1e-12, atol=0)
+        assert np.allclose(g[:, F["reward"]], ref[:, F["reward"]], rtol=1e-12)
+    with pytest.raises(ValueError):
+        rfi.rl_evaluate(w.cuda(), torch.from_numpy(masks[:5]).cuda(), thr)
+
+
 def test_rl_argument_validation():
     w = synth.rl_windows(4, 10, 2).cuda()
     with pytest.raises(rfi.RfiError):
