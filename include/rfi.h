@@ -246,7 +246,7 @@ int rfi_confusion_counts(rfi_plan *plan, const uint32_t *d_truth, uint64_t *d_co
  * launch -- the thread that packs a (set, window) flag word compares it with the truth word, so a tuning loop
  * (false-alarm / missed-detection probabilities per candidate threshold set) needs no second pass over
  * the K masks; the other kernels are followed by the mask pass of rfi_confusion_counts on the same stream.  Same
- * exact integers either way.  rfi_process_chunk_host does not count.  Call it after rfi_set_thresholds: d_counts is sized
+ * exact integers either way (rfi_process_chunk_host: the mask pass after its last slab, before it returns).  Call it after rfi_set_thresholds: d_counts is sized
  * for the K of that moment, and rfi_process_chunk returns RFI_ESTATE if K has changed since.  RFI_EINVAL if exactly one
  * pointer is NULL or a pointer is misaligned (4 / 8 bytes). */
 int rfi_plan_set_truth(rfi_plan *plan, const uint32_t *d_truth, uint64_t *d_counts);

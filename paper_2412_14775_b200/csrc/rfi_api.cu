@@ -763,6 +763,17 @@ int rfi_process_chunk_host(rfi_plan* p, const void* h_vis, void* h_avg, void* h_
         }
         const int rc3 = finish_adaptive(p, comp_st);
         if (rc3 != RFI_OK) return rc3;
+        if (p->d_truth) {                                      // rfi_plan_set_truth: the mask pass over the completed flags
+            if (p->truth_K != p->K) {
+                snprintf(g_cuda_err, sizeof(g_cuda_err), "rfi_plan_set_truth was called with K = %d threshold sets, the plan now has %d",
+                         p->truth_K, p->K);
+                return RFI_ESTATE;
+            }
+            const int rc4 = launch_confusion(p->d_flags, p->d_truth, p->d_counts, p->K,
+                                             (size_t)p->n_win() * p->n_baselines * p->wpb(), p->wpb(), p->n_chan, p->sm_count, comp_st);
+            if (rc4 != RFI_OK) return rc4;
+            p->launches++;
+        }
         RFI_CUDA(cudaMemcpyAsync(h_avg, p->d_avg, rfi_avg_bytes(p), cudaMemcpyDeviceToHost, comp_st));
         RFI_CUDA(cudaMemcpyAsync(h_weight, p->d_weight, rfi_weight_bytes(p), cudaMemcpyDeviceToHost, comp_st));
         RFI_CUDA(cudaMemcpyAsync(h_flags, p->d_flags, rfi_flags_bytes(p), cudaMemcpyDeviceToHost, comp_st));

@@ -510,6 +510,14 @@ def test_in_kernel_confusion_counters_equal_the_mask_pass(monkeypatch, n_chan, K
     separate = plan.confusion_counts(tw).cpu().numpy()
     plan.destroy()
     np.testing.assert_array_equal(fused, separate)
+    if layout == "time_major" and K in (1, 40):            # the host path fills the same counters
+        plan3 = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M,
+                            rfi.RFI_FP16 if fp16 else rfi.RFI_FP32, n_int=w.n_int)
+        plan3.set_thresholds(thr)
+        c3 = plan3.set_truth(tw)
+        plan3.process_chunk_host(vis.pin_memory())
+        np.testing.assert_array_equal(c3.cpu().numpy(), separate)
+        plan3.destroy()
     if K == 5:                                             # the counter buffer was sized for K sets: a new K needs a new one
         plan2 = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M, n_int=w.n_int)
         plan2.set_thresholds(thr)
