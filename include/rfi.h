@@ -352,6 +352,34 @@ int rfi_sim42_generate(const rfi_sim42_config *cfg, void *d_vis, uint32_t *d_tru
 size_t rfi_sim42_vis_bytes(const rfi_sim42_config *cfg);      /* n_time * n_real * n_chan * 32 */
 size_t rfi_sim42_truth_bytes(const rfi_sim42_config *cfg);    /* (n_time/window_T) * n_real * ceil(n_chan/32) * 4 */
 
+/* rfi_sim42_generate for callers that cannot allocate device memory.  The generator needs two work arrays between its
+ * kernels (parameter table, source coherence).  rfi_sim42_generate either allocates them on every call (cudaMalloc +
+ * cudaFree, both of which serialise with all streams of the device) or takes them from the caller.  Neither suits code
+ * that lives inside another program's memory budget: a plug-in of a correlator / beam-former process that partitioned
+ * the whole GPU at start-up and passes only each call's input and output buffers, or a tuning loop generating fresh
+ * section-4.2 blocks beside live flagging streams that an allocation would stall.  This entry point keeps the work
+ * arrays in a fixed array inside the library image instead and calls no cudaMalloc, cudaFree or other allocating
+ * routine -- the caller passes only the configuration and the outputs:
+ *   d_vis, d_truth (nullable), cuda_stream: as for rfi_sim42_generate; same kernels, same draws, so the same output
+ *   (bit for bit where inr = 0; otherwise equal up to the summation order of the two power totals, which are
+ *   accumulated with floating-point atomics in either entry point).  Only enqueues work; does not synchronise.
+ * Limits: n_real <= RFI_SIM42_STATIC_MAX_REAL and n_real * n_chan <= RFI_SIM42_STATIC_MAX_CELLS (the paper's 400-run
+ *   sweep at 512 channels fits); larger requests are refused with RFI_EINVAL and a message in
+ *   rfi_last_cuda_error -- split the batch over calls (realisation r of a call with seed s depends on (s, r) only).
+ * Cost: the array (rfi_sim42_static_bytes(), about 4.8 MiB) occupies every GPU that loads the library until the
+ *   process exits, used or not.
+ * First call on a device: looks up the array's address on that device (the current device; one cudaGetSymbolAddress,
+ *   which may make the runtime load the module there).  Make that first call before any stream capture begins.
+ * Sharing: all calls on a device use the same array and find the previous call's contents in it.  Nothing needs
+ *   clearing by the caller -- the first kernel rewrites every table row it uses, accumulators included -- but two
+ *   calls that can overlap on the GPU (different streams without an ordering between them, or two host threads)
+ *   race on it and corrupt each other: order them, e.g. issue them on one stream.
+ * d_vis must be memory of the current device (RFI_EINVAL otherwise); the stream must belong to it too. */
+#define RFI_SIM42_STATIC_MAX_REAL 512
+#define RFI_SIM42_STATIC_MAX_CELLS 262144
+int rfi_sim42_generate_static(const rfi_sim42_config *cfg, void *d_vis, uint32_t *d_truth, void *cuda_stream);
+size_t rfi_sim42_static_bytes(void);                           /* size of the built-in work array, per GPU */
+
 /* Diagnostics (not part of the method): read-only streaming bandwidth of the current device.  Reads `bytes` (>= 32,
  * a multiple of 32 is used) of the 32-byte aligned device buffer d_buf once per launch with the 256-bit streaming
  * load of the direct kernel, `repeats` timed launches after two warm-up launches, CUDA events on the stream;

@@ -4,5 +4,5 @@
 seeded input generators.  There is no CPU implementation in this package.
 """
 from .binding import (RFI_FP16, RFI_FP32, RfiError, RfiPlan, load_library, library_path,  # noqa: F401
-                      pack_flags, probe_mix_bandwidth, probe_read_bandwidth, rl_evaluate, sim42_generate, unpack_flags)
+                      pack_flags, probe_mix_bandwidth, probe_read_bandwidth, rl_evaluate, sim42_generate, sim42_generate_static, unpack_flags)
 from . import synth  # noqa: F401

@@ -26,6 +26,7 @@ EXPORTS = [
     "rfi_strerror", "rfi_last_cuda_error", "rfi_flags_bytes", "rfi_avg_bytes", "rfi_weight_bytes",
     "rfi_stats_bytes", "rfi_vis_bytes", "rfi_plan_launch_count", "rfi_plan_last_variant", "rfi_version",
     "rfi_probe_read_bandwidth", "rfi_probe_mix_bandwidth", "rfi_sim42_generate", "rfi_sim42_vis_bytes", "rfi_sim42_truth_bytes",
+    "rfi_sim42_generate_static", "rfi_sim42_static_bytes",
     "rfi_rl_evaluate", "rfi_rl_evaluate_masks", "rfi_plan_set_adaptive", "rfi_plan_set_adaptive_scope", "rfi_plan_set_stream_thresholds", "rfi_plan_get_stream_thresholds",
     "rfi_plan_get_stream_histograms", "rfi_plan_get_thresholds",
     "rfi_plan_get_adaptive_histogram",
@@ -130,6 +131,10 @@ def load_library(build_if_missing: bool = True):
     lib.rfi_rl_evaluate.restype = ci
     lib.rfi_sim42_generate.argtypes = [ctypes.POINTER(Sim42Config), vp, vp, vp, vp, vp]
     lib.rfi_sim42_generate.restype = ci
+    lib.rfi_sim42_generate_static.argtypes = [ctypes.POINTER(Sim42Config), vp, vp, vp]
+    lib.rfi_sim42_generate_static.restype = ci
+    lib.rfi_sim42_static_bytes.argtypes = []
+    lib.rfi_sim42_static_bytes.restype = sz
     for name in ("rfi_sim42_vis_bytes", "rfi_sim42_truth_bytes"):
         getattr(lib, name).argtypes = [ctypes.POINTER(Sim42Config)]
         getattr(lib, name).restype = sz
@@ -456,6 +461,35 @@ def sim42_generate(n_real: int, inr: float, seed: int = 1, n_time: int = 2000, n
     n = ctypes.sizeof(Sim42Realisation)
     tab = [Sim42Realisation.from_buffer_copy(raw[i * n:(i + 1) * n]) for i in range(n_real)]
     return vis, truth, tab, src
+
+
+SIM42_STATIC_MAX_REAL = 512
+SIM42_STATIC_MAX_CELLS = 262144
+
+
+def sim42_generate_static(vis: torch.Tensor, truth: Optional[torch.Tensor], inr: float, seed: int = 1, n_sources: int = 200,
+                          n_broadband: int = 5, n_narrowband: int = 1, n_narrowdur: int = 1, polarized: bool = True,
+                          window_T: int = 10, window_F: int = 2) -> None:
+    """rfi_sim42_generate_static: the section-4.2 generator for callers that may not allocate device memory (a plug-in
+    inside a process that has handed the whole GPU to its own pool, a loop running beside live streams that a
+    cudaMalloc / cudaFree would stall).  Its work arrays sit in a fixed array inside librfi.so, so the call allocates
+    nothing -- and neither does this wrapper: the caller brings both outputs.
+      vis    [n_time, n_real, n_chan, 4, 2] float32, contiguous, CUDA: filled in place
+      truth  [n_time // window_T, n_real, ceil(n_chan / 32)] int32, contiguous, same device; or None
+    Limits: n_real <= SIM42_STATIC_MAX_REAL, n_real * n_chan <= SIM42_STATIC_MAX_CELLS (RfiError otherwise).  Calls on
+    one device share the array: keep them ordered on one stream.  Runs on vis's current stream; asynchronous."""
+    if not (vis.is_cuda and vis.is_contiguous() and vis.dtype == torch.float32 and vis.dim() == 5 and vis.shape[3:] == (4, 2)):
+        raise ValueError("vis must be a contiguous CUDA float32 tensor [n_time, n_real, n_chan, 4, 2]")
+    n_time, n_real, n_chan = int(vis.shape[0]), int(vis.shape[1]), int(vis.shape[2])
+    if truth is not None and not (truth.is_cuda and truth.device == vis.device and truth.is_contiguous() and truth.dtype == torch.int32
+                                  and window_T > 0 and tuple(truth.shape) == (n_time // window_T, n_real, (n_chan + 31) // 32)):
+        raise ValueError("truth must be a contiguous int32 tensor [n_time // window_T, n_real, ceil(n_chan / 32)] on vis's device")
+    lib = load_library()
+    cfg = Sim42Config(n_time, n_chan, n_real, n_sources, n_broadband, n_narrowband, n_narrowdur, 1 if polarized else 0,
+                      float(inr), window_T, window_F, seed)
+    with torch.cuda.device(vis.device):
+        _check(lib.rfi_sim42_generate_static(ctypes.byref(cfg), vis.data_ptr(), truth.data_ptr() if truth is not None else None,
+                                             torch.cuda.current_stream(vis.device).cuda_stream), "rfi_sim42_generate_static")
 
 
 def probe_read_bandwidth(buf: torch.Tensor, repeats: int = 10) -> float:

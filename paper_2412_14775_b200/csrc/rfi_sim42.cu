@@ -17,6 +17,7 @@
 #include "rfi_internal.h"
 
 #include <cmath>
+#include <mutex>
 
 namespace rfi {
 
@@ -384,6 +385,109 @@ int rfi_sim42_generate(const rfi_sim42_config* c, void* d_vis, uint32_t* d_truth
         if (rc == RFI_OK && e != cudaSuccess) { cuda_ok(e, "cudaStreamSynchronize"); rc = RFI_ECUDA; }
     }
     return rc;
+}
+
+}  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------
+// rfi_sim42_generate_static: the same generator for callers that have no way to obtain device work memory.
+//
+// Who that is: code that runs inside somebody else's memory budget.  A correlator or beam-former process typically
+// carves up the whole GPU at start-up (ring buffers for the ingest, a pool for everything else) and hands a plug-in
+// only the input and output buffers of each call; a tuning loop that wants fresh section-4.2 blocks next to the live
+// flagging streams must not call cudaMalloc / cudaFree either, because both serialise with every stream of the device
+// and would stall the ingest for the duration.  rfi_sim42_generate needs two work arrays between its kernels (the
+// parameter table and the source coherence) and either allocates them itself or takes them from the caller -- neither
+// works for such a caller.  Here they live in one array that is part of the library image: the driver places it in
+// device memory when the module is loaded on a GPU, so this entry point performs no allocation of any kind.
+//
+// The price: every GPU that loads librfi.so carries the array (kSim42StaticBytes, about 4.8 MiB) until the process
+// exits, sizes are capped (RFI_SIM42_STATIC_MAX_REAL realisations, RFI_SIM42_STATIC_MAX_CELLS realisation x channel
+// cells), and all calls on one device share the one array -- see the notes at the entry point.
+constexpr size_t kSim42StaticTabBytes =
+    (sizeof(rfi_sim42_realisation) * (size_t)RFI_SIM42_STATIC_MAX_REAL + 255) / 256 * 256;   // region 0: parameter table
+constexpr size_t kSim42StaticSrcBytes = sizeof(double2) * (size_t)RFI_SIM42_STATIC_MAX_CELLS;  // region 1: source coherence
+constexpr size_t kSim42StaticBytes = kSim42StaticTabBytes + kSim42StaticSrcBytes;
+static_assert(sizeof(rfi_sim42_realisation) % 8 == 0 && kSim42StaticTabBytes % 256 == 0, "regions keep their alignment");
+static_assert(kSim42StaticBytes <= (8u << 20), "the built-in work area is meant to stay small");
+
+// One instance per device.  In host code this name is only a handle for the runtime's symbol calls, never a device
+// address: the kernels get the pointer cudaGetSymbolAddress returns (sim42_static_scratch below).
+static __device__ __align__(256) unsigned char g_sim42_static_scratch[kSim42StaticBytes];
+
+namespace {
+
+constexpr int kSim42StaticMaxDevices = 64;
+std::mutex g_sim42_static_mu;
+unsigned char* g_sim42_static_addr[kSim42StaticMaxDevices] = {};   // device address of the array, per device ordinal
+
+// Device address of the work area on the CURRENT device; resolved once per device (the first call on a device makes
+// the runtime load this module there, which is why that call should not happen inside a stream capture).
+int sim42_static_scratch(int* dev_out, unsigned char** base_out) {
+    using namespace rfi_host;
+    int dev = -1;
+    RFI_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kSim42StaticMaxDevices) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "rfi_sim42_generate_static: device ordinal %d is outside 0..%d", dev,
+                 kSim42StaticMaxDevices - 1);
+        return RFI_EINVAL;
+    }
+    std::lock_guard<std::mutex> lock(g_sim42_static_mu);
+    if (!g_sim42_static_addr[dev]) {
+        void* p = nullptr;
+        RFI_CUDA(cudaGetSymbolAddress(&p, g_sim42_static_scratch));
+        if (!p || reinterpret_cast<uintptr_t>(p) % 256) {
+            snprintf(g_cuda_err, sizeof(g_cuda_err), "rfi_sim42_generate_static: the runtime returned an unusable address for the work area");
+            return RFI_ECUDA;
+        }
+        g_sim42_static_addr[dev] = static_cast<unsigned char*>(p);
+    }
+    *dev_out = dev;
+    *base_out = g_sim42_static_addr[dev];
+    return RFI_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t rfi_sim42_static_bytes(void) { return kSim42StaticBytes; }
+
+int rfi_sim42_generate_static(const rfi_sim42_config* c, void* d_vis, uint32_t* d_truth, void* cuda_stream) {
+    using namespace rfi_host;
+    g_cuda_err[0] = 0;
+    if (!c || !d_vis) return RFI_EINVAL;
+    // the cap first, with its own message; every other rule of the configuration is checked by rfi_sim42_generate
+    if (c->n_real >= 1 && c->n_chan >= 1 &&
+        (c->n_real > RFI_SIM42_STATIC_MAX_REAL || (size_t)c->n_real * (size_t)c->n_chan > (size_t)RFI_SIM42_STATIC_MAX_CELLS)) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err),
+                 "rfi_sim42_generate_static: n_real = %d, n_real * n_chan = %zu do not fit the built-in work area (at most %d "
+                 "realisations and %d realisation-channel cells per call); split the batch, or use rfi_sim42_generate with "
+                 "your own d_table / d_sources", c->n_real, (size_t)c->n_real * (size_t)c->n_chan,
+                 RFI_SIM42_STATIC_MAX_REAL, RFI_SIM42_STATIC_MAX_CELLS);
+        return RFI_EINVAL;
+    }
+    int dev = -1;
+    unsigned char* base = nullptr;
+    const int rc = sim42_static_scratch(&dev, &base);
+    if (rc != RFI_OK) return rc;
+    // the work area belongs to the current device: output buffers that live on another GPU would be written by
+    // kernels running here through peer access at best, and not at all otherwise
+    cudaPointerAttributes attr{};
+    if (cudaPointerGetAttributes(&attr, d_vis) == cudaSuccess) {
+        if (attr.type == cudaMemoryTypeDevice && attr.device != dev) {
+            snprintf(g_cuda_err, sizeof(g_cuda_err), "rfi_sim42_generate_static: d_vis lives on device %d, the current device is %d",
+                     attr.device, dev);
+            return RFI_EINVAL;
+        }
+    } else {
+        cudaGetLastError();
+    }
+    // With both work arrays given, rfi_sim42_generate only enqueues its kernels: no allocation, no synchronisation.
+    // Nothing in the area has to be cleared here -- kernel 1 rewrites every field of the table rows it uses, the three
+    // accumulators (p_cel, p_rfi, gain) to zero, and kernel 2 writes every source cell before kernel 3 reads it.
+    return rfi_sim42_generate(c, d_vis, d_truth, reinterpret_cast<rfi_sim42_realisation*>(base),
+                              reinterpret_cast<double*>(base + kSim42StaticTabBytes), cuda_stream);
 }
 
 }  // extern "C"
