@@ -79,7 +79,8 @@ enum {
     RFI_VARIANT_TABLES = 4,   /* reported when the arithmetic mode is RFI_ARITH_TABLES */
     RFI_VARIANT_SPLIT  = 5    /* small chunks, low latency: one CTA per (tile, integration), its rows split over up to
                                  16 warps so that the whole unit is in flight at once (windows are kept small
-                                 for latency).  K = 1, RFI_ARITH_FAST, time-major, n_int / block length <= 96.  The SK
+                                 for latency).  K = 1, RFI_ARITH_FAST, time-major, n_int / block length <= 96 -- a plan in
+                                 any other mode refuses the request (rfi_process_chunk: RFI_EINVAL with a message).  The SK
                                  statistic is bit-identical to the direct kernel; alignment statistics and averages are
                                  summed block-wise, i.e. equal to the other variants within the stated tolerances, not
                                  bit for bit.  Never chosen by RFI_VARIANT_AUTO. */
@@ -181,12 +182,28 @@ int rfi_set_thresholds(rfi_plan *plan, int K, const rfi_thresholds *h_sets);
  * returns RFI_EINVAL).  RFI_EINVAL unless 0 <= false_alarm < 0.5 and 0 <= forget < 1. */
 int rfi_plan_set_adaptive(rfi_plan *plan, float false_alarm, float forget);
 
+/* What the rule above costs under heavy RFI, and a bound on it (reading A8).  The histograms count every window with
+ * finite statistics, contaminated ones included, so the quantiles are those of the MIXTURE: from the second chunk on
+ * the detector flags about `false_alarm` of ALL windows of a stream.  While the RFI occupancy rho of the stream stays
+ * below false_alarm this is conservative (a few extra flags); once rho exceeds it, the thresholds sit inside the RFI
+ * distribution and at least (rho - flagged fraction) / rho of the RFI windows go unflagged.  On the paper's own
+ * section-4.2 scenario (five broadband footprints, two narrowband; window-level occupancy about 0.55) the oracle
+ * measures 0.73 missed detections after one update against 0.012 with the a-priori set (tests/test_adapt_oracle.py).
+ * rfi_plan_set_adaptive_limit bounds the drift: an update moves a threshold at most max_loosen * |its a-priori value|
+ * in the loosening direction (s_low down, s_high up, gamma up; a-priori = the set of rfi_set_thresholds or the
+ * stream's row of rfi_plan_set_stream_thresholds) and any distance in the tightening direction.  max_loosen = 0 never
+ * loosens; a negative value (the default) switches the bound off.  Applies from the next update on, in both scopes,
+ * without restarting the adaptation.  RFI_EINVAL for NaN. */
+int rfi_plan_set_adaptive_limit(rfi_plan *plan, float max_loosen);
+
 /* Scope of the adaptation.  RFI_ADAPT_PER_CLASS (default): one pair of histograms and one threshold set per baseline
  * class, as above.  RFI_ADAPT_PER_BASELINE: "fine-tuning for each data stream" (every baseline stream is
  * mitigated separately) -- every baseline of the plan (of its shard) keeps its own running histograms and
  * its own (s_low, s_high, gamma); it starts from the a-priori set of its class and follows its own null distribution
  * from the second chunk on (same rule, readings A1-A6 with "class" read as "baseline"; a baseline contributes
- * n_chan / F x windows counts per chunk, and keeps its thresholds while it has fewer than 1000).  The streaming kernel
+ * n_chan counts per window step -- with T x F footprints every footprint is counted once per channel it covers, F
+ * times, which leaves the quantiles unchanged but means the 1000-count gate is reached after 1000 / F independent
+ * windows -- and keeps its thresholds while it has fewer than 1000 counts).  The streaming kernel
  * counts into a histogram private to the warp -- a 32-cell tile lies in one baseline, hence n_chan % 32 == 0 is required
  * (RFI_EINVAL from rfi_process_chunk otherwise) -- and adds it to the baseline's device histogram at the end of each
  * (tile, integration) unit; the update kernel runs one CTA per two baselines.  Restarts the adaptation. */

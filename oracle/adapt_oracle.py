@@ -22,6 +22,14 @@ The paper names the problem and gives no algorithm: the hyper-parameters come fr
       RFI_ADAPT_PER_BASELINE, one per baseline ("fine-tuning for each data stream") -- the tests then call
       them baseline by baseline.
 
+  A8  (optional, off by default) loosening bound.  A1 histograms every finite window, contaminated ones included, so
+      the quantiles are those of the mixture: the detector flags about alpha of ALL windows, and when the RFI occupancy
+      rho of a stream exceeds alpha at least (rho - alpha) / rho of its RFI goes unflagged from the second chunk on.
+      The a-priori set is the operator's statement of the null and the adaptation is "fine-tuning"
+      (PAPER.md:259), so with a bound lam >= 0 an update may move a threshold at most lam * |a-priori value| in the
+      loosening direction -- s_low >= s_low0 - lam |s_low0|, s_high <= s_high0 + lam |s_high0|,
+      gamma <= gamma0 + lam |gamma0| -- and as far as it likes in the tightening direction.
+
 Plain numpy / fp64; shares no code with csrc/rfi_adapt.cu; only tests/ may import it.
 """
 from __future__ import annotations
@@ -81,13 +89,24 @@ def beta_of(alpha: float) -> float:
     return 1.0 - np.sqrt(1.0 - alpha)
 
 
-def update(acc_tau, acc_r, chunk_tau, chunk_r, alpha: float, forget: float, previous):
-    """A3, A5, A6 for one class.  acc_*: float64 running histograms (or None); chunk_*: this chunk's counts;
-    previous: (s_low, s_high, gamma).  Returns (acc_tau, acc_r, (s_low, s_high, gamma))."""
+def bound(new, prior, lam):
+    """A8: (s_low, s_high, gamma) limited to lam * |a-priori value| of loosening; lam None or negative: no bound."""
+    if lam is None or lam < 0:
+        return tuple(new)
+    s_low0, s_high0, gamma0 = (float(x) for x in prior)
+    return (max(new[0], s_low0 - lam * abs(s_low0)), min(new[1], s_high0 + lam * abs(s_high0)),
+            min(new[2], gamma0 + lam * abs(gamma0)))
+
+
+def update(acc_tau, acc_r, chunk_tau, chunk_r, alpha: float, forget: float, previous, prior=None, max_loosen=None):
+    """A3, A5, A6 (and A8 when max_loosen >= 0, against the a-priori set `prior`) for one class.  acc_*: float64 running
+    histograms (or None); chunk_*: this chunk's counts; previous: (s_low, s_high, gamma).
+    Returns (acc_tau, acc_r, (s_low, s_high, gamma))."""
     acc_tau = np.asarray(chunk_tau, np.float64) + (forget * acc_tau if acc_tau is not None else 0.0)
     acc_r = np.asarray(chunk_r, np.float64) + (forget * acc_r if acc_r is not None else 0.0)
     if acc_tau.sum() < N_MIN:
         return acc_tau, acc_r, tuple(previous)
     b = beta_of(alpha)
     et, er = bin_edges(TAU_LO_EXP, N_TAU), bin_edges(R_LO_EXP, N_R)
-    return acc_tau, acc_r, (quantile(acc_tau, et, b / 2), quantile(acc_tau, et, 1 - b / 2), quantile(acc_r, er, 1 - b))
+    new = (quantile(acc_tau, et, b / 2), quantile(acc_tau, et, 1 - b / 2), quantile(acc_r, er, 1 - b))
+    return acc_tau, acc_r, bound(new, prior, max_loosen)

@@ -27,7 +27,7 @@ EXPORTS = [
     "rfi_stats_bytes", "rfi_vis_bytes", "rfi_plan_launch_count", "rfi_plan_last_variant", "rfi_version",
     "rfi_probe_read_bandwidth", "rfi_probe_mix_bandwidth", "rfi_sim42_generate", "rfi_sim42_vis_bytes", "rfi_sim42_truth_bytes",
     "rfi_sim42_generate_static", "rfi_sim42_static_bytes",
-    "rfi_rl_evaluate", "rfi_rl_evaluate_masks", "rfi_plan_set_adaptive", "rfi_plan_set_adaptive_scope", "rfi_plan_set_stream_thresholds", "rfi_plan_get_stream_thresholds",
+    "rfi_rl_evaluate", "rfi_rl_evaluate_masks", "rfi_plan_set_adaptive", "rfi_plan_set_adaptive_limit", "rfi_plan_set_adaptive_scope", "rfi_plan_set_stream_thresholds", "rfi_plan_get_stream_thresholds",
     "rfi_plan_get_stream_histograms", "rfi_plan_get_thresholds",
     "rfi_plan_get_adaptive_histogram",
 ]
@@ -101,6 +101,8 @@ def load_library(build_if_missing: bool = True):
     lib.rfi_plan_set_variant.argtypes = [vp, ci]
     lib.rfi_plan_set_adaptive.argtypes = [vp, ctypes.c_float, ctypes.c_float]
     lib.rfi_plan_set_adaptive.restype = ci
+    lib.rfi_plan_set_adaptive_limit.argtypes = [vp, ctypes.c_float]
+    lib.rfi_plan_set_adaptive_limit.restype = ci
     lib.rfi_plan_set_adaptive_scope.argtypes = [vp, ci]
     lib.rfi_plan_set_adaptive_scope.restype = ci
     lib.rfi_plan_set_stream_thresholds.argtypes = [vp, ctypes.POINTER(RfiThresholds)]
@@ -249,6 +251,13 @@ class RfiPlan:
         """rfi_plan_set_adaptive: hold `false_alarm` on RFI-free data by tracking the null quantiles of both statistics
         per baseline class, chunk by chunk, on the device (0 switches it off)."""
         _check(self._lib.rfi_plan_set_adaptive(self._h, float(false_alarm), float(forget)), "rfi_plan_set_adaptive")
+
+    def set_adaptive_limit(self, max_loosen: Optional[float]):
+        """rfi_plan_set_adaptive_limit: an update may loosen a threshold by at most max_loosen * |a-priori value|
+        (None or a negative value: no bound).  Keeps the adaptation from drifting into the RFI when a stream's RFI
+        occupancy exceeds the requested false-alarm rate."""
+        _check(self._lib.rfi_plan_set_adaptive_limit(self._h, -1.0 if max_loosen is None else float(max_loosen)),
+               "rfi_plan_set_adaptive_limit")
 
     def set_adaptive_scope(self, scope: str):
         """rfi_plan_set_adaptive_scope: "class" (one threshold set per baseline class) or "baseline" (every baseline

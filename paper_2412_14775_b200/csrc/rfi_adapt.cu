@@ -7,7 +7,9 @@
 //
 // Readings A1-A6: constant false-alarm rate by rank -- s_low = Q_tau(beta/2),
 // s_high = Q_tau(1 - beta/2), gamma = Q_r(1 - beta), beta = 1 - sqrt(1 - alpha) (two OR-ed detectors);
-// a class with fewer than n_min counted windows keeps its thresholds.
+// a class with fewer than n_min counted windows keeps its thresholds.  Reading A8 (rfi_plan_set_adaptive_limit): with
+// a bound lam >= 0 a threshold moves at most lam * |its a-priori value| in the loosening direction, because the
+// histograms hold the contaminated windows too and their quantiles drift into the RFI once its occupancy exceeds alpha.
 #include "rfi_internal.h"
 
 namespace rfi {
@@ -55,7 +57,9 @@ __device__ double adapt_quantile_warp(const double* h, int n_bins, int lo_exp, d
 
 // hist: this chunk's counts [2][kAdaptBins] (zeroed here for the next chunk); acc: running histograms (double);
 // thr: the device thresholds the streaming kernel reads; raw: the same as (d, s_low, s_high, gamma) for inspection.
+// prior: the a-priori sets (never written); lam < 0: no loosening bound.
 __global__ void __launch_bounds__(256) rfi_adapt_update_kernel(uint32_t* hist, double* acc, Thr* thr, rfi_thresholds* raw,
+                                                               const rfi_thresholds* __restrict__ prior, double lam,
                                                                int n_classes, double beta, double forget, double n_min) {
     __shared__ double sh[2 * kAdaptBins];
     __shared__ double tot[4];
@@ -64,6 +68,7 @@ __global__ void __launch_bounds__(256) rfi_adapt_update_kernel(uint32_t* hist, d
     acc += (size_t)blockIdx.x * 2 * kAdaptBins;
     thr += blockIdx.x * 2;
     raw += blockIdx.x * 2;
+    prior += blockIdx.x * 2;
     n_classes = min(2, n_classes - 2 * (int)blockIdx.x);
     for (int i = threadIdx.x; i < n_classes * kAdaptBins; i += blockDim.x) {
         const double v = forget * acc[i] + (double)hist[i];   // A3
@@ -90,13 +95,19 @@ __global__ void __launch_bounds__(256) rfi_adapt_update_kernel(uint32_t* hist, d
         const double* ht = sh + cls * kAdaptBins;
         if (tot[2 * cls] >= n_min) {
             if (j == 0) {
-                const float s_low = (float)adapt_quantile_warp(ht, kAdaptTauBins, kAdaptTauLoExp, tot[2 * cls], 0.5 * beta);
+                double q = adapt_quantile_warp(ht, kAdaptTauBins, kAdaptTauLoExp, tot[2 * cls], 0.5 * beta);
+                if (lam >= 0.0) q = fmax(q, (double)prior[cls].s_low - lam * fabs((double)prior[cls].s_low));        // A8
+                const float s_low = (float)q;
                 if (lane == 0) { thr[cls].x_low = (float)((double)s_low / (double)thr[cls].c); raw[cls].s_low = s_low; }   // x = tau / c
             } else if (j == 1) {
-                const float s_high = (float)adapt_quantile_warp(ht, kAdaptTauBins, kAdaptTauLoExp, tot[2 * cls], 1.0 - 0.5 * beta);
+                double q = adapt_quantile_warp(ht, kAdaptTauBins, kAdaptTauLoExp, tot[2 * cls], 1.0 - 0.5 * beta);
+                if (lam >= 0.0) q = fmin(q, (double)prior[cls].s_high + lam * fabs((double)prior[cls].s_high));
+                const float s_high = (float)q;
                 if (lane == 0) { thr[cls].x_high = (float)((double)s_high / (double)thr[cls].c); raw[cls].s_high = s_high; }
             } else {
-                const float gamma = (float)adapt_quantile_warp(ht + kAdaptTauBins, kAdaptRBins, kAdaptRLoExp, tot[2 * cls + 1], 1.0 - beta);
+                double q = adapt_quantile_warp(ht + kAdaptTauBins, kAdaptRBins, kAdaptRLoExp, tot[2 * cls + 1], 1.0 - beta);
+                if (lam >= 0.0) q = fmin(q, (double)prior[cls].gamma + lam * fabs((double)prior[cls].gamma));
+                const float gamma = (float)q;
                 if (lane == 0) { thr[cls].gamma = gamma; raw[cls].gamma = gamma; }
             }
         }
@@ -107,10 +118,11 @@ __global__ void __launch_bounds__(256) rfi_adapt_update_kernel(uint32_t* hist, d
 
 namespace rfi_host {
 
-int launch_adapt_update(uint32_t* d_hist, double* d_acc, rfi::Thr* d_thr, rfi_thresholds* d_raw, int n_classes,
-                        double alpha, double forget, cudaStream_t st) {
+int launch_adapt_update(uint32_t* d_hist, double* d_acc, rfi::Thr* d_thr, rfi_thresholds* d_raw, const rfi_thresholds* d_prior,
+                        double max_loosen, int n_classes, double alpha, double forget, cudaStream_t st) {
     const double beta = 1.0 - sqrt(1.0 - alpha);
-    rfi::rfi_adapt_update_kernel<<<(unsigned)((n_classes + 1) / 2), 256, 0, st>>>(d_hist, d_acc, d_thr, d_raw, n_classes, beta, forget, 1000.0);
+    rfi::rfi_adapt_update_kernel<<<(unsigned)((n_classes + 1) / 2), 256, 0, st>>>(d_hist, d_acc, d_thr, d_raw, d_prior, max_loosen,
+                                                                                  n_classes, beta, forget, 1000.0);
     RFI_CUDA(cudaGetLastError());
     return RFI_OK;
 }

@@ -75,8 +75,10 @@ struct rfi_plan {
     std::vector<MapEntry> maps;
     // on-line threshold adaptation (rfi_plan_set_adaptive): device-resident thresholds, chunk and running histograms
     double adapt_alpha = 0.0, adapt_forget = 0.0;
+    double adapt_loosen = -1.0;                // rfi_plan_set_adaptive_limit: < 0 = no bound (reading A8)
+    int adapt_ns = 0;                          // streams of the state last uploaded (offset of the a-priori copy in d_thr_raw)
     rfi::Thr* d_thr = nullptr;                 // [2] thresholds the ADAPT kernel loads
-    rfi_thresholds* d_thr_raw = nullptr;       // [2] the same as (d, s_low, s_high, gamma)
+    rfi_thresholds* d_thr_raw = nullptr;       // [2] the same as (d, s_low, s_high, gamma), then [2] the a-priori sets (kept)
     uint32_t* d_hist = nullptr;                // [2][kAdaptBins] this chunk's counts
     double* d_hist_acc = nullptr;              // [2][kAdaptBins] running histograms
     std::vector<rfi::Thr> adapt_stage_thr;     // host staging of the a-priori thresholds (per class or per stream)
@@ -405,6 +407,12 @@ int prepare(rfi_plan* p, cudaStream_t st) {
         RFI_CUDA(cudaMemcpy(p->d_cls, p->h_cls.data(), p->h_cls.size(), cudaMemcpyHostToDevice));
         p->cls_uploaded = true;
     }
+    if (p->variant == RFI_VARIANT_SPLIT && (p->K != 1 || p->arith != RFI_ARITH_FAST || p->layout != RFI_LAYOUT_TIME_MAJOR)) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "RFI_VARIANT_SPLIT needs K = 1, RFI_ARITH_FAST and the time-major layout "
+                 "(the plan has K = %d%s%s); use RFI_VARIANT_AUTO", p->K, p->arith != RFI_ARITH_FAST ? ", tables arithmetic" : "",
+                 p->layout != RFI_LAYOUT_TIME_MAJOR ? ", cell-major layout" : "");
+        return RFI_EINVAL;
+    }
     const bool flags_atomic = (p->n_chan % 32 != 0 && 32 % p->n_chan != 0);
     if (flags_atomic) RFI_CUDA(cudaMemsetAsync(p->d_flags, 0, p->flags_words() * sizeof(uint32_t), st));
     const bool stream_table = !p->stream_thr.empty();
@@ -429,7 +437,7 @@ int prepare(rfi_plan* p, cudaStream_t st) {
         if (!p->d_thr || ns > p->adapt_cap) {
             cudaFree(p->d_thr); cudaFree(p->d_thr_raw); cudaFree(p->d_hist); cudaFree(p->d_hist_acc);
             p->d_thr = nullptr; p->d_thr_raw = nullptr; p->d_hist = nullptr; p->d_hist_acc = nullptr; p->adapt_cap = 0;
-            if (cudaMalloc(&p->d_thr, ns * sizeof(rfi::Thr)) != cudaSuccess || cudaMalloc(&p->d_thr_raw, ns * sizeof(rfi_thresholds)) != cudaSuccess ||
+            if (cudaMalloc(&p->d_thr, ns * sizeof(rfi::Thr)) != cudaSuccess || cudaMalloc(&p->d_thr_raw, 2 * ns * sizeof(rfi_thresholds)) != cudaSuccess ||
                 cudaMalloc(&p->d_hist, hb * sizeof(uint32_t)) != cudaSuccess || cudaMalloc(&p->d_hist_acc, hb * sizeof(double)) != cudaSuccess) {
                 cudaGetLastError();
                 return RFI_ENOMEM;
@@ -442,7 +450,7 @@ int prepare(rfi_plan* p, cudaStream_t st) {
             // staging vectors live in the plan, so the asynchronous copies may complete after this call returns.
             const int nc = p->n_classes;
             p->adapt_stage_thr.resize(ns);
-            p->adapt_stage_raw.resize(ns);
+            p->adapt_stage_raw.resize(2 * (size_t)ns);     // [ns] current (updated on the device), [ns] a priori (kept: A8)
             for (int i = 0; i < ns; ++i) {
                 int cls = i == 0 ? 0 : nc - 1;                // per class: [0] = class 0, [1] = class 1 (or 0 again)
                 if (p->per_stream()) cls = nc > 1 ? (int)p->h_cls[p->b_first + i] : 0;
@@ -450,9 +458,11 @@ int prepare(rfi_plan* p, cudaStream_t st) {
                 const rfi_thresholds& src = (stream_table && p->per_stream()) ? p->stream_thr[i] : p->thr[cls];
                 p->adapt_stage_thr[i] = to_device_thr(src, p->M * p->F);
                 p->adapt_stage_raw[i] = src;
+                p->adapt_stage_raw[ns + i] = src;
             }
+            p->adapt_ns = ns;
             RFI_CUDA(cudaMemcpyAsync(p->d_thr, p->adapt_stage_thr.data(), ns * sizeof(rfi::Thr), cudaMemcpyHostToDevice, st));
-            RFI_CUDA(cudaMemcpyAsync(p->d_thr_raw, p->adapt_stage_raw.data(), ns * sizeof(rfi_thresholds), cudaMemcpyHostToDevice, st));
+            RFI_CUDA(cudaMemcpyAsync(p->d_thr_raw, p->adapt_stage_raw.data(), 2 * ns * sizeof(rfi_thresholds), cudaMemcpyHostToDevice, st));
             RFI_CUDA(cudaMemsetAsync(p->d_hist, 0, hb * sizeof(uint32_t), st));
             RFI_CUDA(cudaMemsetAsync(p->d_hist_acc, 0, hb * sizeof(double), st));
             p->adapt_uploaded = true;
@@ -464,7 +474,7 @@ int prepare(rfi_plan* p, cudaStream_t st) {
 // After the chunk's kernels: fold the chunk's histograms into the running ones and set the next chunk's thresholds.
 int finish_adaptive(rfi_plan* p, cudaStream_t st) {
     if (p->adapt_alpha <= 0.0) return RFI_OK;                 // (static per-stream thresholds: nothing to update)
-    const int rc = launch_adapt_update(p->d_hist, p->d_hist_acc, p->d_thr, p->d_thr_raw,
+    const int rc = launch_adapt_update(p->d_hist, p->d_hist_acc, p->d_thr, p->d_thr_raw, p->d_thr_raw + p->adapt_ns, p->adapt_loosen,
                                        p->adapt_scope == RFI_ADAPT_PER_BASELINE ? p->n_baselines : p->n_classes, p->adapt_alpha,
                                        p->adapt_forget, st);
     if (rc == RFI_OK) p->launches++;
@@ -590,6 +600,12 @@ int rfi_plan_set_adaptive(rfi_plan* p, float false_alarm, float forget) {
     p->adapt_forget = forget;
     p->adapt_uploaded = false;
     p->have_result = false;
+    return RFI_OK;
+}
+
+int rfi_plan_set_adaptive_limit(rfi_plan* p, float max_loosen) {
+    if (!p || std::isnan(max_loosen)) return RFI_EINVAL;
+    p->adapt_loosen = max_loosen < 0.f ? -1.0 : (double)max_loosen;     // applies from the next update on; no restart
     return RFI_OK;
 }
 
@@ -745,6 +761,11 @@ int rfi_process_chunk_host(rfi_plan* p, const void* h_vis, void* h_avg, void* h_
     cudaStream_t copy_st = p->streams[0], comp_st = p->streams[1];
     rc = prepare(p, comp_st);
     if (rc != RFI_OK) return rc;
+    if (p->d_truth && p->truth_K != p->K) {                    // before any slab is enqueued: flags and adaptive state stay untouched
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "rfi_plan_set_truth was called with K = %d threshold sets, the plan now has %d: "
+                 "set the truth mask (and a counter buffer of K x 4) again", p->truth_K, p->K);
+        return RFI_ESTATE;
+    }
     const int n_out = p->n_out();
     const uint8_t* src = static_cast<const uint8_t*>(h_vis);
     // Every exit path below drains both internal streams first: no copy from (or to) the caller's host buffers is
@@ -764,11 +785,6 @@ int rfi_process_chunk_host(rfi_plan* p, const void* h_vis, void* h_avg, void* h_
         const int rc3 = finish_adaptive(p, comp_st);
         if (rc3 != RFI_OK) return rc3;
         if (p->d_truth) {                                      // rfi_plan_set_truth: the mask pass over the completed flags
-            if (p->truth_K != p->K) {
-                snprintf(g_cuda_err, sizeof(g_cuda_err), "rfi_plan_set_truth was called with K = %d threshold sets, the plan now has %d",
-                         p->truth_K, p->K);
-                return RFI_ESTATE;
-            }
             const int rc4 = launch_confusion(p->d_flags, p->d_truth, p->d_counts, p->K,
                                              (size_t)p->n_win() * p->n_baselines * p->wpb(), p->wpb(), p->n_chan, p->sm_count, comp_st);
             if (rc4 != RFI_OK) return rc4;

@@ -69,8 +69,8 @@ int launch_tables_ps(const rfi::KParams& kp, cudaStream_t st);          // R = 4
 
 int launch_batched_tma_cellmajor(bool fp16, const rfi::KParams& kp, const rfi::BatchThr& bt, const CUtensorMap* map,
                                  int sm_count, int smem_optin, cudaStream_t st);
-int launch_adapt_update(uint32_t* d_hist, double* d_acc, rfi::Thr* d_thr, rfi_thresholds* d_raw, int n_classes,
-                        double alpha, double forget, cudaStream_t st);
+int launch_adapt_update(uint32_t* d_hist, double* d_acc, rfi::Thr* d_thr, rfi_thresholds* d_raw, const rfi_thresholds* d_prior,
+                        double max_loosen, int n_classes, double alpha, double forget, cudaStream_t st);
 int launch_confusion(const uint32_t* d_flags, const uint32_t* d_truth, uint64_t* d_counts, int K, size_t n_words,
                      int wpb, int n_chan, int sm_count, cudaStream_t st);
 bool batched_tma_supported(bool fp16, const rfi::KParams& kp, int R);

@@ -9,9 +9,14 @@ template <int R, bool FP16>
 int launch_r(const rfi::KParams& kp, int smem_optin, cudaStream_t st) {
     const int nb = kp.n_int / R;
     const size_t smem = ((size_t)nb * rfi::kSplitPartFloats + (size_t)kp.wpo * rfi::kSplitRecFloats) * 32 * sizeof(float);
-    if (nb > rfi::kSplitMaxBlocks || (long)smem > smem_optin) {
+    if (nb > rfi::kSplitMaxBlocks) {
         snprintf(g_cuda_err, sizeof(g_cuda_err), "RFI_VARIANT_SPLIT is for small chunks: n_int / %d = %d blocks per unit exceed %d "
                  "(use RFI_VARIANT_AUTO)", R, nb, rfi::kSplitMaxBlocks);
+        return RFI_EINVAL;
+    }
+    if ((long)smem > smem_optin) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "RFI_VARIANT_SPLIT is for small chunks: %d blocks and %d windows per unit need %zu bytes of "
+                 "shared memory, the device offers %d (use RFI_VARIANT_AUTO)", nb, kp.wpo, smem, smem_optin);
         return RFI_EINVAL;
     }
     const int n_tiles = (kp.n_cells + 31) / 32;

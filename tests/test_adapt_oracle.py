@@ -77,3 +77,52 @@ def test_update_keeps_thresholds_below_n_min_and_forgets():
     tau2 = np.float32(np.linspace(2.0, 3.0, 5000)); r2 = np.float32(np.linspace(0.1, 0.9, 5000))
     a, b, thr = ao.update(a, b, *ao.histogram(tau2, r2), alpha=0.05, forget=0.0, previous=thr)
     assert a.sum() == 5000 and 2.0 <= thr[0] < thr[1] <= 3.0                    # forget = 0: the old chunk is gone
+
+
+def test_loosening_bound_closed_forms():
+    """A8: at most lam * |a-priori value| looser, any amount tighter, sign-safe, off by default."""
+    prior = (0.06, 0.52, 0.46)
+    assert ao.bound((0.01, 2.0, 0.99), prior, 0.25) == (0.06 - 0.25 * 0.06, 0.52 + 0.25 * 0.52, 0.46 + 0.25 * 0.46)
+    assert ao.bound((0.10, 0.40, 0.30), prior, 0.25) == (0.10, 0.40, 0.30)          # tighter than a priori: untouched
+    assert ao.bound((0.01, 2.0, 0.99), prior, 0.0) == prior                         # lam = 0: never looser than a priori
+    assert ao.bound((0.01, 2.0, 0.99), prior, None) == (0.01, 2.0, 0.99) == ao.bound((0.01, 2.0, 0.99), prior, -1.0)
+    assert ao.bound((-3.0, 2.0, 0.9), (-1.0, 1.0, 0.5), 0.5) == (-1.5, 1.5, 0.75)   # a negative s_low loosens downwards
+
+
+def _sim42_statistics(seed):
+    """A section-4.2 block (five broadband footprints, two narrowband, INR 100) through the fp64
+    oracle at the paper's 10 x 2 window: tau, max(r), window-level truth."""
+    from oracle import rfi_oracle as orc, sim42_oracle as so
+    cfg = so.Sim42Config(n_time=400, n_chan=64, n_real=4, n_sources=20, inr=100.0, seed=seed)
+    ref = so.generate(cfg)
+    res = orc.process(ref["vis"].reshape(cfg.n_time, cfg.n_real * cfg.n_chan, 4), 10, cfg.n_time, [[1.0, 0.0, 1e30, 1.0]], F=2)
+    return res.tau[0], np.fmax(res.r_re, res.r_im), ref["truth"].reshape(-1, cfg.n_real * cfg.n_chan)
+
+
+def _rates(tau, rmax, thr, truth):
+    flagged = ~((tau > thr[0]) & (tau < thr[1])) | (rmax > thr[2])                  # Eq.(5), Eq.(10), OR-ed (PAPER.md:105)
+    return (flagged & ~truth).sum() / (~truth).sum(), (~flagged & truth).sum() / truth.sum(), flagged.mean()
+
+
+def test_missed_detections_when_the_rfi_occupancy_exceeds_alpha():
+    """The price of A1 (every finite window is histogrammed) on the paper's own scenario, and what A8 buys back.
+    Occupancy rho > alpha: the unbounded rule flags about alpha-to-a-few-alpha of all windows, so it misses at least
+    (rho - flagged fraction) / rho of the RFI; with the loosening bound the thresholds stay at the a-priori ones'
+    side and the missed-detection rate stays near the a-priori one."""
+    from paper_2412_14775_b200 import synth
+    prior = tuple(synth.default_thresholds(20)[0][1:])
+    alpha = 0.05
+    tau_a, r_a, truth_a = _sim42_statistics(1)
+    tau_b, r_b, truth_b = _sim42_statistics(2)
+    rho = truth_b.mean()
+    assert truth_a.mean() > 4 * alpha and rho > 4 * alpha                           # far above alpha (about 0.55)
+    ht, hr = ao.histogram(tau_a, r_a)
+    free = ao.update(None, None, ht, hr, alpha, 0.0, prior)[2]
+    held = ao.update(None, None, ht, hr, alpha, 0.0, prior, prior=prior, max_loosen=0.25)[2]
+    assert free[0] < prior[0] and free[1] > 2 * prior[1] and free[2] > 1.5 * prior[2]   # the mixture's quantiles: far looser
+    assert held == ao.bound(free, prior, 0.25) == (0.75 * prior[0], 1.25 * prior[1], 1.25 * prior[2])
+    _, md_prior, _ = _rates(tau_b, r_b, prior, truth_b)
+    _, md_free, frac_free = _rates(tau_b, r_b, free, truth_b)
+    _, md_held, _ = _rates(tau_b, r_b, held, truth_b)
+    assert md_free >= (rho - frac_free) / rho - 1e-12                               # the bound of A8's note, exactly
+    assert md_free > 0.5 and md_prior < 0.05 and md_held < md_prior + 0.05

@@ -298,3 +298,62 @@ def test_adaptive_step_is_cuda_graph_capturable(scope):
         assert thresholds(plan) == ref[i][0]
         assert torch.equal(plan.get_flags(), ref[i][1]) and torch.equal(avg, ref[i][2])
     plan.destroy()
+
+
+def _sim42_chunk(seed, n_real=16, n_time=800, n_chan=64):
+    vis, truth = rfi.sim42_generate(n_real, 100.0, seed=seed, n_time=n_time, n_chan=n_chan, n_sources=20)
+    return vis, rfi.unpack_flags(truth, n_chan).cpu().numpy().reshape(-1, n_real * n_chan)
+
+
+def _md(flags, truth):
+    f = flags.reshape(truth.shape).astype(bool)
+    return (~f & truth).sum() / truth.sum(), f.mean()
+
+
+@pytest.mark.parametrize("scope", ["class", "baseline"])
+def test_loosening_bound_keeps_missed_detections_down_when_occupancy_exceeds_alpha(scope):
+    """Advisor finding (reading A8): on section-4.2 blocks (window-level RFI occupancy far above the
+    requested alpha = 0.05) the unbounded rule moves the thresholds into the RFI and misses most of it on chunk 2; with
+    rfi_plan_set_adaptive_limit(0.25) the thresholds in force are the oracle's bounded ones and the missed-detection rate
+    stays at the a-priori level.  Thresholds vs oracle/adapt_oracle.py from the kernel's own stored statistics."""
+    n_real, n_time, n_chan = 16, 800, 64
+    prior = synth.default_thresholds(20)[0]
+    vis1, truth1 = _sim42_chunk(11)
+    vis2, truth2 = _sim42_chunk(12)
+    rho = truth2.mean()
+    assert rho > 0.2
+    md = {}
+    for lam in (None, 0.25, "prior"):
+        plan = rfi.RfiPlan(5, 15, n_chan, n_time, 10, n_int=n_time)             # 15 baselines = 5 stations with autos
+        plan.set_window_freq(2)
+        plan.set_thresholds([prior])
+        if lam != "prior":
+            plan.set_adaptive(0.05, 0.0)
+            plan.set_adaptive_scope(scope)
+            plan.set_adaptive_limit(lam)
+        avg, weight, stats = plan.alloc_outputs(stats=True)
+        plan.process_chunk(vis1[:, :15].contiguous(), avg, weight, stats)
+        torch.cuda.synchronize()
+        out1 = gpu_outputs_to_numpy(plan, avg, weight, stats, rfi.unpack_flags(plan.get_flags(), n_chan))
+        if lam != "prior":                                                     # the thresholds for chunk 2 against the oracle
+            got = plan.get_thresholds()[0] if scope == "class" else None
+            streams = plan.get_stream_thresholds() if scope == "baseline" else None
+            for b in range(15 if scope == "baseline" else 1):
+                sel = slice(b * n_chan, (b + 1) * n_chan) if scope == "baseline" else slice(None)
+                tau = out1["tau"][:, sel]
+                rmax = np.fmax(out1["r_re"][:, sel], out1["r_im"][:, sel])
+                ht, hr = ao.histogram(tau, rmax)
+                want = ao.update(None, None, ht, hr, 0.05, 0.0, tuple(prior[1:]), prior=tuple(np.float32(prior[1:]).astype(np.float64)),
+                                 max_loosen=lam)[2]
+                have = got[1:] if scope == "class" else streams[b, 1:]
+                assert np.allclose(have, np.float32(want), rtol=1e-6, atol=0), (lam, b, have, want)
+        plan.process_chunk(vis2[:, :15].contiguous(), avg, weight, stats)
+        torch.cuda.synchronize()
+        flags2 = rfi.unpack_flags(plan.get_flags(), n_chan).cpu().numpy()
+        t2 = truth2.reshape(-1, n_real, n_chan)[:, :15].reshape(-1, 15 * n_chan)
+        md[lam] = _md(flags2, t2)
+        plan.destroy()
+    (md_free, frac_free), (md_held, _), (md_prior, _) = md[None], md[0.25], md["prior"]
+    rho15 = truth2.reshape(-1, n_real, n_chan)[:, :15].mean()
+    assert md_free >= (rho15 - frac_free) / rho15 - 1e-12 and md_free > 0.25    # the stated bound, and it bites
+    assert md_prior < 0.05 and md_held < md_prior + 0.05 and md_free > md_held + 0.2, (md_free, md_held, md_prior)

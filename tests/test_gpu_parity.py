@@ -799,3 +799,52 @@ def test_mix_probe_moves_the_bytes_it_reports():
                                      ctypes.byref(ms), ctypes.byref(moved), None)
     assert rc != 0
     assert rfi.probe_mix_bandwidth(buf, out.numel() * 4, repeats=2) > 0
+
+
+@pytest.mark.parametrize("what", ["K", "tables", "cell_major"])
+def test_split_variant_is_refused_where_it_cannot_run(what):
+    """RFI_VARIANT_SPLIT exists for K = 1, fast arithmetic, time-major input only: a plan in any other mode refuses
+    the request with a message instead of quietly running another kernel."""
+    w = synth.WORKLOADS["tiny"]
+    vis, _ = synth.make_chunk(w, seed=3)
+    plan = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M, n_int=w.n_int)
+    plan.set_thresholds(synth.sweep_thresholds(w.window_M, 3, seed=1) if what == "K" else synth.default_thresholds(w.window_M))
+    d_vis = vis.cuda()
+    if what == "tables":
+        plan.set_arithmetic("tables", 0x3C50)
+    if what == "cell_major":
+        plan.set_layout("cell_major")
+        d_vis = d_vis.permute(1, 2, 0, 3, 4).contiguous()
+    plan.set_variant("split")
+    avg, weight, _ = plan.alloc_outputs()
+    n0 = plan.launch_count
+    with pytest.raises(rfi.RfiError) as e:
+        plan.process_chunk(d_vis, avg, weight)
+    assert e.value.code == -1 and "RFI_VARIANT_SPLIT needs K = 1" in str(e.value)
+    assert plan.launch_count == n0
+    plan.set_variant("auto")                                   # the same plan runs once the request is withdrawn
+    plan.process_chunk(d_vis, avg, weight)
+    torch.cuda.synchronize()
+    plan.destroy()
+
+
+def test_host_path_refuses_a_changed_K_before_it_enqueues_anything():
+    """rfi_plan_set_truth sized the counters for K sets; with another K rfi_process_chunk_host returns RFI_ESTATE
+    up front: no kernel launched, the flags of the previous chunk still in place."""
+    w = synth.Workload("hostK", 6, True, 64, 256, 16, 128, burst_cell_frac=0.2)
+    vis, truth = synth.make_chunk(w, seed=8)
+    thr = synth.sweep_thresholds(16, 5, seed=2)
+    plan = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M, n_int=w.n_int)
+    plan.set_thresholds(thr)
+    tw = rfi.pack_flags(truth.reshape(plan.n_win, w.n_baselines, w.n_chan).cuda())
+    counts = plan.set_truth(tw)
+    h = vis.pin_memory()
+    plan.process_chunk_host(h)
+    before, n0 = counts.cpu().numpy().copy(), plan.launch_count
+    plan.set_thresholds(thr[:3])
+    with pytest.raises(rfi.RfiError) as e:
+        plan.process_chunk_host(h)
+    assert e.value.code == -4 and "rfi_plan_set_truth was called with K = 5" in str(e.value)
+    assert plan.launch_count == n0
+    np.testing.assert_array_equal(counts.cpu().numpy(), before)
+    plan.destroy()
