@@ -403,7 +403,7 @@ def run_sim42(args):
                    "input_bytes": vis.numel() * 4, "l2": "input (13.3 GB) is far larger than the 126 MB L2: no flush needed"},
         "roofline": {"bound": "hbm", "achieved": algo / (k_med * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
                      "frac": algo / (k_med * 1e-3) / 1e9 / peak, "traffic": None, "peak_source": peak_src,
-                     "kernel": "rfi_batched_tma_kernel", "kernel_ms_best": min(kernel_ms), "kernel_ms_median": k_med,
+                     "kernel": "rfi_batched_mask_kernel<5, fp32>", "kernel_ms_best": min(kernel_ms), "kernel_ms_median": k_med,
                      "frac_of_nominal_8TBs": algo / (k_med * 1e-3) / 1e9 / 8000.0, "algorithmic_bytes_per_launch": algo},
         "cpu_baseline": None, "e2e": None, "gpu_launches": int(plan.launch_count), "clocks": clocks,
         "sim42": {"generator_ms_median": statistics.median(gen_ms), "generator_gbytes_per_s": vis.numel() * 4 / (statistics.median(gen_ms) * 1e-3) / 1e9,

@@ -39,7 +39,8 @@
  *                                                                  unused high bits of a baseline's last word are 0
  *
  * Ownership: the caller owns vis/avg/weight/stats and the stream; the plan owns its device threshold table,
- * its flag buffer and (for the host path) its staging buffers.  vis is read exactly once and never written.
+ * its flag buffer and (for the host path) its staging buffers.  vis is never written and is read
+ * once per launch: exactly once for K <= 64 threshold sets, once per 64 sets beyond that (rfi_set_thresholds).
  * rfi_process_chunk enqueues work on the stream and returns without synchronising the host.
  *
  * Errors: every function returns RFI_OK (0) or a negative code; nothing throws or aborts.

@@ -39,7 +39,9 @@ def build(force: bool = False) -> str:
 def _load():
     global _lib
     if _lib is None:
-        lib = ctypes.CDLL(build())
+        # ORACLE_RFI_LIB: load a pre-built library instead (tests/test_oracle_sanitizers.py: the same sources built
+        # with -fsanitize=address,undefined)
+        lib = ctypes.CDLL(os.environ.get("ORACLE_RFI_LIB") or build())
         c_dp = ctypes.POINTER(ctypes.c_double)
         lib.oracle_rfi_stokes.argtypes = [c_dp, c_dp]
         lib.oracle_rfi_stokes.restype = None

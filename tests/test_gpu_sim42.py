@@ -142,3 +142,17 @@ def test_fig2_shaped_scenario_detector_ordering():
     assert md[1] < 0.5 * md[0]                                    # polarisation beats energy on polarised RFI
     assert md[2] <= md[1] + 1e-12                                 # OR-combination can only remove missed detections
     assert md[2] < 0.5
+
+
+def test_device_philox_known_answer_through_the_parameter_table():
+    """The device generator's first draw of realisation 0 with seed 0 is Philox-4x32-10 of the all-zero counter and key:
+    word 0 of the published vector (tests/golden/philox_kat.txt, 6627e8d5) fixes the receiver-noise scale
+    a = 100 (x + 1/2) 2^-32 exactly (one rounding, IEEE on both sides).  With seed = key (ffffffff, ffffffff) and the
+    pi vector no counter of the draw table matches, so those two stay CPU-side pins of the oracle, which the element by
+    element parity above ties to the device."""
+    _, _, tab, _ = rfi.sim42_generate(1, 1.0, seed=0, n_time=10, n_chan=8, n_sources=1, diagnostics=True)
+    torch.cuda.synchronize()
+    assert tab[0].a == 100.0 * ((0x6627E8D5 + 0.5) * 2.0 ** -32)
+    # words 0..3 of that vector drive (u, v) through the next call's pair as well: against the oracle's own draw
+    p = so.draw_params(so.Sim42Config(n_time=10, n_chan=8, n_real=1, n_sources=1, inr=1.0, seed=0), 0)
+    assert p["a"] == tab[0].a
