@@ -8,7 +8,9 @@ seeded synthetic correlator output that is already resident in HBM.  The default
 BASELINE.json configs[1] (LOFAR-subband-scale fp32, 18.5 GB, far larger than the 126 MB L2, so no cache
 flush is needed between iterations).  One JSON line is printed by rank 0 (see README / DESIGN.md for keys).
 
-N > 1 (launched by torchrun): the path shards by baseline with no data-path collective (every cell is an
+N > 1: `python bench.py --gpus N` starts N ranks itself (torch.distributed.run, one process per GPU, rendezvous on
+127.0.0.1; it refuses a node with fewer than N GPUs), and it runs as one of the ranks when a launcher (the driver's
+torchrun command) has already set WORLD_SIZE.  The path shards by baseline with no data-path collective (every cell is an
 independent stream), so every rank processes its own chunk ("scaling": "weak"); the timed region
 is bracketed by a barrier and the time is the max over ranks.
 
@@ -713,6 +715,56 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def self_launch(args) -> int:
+    """`python bench.py --gpus N` without torchrun around it: start the N ranks here, one process per GPU, the way the
+    driver's own command does (torch.distributed.run, one node, rendezvous on 127.0.0.1), with the same arguments.
+    Returns the launcher's exit code.  Refuses, loudly, a box with fewer than N GPUs (--dry-launch needs none)."""
+    import socket
+    if not args.dry_launch:
+        import torch
+        found = torch.cuda.device_count() if torch.cuda.is_available() else 0
+        if found < args.gpus:
+            sys.stderr.write(f"bench.py: --gpus {args.gpus} needs {args.gpus} GPUs on this node, found {found}\n")
+            return 2
+    with socket.socket() as sk:                                # a free rendezvous port
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "INFO")                       # the communicator lines show which ranks / devices joined
+    env.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+    env.setdefault("OMP_NUM_THREADS", "1")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__), *sys.argv[1:]]
+    return subprocess.call(cmd, env=env)
+
+
+def run_dry_launch(args):
+    """--dry-launch: the N-rank plumbing of run_ours without a GPU (CPU test of the launcher): ranks join a gloo group,
+    take their share of the work from sharding.rank_work, reduce a time (MAX) and a sample count (SUM) with the helpers
+    the timed path uses, and rank 0 prints one JSON line."""
+    import torch.distributed as dist
+    from paper_2412_14775_b200 import sharding, synth
+    world, rank = int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("RANK", "0"))
+    if world > 1:
+        dist.init_process_group("gloo")
+    w = synth.WORKLOADS[args.workload]
+    work = sharding.rank_work(w.n_baselines, world, rank, args.scaling)
+    samples = w.n_time * work["b_count"] * w.n_chan
+    total = sharding.sum_scalar_over_ranks(samples)
+    slowest = sharding.max_over_ranks(1.0 + rank)              # stands in for the device-measured milliseconds
+    shares = [None] * world
+    if world > 1:
+        dist.all_gather_object(shares, work)
+    else:
+        shares = [work]
+    if rank == 0:
+        print(json.dumps({"dry_launch": True, "n_gpus": world, "scaling": args.scaling, "total_samples": total,
+                          "max_ms": slowest, "work": shares}))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -738,9 +790,18 @@ def main():
                     help="hold this false-alarm rate by on-line threshold adaptation (rfi_plan_set_adaptive, DESIGN.md NEXT-3)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--dry-launch", action="store_true",
+                    help="exercise the N-rank launch and the rank bookkeeping on CPU (gloo), no kernels: tests/test_sharding.py")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
-    if args.impl == "reference":
+    world_env = os.environ.get("WORLD_SIZE")
+    if args.impl == "ours" and args.gpus > 1 and world_env is None:
+        sys.exit(self_launch(args))                            # not under torchrun: start the N ranks ourselves
+    if args.impl == "ours" and world_env is not None and int(world_env) != args.gpus:
+        sys.exit(f"bench.py: --gpus {args.gpus} but the launcher started WORLD_SIZE = {world_env} ranks")
+    if args.dry_launch:
+        run_dry_launch(args)
+    elif args.impl == "reference":
         run_reference(args)
     elif args.workload == "sim42":
         if args.K <= 1:

@@ -88,3 +88,40 @@ def test_world_size_2_gloo_partition_and_reductions(tmp_path):
     mp.spawn(_worker, args=(world, _free_port(), 15, 4, 6, 3, str(tmp_path)), nprocs=world, join=True)
     parts = [np.load(tmp_path / f"ok{r}.npy") for r in range(world)]
     assert parts[0].tolist() == [0, 8] and parts[1].tolist() == [8, 7]
+
+
+# ---- bench.py --gpus N starts its own ranks; the plumbing on CPU through --dry-launch -------------------
+def _bench(*argv, env_extra=None):
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    env.update(env_extra or {})
+    return subprocess.run([sys.executable, os.path.join(root, "bench.py"), *argv], capture_output=True, text=True, env=env,
+                          cwd=root, timeout=600)
+
+
+@pytest.mark.parametrize("scaling", ["weak", "strong"])
+def test_bench_gpus_2_launches_two_ranks_by_itself(scaling):
+    import json
+    res = _bench("--gpus", "2", "--dry-launch", "--scaling", scaling)
+    assert res.returncode == 0, res.stderr[-3000:]
+    lines = [json.loads(l) for l in res.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1, res.stdout                                                 # rank 0 alone prints
+    rec = lines[0]
+    assert rec["dry_launch"] and rec["n_gpus"] == 2 and rec["scaling"] == scaling and rec["max_ms"] == 2.0
+    want = [sharding.rank_work(1176, 2, r, scaling) for r in range(2)]
+    assert rec["work"] == want
+    cells = 1176 * 64 * 7680                                                           # the lofar chunk (BASELINE.json configs[1])
+    assert rec["total_samples"] == (2 * cells if scaling == "weak" else cells)
+
+
+def test_bench_refuses_more_gpus_than_the_node_has():
+    n = (torch.cuda.device_count() if torch.cuda.is_available() else 0) + 1
+    res = _bench("--gpus", str(max(n, 2)), "--steps", "1")
+    assert res.returncode != 0 and "GPUs on this node, found" in res.stderr
+
+
+def test_bench_refuses_a_world_size_that_contradicts_gpus():
+    res = _bench("--gpus", "2", "--dry-launch", env_extra={"WORLD_SIZE": "3", "RANK": "0"})
+    assert res.returncode != 0 and "WORLD_SIZE = 3" in res.stderr
