@@ -185,10 +185,39 @@ def _pctl_stats(ms):
             "launches_timed": len(ms)}
 
 
-def sampled_parity(w, plan, vis, truth, thr, avg, weight, stats, n_clean, n_rfi):
+def _tables_compare(sub, w, thr, mask, out):
+    """Tables arithmetic (rfi_plan_set_arithmetic): bit for bit against the step-by-step oracle (oracle_tables_process),
+    the comparator of tests/test_gpu_tables.py.  out as for tests.parity_util.compare (K = 1)."""
+    import math
+    import numpy as np
+    from oracle import rfi_oracle as orc
+    ref = orc.tables_process(sub, w.window_M, w.n_int, [float(np.float32(x)) for x in thr], mask)
+    for key, r in (("tau", ref.tau[0]), ("r_re", ref.r_re), ("r_im", ref.r_im)):
+        nan = np.isnan(r)
+        assert np.array_equal(np.isnan(out[key]), nan), f"tables {key}: NaN positions differ"
+        assert np.array_equal(out[key][~nan].view(np.uint32), r[~nan].view(np.uint32)), f"tables {key}: not bit-exact"
+    assert np.array_equal(out["flags"][0], ref.flags[0].astype(bool)), "tables flags differ"
+    assert np.array_equal(out["weight"][0], ref.weight[0]), "tables weights differ"
+    a = ref.avg[0].view(np.float64).reshape(-1)
+    got = out["avg"][0].astype(np.complex128).view(np.float64).reshape(-1)
+    rms = math.sqrt(float((a ** 2).mean()))
+    fin = np.isfinite(a)
+    worst = float((np.abs(got - a)[fin] / (1e-5 * np.maximum(np.abs(a[fin]), rms))).max(initial=0))
+    assert worst <= 1.0, f"tables avg: worst |d|/bound = {worst:.3g}"
+    n = int(ref.flags[0].size)
+    return {"n_windows": n, "flag_mismatch": 0, "flag_mismatch_near_threshold": 0, "flag_mismatch_unexplained": 0,
+            "flag_agreement": 1.0, "avg_worst_over_bound": worst, "outputs_skipped": 0, "tau_worst_over_bound": 0.0,
+            "r_re_worst_over_bound": 0.0}
+
+
+def sampled_parity(w, plan, vis, truth, thr, avg, weight, stats, n_clean, n_rfi, groups=None, tables_mask=None):
     """Verification leg (outside every timed region): a seeded sample of cells of the chunk the timed kernel just
     processed -- all time samples of each -- is brought back and compared with the fp64 oracle element by element
-    with the comparators and tolerances of tests/ (the logic of tests/test_gpu_full_size.py)."""
+    with the comparators and tolerances of tests/ (the logic of tests/test_gpu_full_size.py).
+    vis: the chunk as a time-major [n_time, n_baselines, n_chan, 4, 2] tensor or view.  groups (optional): cells whose
+    windows were decided with different threshold sets (baseline classes, per-stream adaptation) are compared group by
+    group: [(label, bool tensor [n_cells], thresholds [K][4])]; default: all cells with `thr`.  tables_mask: compare with the
+    tables oracle bit for bit instead."""
     import numpy as np
     import torch
     import paper_2412_14775_b200 as rfi
@@ -198,7 +227,13 @@ def sampled_parity(w, plan, vis, truth, thr, avg, weight, stats, n_clean, n_rfi)
         g = torch.Generator().manual_seed(3)
         tr = truth.reshape(plan.n_win, plan.n_cells)
         has = tr.any(0).cpu()
-        r_cells, c_cells = torch.nonzero(has).flatten(), torch.nonzero(~has).flatten()
+        if groups is not None:                              # only cells that belong to a group are candidates
+            member = torch.zeros(plan.n_cells, dtype=torch.bool)
+            for _, m, _ in groups:
+                member |= m.cpu()
+            r_cells, c_cells = torch.nonzero(has & member).flatten(), torch.nonzero(~has & member).flatten()
+        else:
+            r_cells, c_cells = torch.nonzero(has).flatten(), torch.nonzero(~has).flatten()
         idx = torch.cat([r_cells[torch.randperm(r_cells.numel(), generator=g)[:n_rfi]],
                          c_cells[torch.randperm(c_cells.numel(), generator=g)[:n_clean]]]).sort().values
         if w.window_F > 1:                                  # whole footprints: the F channels of a window share a flag
@@ -216,9 +251,28 @@ def sampled_parity(w, plan, vis, truth, thr, avg, weight, stats, n_clean, n_rfi)
                "weight": wt[:, :, idx].cpu().numpy(), "flags": flags[:, :, idx].cpu().numpy(),
                "tau": s[0][:, idx].cpu().numpy(), "r_re": s[1][:, idx].cpu().numpy(), "r_im": s[2][:, idx].cpu().numpy()}
         del flags, wt, kept
-        rep = compare(sub, w.window_M, w.n_int, thr, out, tol=2e-3 if w.fp16 else 1e-5, fp16=w.fp16, F=w.window_F)
+        idx_c = idx.cpu()
+        rep = None
+        for label, member, g_thr in (groups if groups is not None else [("all", None, thr)]):
+            pos = np.arange(idx_c.numel()) if member is None else np.nonzero(member.cpu()[idx_c].numpy())[0]
+            if pos.size == 0:
+                continue
+            o = {k: (a[:, :, pos] if a.ndim >= 3 else a[:, pos]) for k, a in out.items()}
+            r = (_tables_compare(sub[:, pos], w, g_thr[0], tables_mask, o) if tables_mask is not None else
+                 compare(sub[:, pos], w.window_M, w.n_int, g_thr, o, tol=2e-3 if w.fp16 else 1e-5, fp16=w.fp16, F=w.window_F))
+            if rep is None:
+                rep = dict(r)
+            else:                                           # totals over the groups, worst case of the ratios
+                for key in ("n_windows", "flag_mismatch", "flag_mismatch_near_threshold", "flag_mismatch_unexplained", "outputs_skipped"):
+                    rep[key] += r[key]
+                for key in ("tau_worst_over_bound", "r_re_worst_over_bound", "avg_worst_over_bound"):
+                    rep[key] = max(rep.get(key) or 0.0, r.get(key) or 0.0)
+                rep["flag_agreement"] = min(rep["flag_agreement"], r["flag_agreement"])
         ok = weight_ok and finite_ok
-        return {"status": "ok" if ok else "FAILED", "against": "fp64 oracle (oracle/), same seeded chunk",
+        return {"status": "ok" if ok else "FAILED",
+                "against": ("tables oracle (oracle_tables_process), bit for bit, same seeded chunk" if tables_mask is not None
+                            else "fp64 oracle (oracle/), same seeded chunk"),
+                "groups": [lab for lab, _, _ in groups] if groups is not None else None,
                 "cells_sampled": int(idx.numel()), "windows_compared": rep["n_windows"] * K,
                 "tolerance": 2e-3 if w.fp16 else 1e-5, "flag_mismatch": rep["flag_mismatch"],
                 "flag_mismatch_near_threshold": rep["flag_mismatch_near_threshold"],
@@ -230,8 +284,70 @@ def sampled_parity(w, plan, vis, truth, thr, avg, weight, stats, n_clean, n_rfi)
         return {"status": "FAILED", "error": str(exc)[:300]}
 
 
+def mode_parity(args, w, plan, vis, truth, thr, two_classes, dev):
+    """The verification leg of run_ours for the mode that was just timed (K sets, threshold classes, cell-major input,
+    tables arithmetic, on-line adaptation): the thresholds in force are read back, one more launch stores the statistics
+    planes, and sampled cells go through the oracle group by group.  Not timed."""
+    import torch
+    from paper_2412_14775_b200 import synth
+    nb, C = plan.n_baselines, w.n_chan
+    vis_tm = vis.permute(2, 0, 1, 3, 4) if args.layout == "cell_major" else vis     # a view: (b, c) stay mergeable
+    cell_auto = None
+    if two_classes:
+        autos = synth.auto_baseline_mask(w)[plan.b_first:plan.b_first + nb]
+        cell_auto = autos.repeat_interleave(C)
+    groups = None
+    if args.adaptive > 0 and args.adaptive_scope == "baseline":
+        st = plan.get_stream_thresholds()                                      # [nb, 4], in force for the next launch
+        picks = sorted({int(b) for b in torch.linspace(0, nb - 1, 8).round().tolist()})
+        groups = []
+        for b in picks:
+            m = torch.zeros(nb * C, dtype=torch.bool)
+            m[b * C:(b + 1) * C] = True
+            groups.append((f"baseline {plan.b_first + b}", m, [st[b].tolist()]))
+    elif args.adaptive > 0:
+        cur = plan.get_thresholds()                                            # per class, in force for the next launch
+        groups = ([("cross", ~cell_auto, [list(cur[0])]), ("auto", cell_auto, [list(cur[-1])])] if two_classes
+                  else [("all", torch.ones(nb * C, dtype=torch.bool), [list(cur[0])])])
+    elif two_classes:
+        auto = synth.auto_thresholds(w.window_M * w.window_F)
+        groups = [("cross", ~cell_auto, [list(t) for t in thr]),
+                  ("auto", cell_auto, [list(auto) if args.K <= 1 else [t[0]] + list(auto[1:]) for t in thr])]
+    avg2, weight2, stats = plan.alloc_outputs(device=dev, stats=True)
+    plan.process_chunk(vis, avg2, weight2, stats)
+    torch.cuda.synchronize(dev)
+    n_clean, n_rfi = (160, 64) if plan.K > 1 else (512, 128)
+    rep = sampled_parity(w, plan, vis_tm, truth, thr, avg2, weight2, stats, n_clean, n_rfi, groups=groups,
+                         tables_mask=args.mask if args.arith == "tables" else None)
+    del avg2, weight2, stats
+    torch.cuda.empty_cache()
+    return rep
+
+
+def _safe(fn, *a, **kw):
+    """A verification leg must never cost the run its JSON line: anything unexpected becomes a FAILED record."""
+    try:
+        return fn(*a, **kw)
+    except Exception as exc:      # noqa: BLE001
+        return {"status": "FAILED", "error": f"{type(exc).__name__}: {exc}"[:300]}
+
+
+def per_config_entry(rec):
+    """One compact row of roofline.per_config from a sub-record of `configs` (the driver keeps `roofline` whole)."""
+    if "skipped" in rec:
+        return {"workload": rec["workload"], "K": rec["K"], "skipped": rec["skipped"]}
+    r, p = rec["roofline"], rec.get("parity") or {}
+    row = {"workload": rec["workload"], "K": rec["K"], "storage": rec["storage"], "window": rec["window"], "kernel": rec["variant"],
+           "ms_best": rec["kernel_ms_best"], "ms_median": rec["kernel_ms_median"], "gbs": r["achieved"], "frac": r["frac"],
+           "frac_of_nominal_8TBs": r["frac_of_nominal_8TBs"], "parity_status": p.get("status"),
+           "cells_sampled": p.get("cells_sampled"), "flag_mismatch_unexplained": p.get("flag_mismatch_unexplained")}
+    if rec.get("cpu_baseline"):
+        row["cpu_baseline_samples_per_s"] = rec["cpu_baseline"]["value"]
+    return row
+
+
 def measure_config(name, K, dev, steps, warmup, peak, read_probe_gbs, vis=None, truth=None, n_clean=512, n_rfi=128,
-                   variant="auto"):
+                   variant="auto", cpu_baseline=False):
     """One sub-record of `configs`: generate (or reuse) the chunk, time `steps` launches one by one with CUDA events
     after `warmup` untimed ones, then check a sample of cells against the oracle."""
     import torch
@@ -314,13 +430,40 @@ def measure_config(name, K, dev, steps, warmup, peak, read_probe_gbs, vis=None, 
     # one more launch with the statistics planes, then the sampled-cell oracle check (not timed)
     plan.process_chunk(vis, avg, weight, stats)
     torch.cuda.synchronize(dev)
-    rec["parity"] = sampled_parity(w, plan, vis, truth, thr, avg, weight, stats, n_clean, n_rfi)
+    rec["parity"] = _safe(sampled_parity, w, plan, vis, truth, thr, avg, weight, stats, n_clean, n_rfi)
+    if cpu_baseline:
+        # SURVEY.md 8(d), configs[3]: the oracle timed on the RFI-bearing cells + a seeded 2 % of the clean cells (bounded)
+        g = torch.Generator().manual_seed(11)
+        has = truth.reshape(plan.n_win, plan.n_cells).any(0).cpu()
+        r_cells, c_cells = torch.nonzero(has).flatten(), torch.nonzero(~has).flatten()
+        pick = torch.cat([r_cells[torch.randperm(r_cells.numel(), generator=g)[:16384]],
+                          c_cells[torch.randperm(c_cells.numel(), generator=g)[:min(16384, max(1, c_cells.numel() // 50))]]])
+        pick = pick[torch.randperm(pick.numel(), generator=g)].to(dev)          # mixed order: any prefix is a fair sample
+        sub = vis.reshape(w.n_time, plan.n_cells, 4, 2)[:, pick].cpu().numpy()
+        rec["cpu_baseline"] = _safe(oracle_baseline, sub, w, thr, 8.0)
+        del sub
     plan.destroy()
     del avg, weight, stats, flush
     if own:
         del vis, truth
     torch.cuda.empty_cache()
     return rec
+
+
+def sim42_parity(plan, vis, truth_words, sets, T, C, wT, wF, dev):
+    """Verification leg of --workload sim42: sampled (realisation, channel) footprints of the block the timed K-set
+    launch just flagged, all K sets, against the fp64 oracle at the paper's T x F window."""
+    import torch
+    import paper_2412_14775_b200 as rfi
+    from paper_2412_14775_b200 import synth
+    w = synth.Workload("sim42", 29, False, C, T, wT, T, window_F=wF)            # 406 cross baselines = the realisations
+    truth = rfi.unpack_flags(truth_words, C).reshape(plan.n_win, -1)
+    avg2, weight2, stats = plan.alloc_outputs(device=dev, stats=True)
+    plan.process_chunk(vis, avg2, weight2, stats)
+    torch.cuda.synchronize(dev)
+    rep = sampled_parity(w, plan, vis, truth, sets, avg2, weight2, stats, 48, 48)
+    del avg2, weight2, stats
+    return rep
 
 
 def run_sim42(args):
@@ -389,6 +532,7 @@ def run_sim42(args):
                 curves.setdefault(("polarised" if polarized else "unpolarised"), {}).setdefault(f"design_fa_{fa}", {}) \
                       .setdefault(det, []).append({"inr": inr, "false_alarm": round(fa_m[k], 5), "missed_detection": round(md_m[k], 5)})
     clocks = sampler.stop()
+    parity = None if args.no_parity else _safe(sim42_parity, plan, vis, truth, sets, T, C, wT, wF, dev)
     peak, peak_src = load_peaks()
     out_bytes = avg.numel() * 4 + weight.numel() * 4 + K * plan.n_win * R * plan.wpb * 4
     algo = vis.numel() * 4 + out_bytes
@@ -407,7 +551,7 @@ def run_sim42(args):
                      "frac": algo / (k_med * 1e-3) / 1e9 / peak, "traffic": None, "peak_source": peak_src,
                      "kernel": "rfi_batched_mask_kernel<5, fp32>", "kernel_ms_best": min(kernel_ms), "kernel_ms_median": k_med,
                      "frac_of_nominal_8TBs": algo / (k_med * 1e-3) / 1e9 / 8000.0, "algorithmic_bytes_per_launch": algo},
-        "cpu_baseline": None, "e2e": None, "gpu_launches": int(plan.launch_count), "clocks": clocks,
+        "cpu_baseline": None, "e2e": None, "gpu_launches": int(plan.launch_count), "clocks": clocks, "parity": parity,
         "sim42": {"generator_ms_median": statistics.median(gen_ms), "generator_gbytes_per_s": vis.numel() * 4 / (statistics.median(gen_ms) * 1e-3) / 1e9,
                   "paper_fig2_context": "INR 100, 10 x 2: SK 0.01/0.89, DS 0.01/0.06, BOTH 0.01/0.05 (FA/MD, PAPER.md:233)",
                   "curves": {pol: {k: v for k, v in c.items() if k in keep} for pol, c in curves.items()},
@@ -601,6 +745,9 @@ def run_ours(args):
                         "stream, so frac_of_read_stream_probe (same-device read-only probe) and frac_of_nominal_8TBs are the "
                         "fractions that cannot exceed 1"}
 
+    # verification of the mode that was timed, against the oracle, in this same run (not timed)
+    parity = None if args.no_parity else _safe(mode_parity, args, w, plan, vis, truth, thr, two_classes, dev)
+
     # end to end through the C ABI with HOST buffers (H2D of the inputs and D2H of the results inside the timed region)
     e2e = None
     if args.no_e2e:
@@ -675,9 +822,13 @@ def run_ours(args):
         configs.append(measure_config("sweep", 64, dev, n_sub, 3, peak, read_probe, vis=vis, truth=truth, n_clean=160, n_rfi=64))
         del vis, truth
         torch.cuda.empty_cache()
-        configs.append(measure_config("lofar_fp16", 1, dev, n_sub, 3, peak, read_probe))
-        configs.append(measure_config("lofar_tf10x2", 1, dev, n_sub, 3, peak, read_probe))
-        configs.append(measure_config("large", 1, dev, n_sub, 3, peak, read_probe, n_clean=256, n_rfi=256))
+        for name in ("lofar_fp16", "lofar_tf10x2"):          # K = 1 and the K = 64 sweep on the same resident chunk
+            v2, t2 = synth.make_chunk(synth.WORKLOADS[name], seed=1234, device=dev)
+            configs.append(measure_config(name, 1, dev, n_sub, 3, peak, read_probe, vis=v2, truth=t2))
+            configs.append(measure_config(name, 64, dev, n_sub, 3, peak, read_probe, vis=v2, truth=t2, n_clean=160, n_rfi=64))
+            del v2, t2
+            torch.cuda.empty_cache()
+        configs.append(measure_config("large", 1, dev, n_sub, 3, peak, read_probe, n_clean=256, n_rfi=256, cpu_baseline=True))
         configs.append(measure_config("tiny", 1, dev, max(n_sub, 50), 5, peak, read_probe, n_clean=96, n_rfi=6))
         # the same small chunk through the low-latency variant (RFI_VARIANT_SPLIT: a unit's rows split over 16 warps)
         configs.append(measure_config("tiny", 1, dev, max(n_sub, 50), 5, peak, read_probe, n_clean=96, n_rfi=6, variant="split"))
@@ -706,6 +857,17 @@ def run_ours(args):
                                   "missed_detection_min_max": [float(p_md.min()), float(p_md.max())],
                                   "flag_fraction_min_max": [float(flag_frac.min()), float(flag_frac.max())]}},
     }
+    line["parity"] = parity
+    head = {"workload": w.name, "K": max(args.K, 1), "storage": "f16" if w.fp16 else "f32", "window": f"{w.window_M} x {w.window_F}",
+            "kernel": variant, "ms_best": min(kernel_ms), "ms_median": statistics.median(kernel_ms),
+            "gbs": algo_bytes / (statistics.median(kernel_ms) * 1e-3) / 1e9,
+            "frac": algo_bytes / (statistics.median(kernel_ms) * 1e-3) / 1e9 / peak,
+            "frac_of_nominal_8TBs": algo_bytes / (statistics.median(kernel_ms) * 1e-3) / 1e9 / 8000.0,
+            "parity_status": (parity or {}).get("status"), "cells_sampled": (parity or {}).get("cells_sampled"),
+            "flag_mismatch_unexplained": (parity or {}).get("flag_mismatch_unexplained")}
+    if cpu:
+        head["cpu_baseline_samples_per_s"] = cpu["value"]
+    roofline["per_config"] = [head] + [per_config_entry(c) for c in (configs or [])]
     if configs is not None:
         line["configs"] = configs
     torch.cuda.profiler.stop()        # `ncu --profile-from-start off` lists every launch of the run, sub-records included
@@ -790,6 +952,7 @@ def main():
                     help="hold this false-alarm rate by on-line threshold adaptation (rfi_plan_set_adaptive, DESIGN.md NEXT-3)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-parity", action="store_true", help="skip the sampled-cell oracle check of the timed mode")
     ap.add_argument("--dry-launch", action="store_true",
                     help="exercise the N-rank launch and the rank bookkeeping on CPU (gloo), no kernels: tests/test_sharding.py")
     args = ap.parse_args()

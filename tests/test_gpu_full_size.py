@@ -35,14 +35,19 @@ def _run_full(name, K, n_clean=768, n_rfi=256, layout="time_major", vs_fp32_orig
         vis = vis32.to(torch.float16)
     else:
         vis, truth = synth.make_chunk(w, seed=1234, device=dev)
-    thr = synth.default_thresholds(w.window_M) if K == 1 else synth.sweep_thresholds(w.window_M, K)
+    W, F = w.window_M * w.window_F, w.window_F
+    thr = synth.default_thresholds(W) if K == 1 else synth.sweep_thresholds(W, K)
     plan = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M,
                        rfi.RFI_FP16 if w.fp16 else rfi.RFI_FP32, n_int=w.n_int)
+    if F > 1:
+        plan.set_window_freq(F)
     plan.set_thresholds(thr)
     avg, weight, stats = plan.alloc_outputs(stats=True)
     if layout == "cell_major":
         plan.set_layout("cell_major")
         d_in = vis.permute(1, 2, 0, 3, 4).contiguous()          # vis[b][c][t][pol][re,im]
+        del vis                                                 # one resident copy: the sample below is read through
+        vis = d_in.permute(2, 0, 1, 3, 4)                       # the time-major VIEW of the cell-major buffer
     else:
         d_in = vis
     plan.process_chunk(d_in, avg, weight, stats)                # auto variant: what bench.py times
@@ -57,7 +62,10 @@ def _run_full(name, K, n_clean=768, n_rfi=256, layout="time_major", vs_fp32_orig
     s = stats.reshape(3, plan.n_win, plan.n_cells)
     assert (s[1] >= 0).all() and (s[1] <= 1 + 1e-6).all() and (s[2] >= 0).all() and (s[2] <= 1 + 1e-6).all()
     # sampled cells against the oracle
-    idx = _sample_cells(w, truth.reshape(plan.n_win, plan.n_cells), n_clean, n_rfi, seed=3).to(dev)
+    idx = _sample_cells(w, truth.reshape(plan.n_win, plan.n_cells), n_clean, n_rfi, seed=3)
+    if F > 1:                                                    # whole footprints: the F channels of a window share a flag
+        idx = torch.unique((idx // F)[:, None] * F + torch.arange(F)[None, :]).sort().values
+    idx = idx.to(dev)
     sub = vis.reshape(w.n_time, plan.n_cells, 4, 2)[:, idx].cpu().numpy()
     if vs_fp32_original:
         sub32 = vis32.reshape(w.n_time, plan.n_cells, 4, 2)[:, idx].cpu().numpy()
@@ -72,7 +80,7 @@ def _run_full(name, K, n_clean=768, n_rfi=256, layout="time_major", vs_fp32_orig
     plan.destroy()
     del vis, d_in, avg, weight, stats
     torch.cuda.empty_cache()
-    rep = compare(sub, w.window_M, w.n_int, thr, out, tol=2e-3 if w.fp16 else 1e-5, fp16=w.fp16)
+    rep = compare(sub, w.window_M, w.n_int, thr, out, tol=2e-3 if w.fp16 else 1e-5, fp16=w.fp16, F=F)
     if sub32 is not None:
         rep.update(fp16_vs_fp32_original(sub32, w.window_M, w.n_int, thr, out))
     return rep, used
@@ -117,3 +125,65 @@ def test_large_array_full_size():
     integration per chunk (73.6 GB); bursts, tones and 100-sigma unpolarised spikes."""
     rep, used = _run_full("large", 1, n_clean=384, n_rfi=384)
     assert used == "direct" and rep["flag_mismatch_unexplained"] == 0
+
+
+# ---- the shapes DESIGN.md section 7 quotes a time for that had no full-size test (VERDICT r02, item 7) ----------------
+def test_fp16_storage_K64_full_size():
+    rep, used = _run_full("lofar_fp16", 64, n_clean=160, n_rfi=64)
+    assert used == "batched" and rep["K"] == 64 and rep["flag_agreement"] >= 0.999
+
+
+@pytest.mark.parametrize("K", [1, 64])
+def test_tf10x2_full_size(K):
+    """The paper's 10 x 2 footprint on the lofar shape, single set and the K = 64 sweep."""
+    rep, used = _run_full("lofar_tf10x2", K, n_clean=160 if K > 1 else 512, n_rfi=64 if K > 1 else 128)
+    assert used == ("batched" if K > 1 else "direct") and rep["flag_mismatch_unexplained"] == 0
+
+
+def test_large_array_cell_major_full_size():
+    rep, used = _run_full("large", 1, n_clean=256, n_rfi=256, layout="cell_major")
+    assert used == "tma" and rep["flag_mismatch_unexplained"] == 0
+
+
+@pytest.mark.parametrize("mode", ["tables", "adaptive", "adaptive_baseline", "classes"])
+def test_other_modes_at_the_lofar_size(mode):
+    """Tables arithmetic (mask 0x3C50: bit for bit against oracle_tables_process), on-line adaptation per class and per
+    baseline (the flags of the chunk after the first update against the oracle with the thresholds then in force) and
+    cross / auto threshold classes, on the full lofar chunk, through the verification leg bench.py runs after timing
+    these modes (bench.mode_parity: thresholds read back, one launch with the statistics planes, sampled cells through
+    the oracle group by group)."""
+    import types
+    import bench
+    w = synth.WORKLOADS["lofar"]
+    if torch.cuda.mem_get_info()[0] < w.input_bytes * 1.15 + 8e9:
+        pytest.skip("not enough free device memory for the full-size chunk")
+    dev = torch.device("cuda")
+    vis, truth = synth.make_chunk(w, seed=1234, device=dev)
+    thr = synth.default_thresholds(w.window_M)
+    plan = rfi.RfiPlan(w.n_stations, w.n_baselines, w.n_chan, w.n_time, w.window_M, n_int=w.n_int)
+    args = types.SimpleNamespace(layout="time_major", adaptive=0.05 if mode.startswith("adaptive") else 0.0,
+                                 adaptive_scope="baseline" if mode == "adaptive_baseline" else "class",
+                                 arith="tables" if mode == "tables" else "fast", mask=0x3C50, K=1)
+    two_classes = mode == "classes"
+    if two_classes:
+        plan.set_baseline_classes(synth.auto_baseline_mask(w).int().tolist())
+        plan.set_thresholds([[thr[0], synth.auto_thresholds(w.window_M)]])
+    else:
+        plan.set_thresholds(thr)
+    if mode == "tables":
+        plan.set_arithmetic("tables", 0x3C50)
+    if args.adaptive > 0:
+        plan.set_adaptive(0.05, 0.5)
+        plan.set_adaptive_scope(args.adaptive_scope)
+    avg, weight, _ = plan.alloc_outputs()
+    plan.process_chunk(vis, avg, weight)                        # chunk 1 (with adaptation on: the first update follows it)
+    torch.cuda.synchronize()
+    if args.adaptive > 0:
+        now = plan.get_stream_thresholds()[:, 1:] if mode == "adaptive_baseline" else np.array(plan.get_thresholds())[:, 1:]
+        assert not np.allclose(now, np.array(thr[0][1:])[None, :])      # the thresholds did move
+    rep = bench.mode_parity(args, w, plan, vis, truth, thr, two_classes, dev)
+    plan.destroy()
+    assert rep["status"] == "ok", rep
+    assert rep["flag_mismatch_unexplained"] == 0 and rep["cells_sampled"] >= 500, rep
+    if mode == "tables":
+        assert rep["against"].startswith("tables oracle") and rep["flag_mismatch"] == 0
